@@ -1,0 +1,140 @@
+/*
+ * sg_b200.h -- C ABI of the B200-native spin-glass sweep library (libsg_b200.so).
+ *
+ * The library performs the Monte Carlo hot path of arXiv:1309.1599 (citations: PAPER.md:<line>):
+ * checkerboard heat-bath (Eq. (A1)) and overrelaxation (Eq. (A2))
+ * sweeps of unit 3-vector spins on an L^3 periodic lattice with one 3x3 coupling matrix per link
+ * (Eq. (1); local field: footnote 64), parallel-tempering swaps
+ * and the energy / overlap / k_min Fourier-mode reductions.  Every step runs in
+ * hand-written CUDA kernels for sm_100a; there is no CPU fallback: without a CUDA device every compute
+ * call returns SG_ECUDA.
+ *
+ * Conventions (DESIGN.md sections 2-3).
+ *   N = L^3, L even >= 2.  Site index i = x1 + L*(x2 + L*x3), colour (x1+x2+x3)&1.  S samples,
+ *   R replicas, T temperatures, C = R*T copies per sample, copy c = r*T + slot, P = R(R-1)/2 replica
+ *   pairs (a<b) in the order (0,1),(0,2),...,(R-2,R-1).  A PT sweep exchanges the *temperatures* of two
+ *   slots; spins never move.  temp_of_slot / slot_of_temp are the per-chain permutation and its inverse.
+ *
+ * Host-visible layouts are logical and fixed here; the device layout is private to the library.
+ *   couplings  float [3][N][3][3]   M[mu][i][a][b]: link (i, mu) joins i and i+e_mu, a acts on s_i
+ *   spins      float [C][3][N]      by slot
+ *
+ * Ownership.  The caller owns all device memory (one workspace of sg_workspace_bytes() bytes, 256-byte
+ * aligned, e.g. a torch tensor's data_ptr()) and the CUDA stream; the library never calls cudaMalloc for
+ * state and never frees caller memory.  Host input arrays are consumed before the call returns; host
+ * output arrays are caller-allocated.  Sweeps and PT are asynchronous on the stream; calls that return
+ * data to the host synchronise the stream.
+ *
+ * Errors.  Every call returns SG_OK (0) or a negative code; nothing is printed, nothing throws.
+ */
+#ifndef SG_B200_H
+#define SG_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sg_ctx sg_ctx; /* opaque; owns only small host book-keeping */
+
+typedef struct {
+    int32_t L;            /* lattice size, even, >= 2 */
+    int32_t n_samples;    /* S: disorder samples held by this context */
+    int32_t n_replicas;   /* R >= 1 */
+    int32_t n_temps;      /* T >= 1 */
+    int32_t first_sample; /* global number of local sample 0 (enters every Philox counter; lets ranks
+                             shard the samples and still draw the single-process numbers) */
+    int32_t reserved;     /* must be 0 */
+    uint64_t seed;        /* Philox key */
+} sg_shape;
+
+enum {
+    SG_OK = 0,
+    SG_EINVAL = -1, /* bad argument: odd or too small L, counts <= 0, non-finite or non-monotone betas,
+                       NULL where not allowed, sample out of range, workspace too small or misaligned */
+    SG_ESTATE = -2, /* a sample was used before sg_init_sample */
+    SG_ECUDA = -3   /* a CUDA call failed (no device, launch failure, ...); see sg_last_cuda_error */
+};
+
+/* coupling generator modes of sg_init_sample */
+enum {
+    SG_GEN_OFFDIAG_SYM = 0, /* M = a*1 + sigma_D * symmetric off-diagonal D, Gaussian (BASELINE configs) */
+    SG_GEN_PAPER_SYM6 = 1,  /* M = a*1 + sigma_D * symmetric D with six independent Gaussian elements    */
+    SG_GEN_GENERAL9 = 2,    /* nine independent Gaussian entries (non-symmetric)                         */
+    SG_GEN_BIMODAL = 3,     /* the paper's J = +-1, D^{ab} = +-sigma_D                                    */
+    SG_GEN_FERRO = 4        /* M = 1                                                                      */
+};
+
+enum { SG_KIND_OR = 0, SG_KIND_HB = 1 };
+
+/* Device bytes the caller must provide for `shape`; 0 if the shape is invalid. */
+size_t sg_workspace_bytes(const sg_shape* shape);
+
+/* Create a context.  betas: host double[T], finite, strictly monotone (neighbouring
+ * temperatures are adjacent entries).  dev_workspace: device pointer, 256-byte aligned, `bytes` >=
+ * sg_workspace_bytes(shape); its contents are overwritten.  cuda_stream: a cudaStream_t (may be NULL =
+ * the legacy default stream).  On success *out is the new context. */
+int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* dev_workspace, size_t bytes,
+              void* cuda_stream);
+int sg_destroy(sg_ctx* ctx);
+
+/* S0.  Sets the quenched couplings and the initial spins of local sample `sample` and
+ * resets its temperature assignment to the identity.
+ *   couplings == NULL: generated from (seed, first_sample+sample) with gen_mode / sigma_D;
+ *                else: host float [3][N][3][3], copied (gen_mode, sigma_D ignored).
+ *   spins     == NULL: uniform on S^2 from Philox stream 3; else host float [C][3][N], copied. */
+int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const float* couplings,
+                   const float* spins);
+
+/* S1 (Eq. (A2)).  n_sweeps full overrelaxation sweeps of every copy of every sample:
+ * colour 0 half-sweep then colour 1.  The last half-sweep also reduces the total energy of every copy. */
+int sg_sweep_or(sg_ctx* ctx, int n_sweeps);
+
+/* S2 (Eq. (A1)).  n_sweeps full heat-bath sweeps at each copy's current temperature;
+ * the HB counter advances by one per sweep.  Energies are reduced as in sg_sweep_or. */
+int sg_sweep_hb(sg_ctx* ctx, int n_sweeps);
+
+/* S4.  One parallel-tempering sweep of every chain (sample, replica): pairs t = 0..T-2 in
+ * order, Metropolis acceptance min(1, exp((beta_t - beta_{t+1})(E_i - E_j))) on the total energies, which
+ * are recomputed first if stale.  The PT counter advances by one. */
+int sg_pt_swap(sg_ctx* ctx);
+
+/* S3 + S5.  Host outputs (any may be NULL):
+ *   e  double [S][R][T]        H/N of the copy of replica r at temperature t
+ *   q0 double [S][P][T]        q^(0)   = sum_x s^a_x.s^b_x / N, both copies at temperature t
+ *   qk double [S][P][T][3][2]  q^(k_mu) = sum_x q_x exp(+i 2 pi x_mu / L) / N, (Re, Im), mu = 0,1,2
+ * Synchronises the stream. */
+int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk);
+
+/* ---- state access: tests, checkpoint / resume (all synchronise) ---- */
+int sg_get_spins(sg_ctx* ctx, int sample, float* out /* [C][3][N] */);
+int sg_set_spins(sg_ctx* ctx, int sample, const float* in /* [C][3][N] */);
+int sg_get_couplings(sg_ctx* ctx, int sample, float* out /* [3][N][3][3] */);
+int sg_get_perm(sg_ctx* ctx, int sample, int32_t* temp_of_slot /* [R][T] */, int32_t* slot_of_temp /* [R][T] */);
+int sg_set_perm(sg_ctx* ctx, int sample, const int32_t* temp_of_slot /* [R][T], a permutation per chain */);
+/* Total H of every slot, double [S][C]; recomputed if stale. */
+int sg_get_energies(sg_ctx* ctx, double* E);
+/* Test hook: overwrite the cached energies (marks them fresh), so that sg_pt_swap can be fed given values. */
+int sg_set_energies(sg_ctx* ctx, const double* E /* [S][C] */);
+int sg_get_counters(sg_ctx* ctx, uint64_t* hb_counter, uint64_t* pt_counter);
+int sg_set_counters(sg_ctx* ctx, uint64_t hb_counter, uint64_t pt_counter);
+/* One half-sweep of one colour (kind SG_KIND_OR / SG_KIND_HB) of every copy with the current HB counter,
+ * which is not advanced: repeated HB calls on one colour are draws in a fixed field. */
+int sg_halfsweep(sg_ctx* ctx, int kind, int colour);
+/* PT statistics since creation, uint64 [S][R][T-1] each (either may be NULL). */
+int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts);
+
+/* ---- utilities ---- */
+int sg_sync(sg_ctx* ctx);                       /* cudaStreamSynchronize on the context's stream        */
+uint64_t sg_kernel_launches(const sg_ctx* ctx); /* kernels launched by this context so far              */
+int sg_last_cuda_error(const sg_ctx* ctx);      /* cudaError_t of the last failed CUDA call, 0 if none  */
+const char* sg_strerror(int code);              /* static string for an SG_* code                       */
+/* Philox4x32-10 block on the host (the library's own implementation; known-answer tests). */
+void sg_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SG_B200_H */

@@ -1,0 +1,235 @@
+"""ctypes binding of libsg_b200.so: argument marshalling only -- every step of the path runs in the
+library's CUDA kernels.  torch is used for device memory (the workspace tensor) and the stream.
+Method names follow include/sg_b200.h (sg_init_sample -> init_sample, ...)."""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libsg_b200.so")
+
+GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2, 3, 4
+KIND_OR, KIND_HB = 0, 1
+SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
+
+# every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
+DECLARED_SYMBOLS = [
+    "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_sweep_or", "sg_sweep_hb",
+    "sg_pt_swap", "sg_measure", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
+    "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
+    "sg_halfsweep", "sg_pt_stats", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
+    "sg_philox4x32_10",
+]
+
+
+class SgShape(ctypes.Structure):
+    _fields_ = [("L", ctypes.c_int32), ("n_samples", ctypes.c_int32), ("n_replicas", ctypes.c_int32),
+                ("n_temps", ctypes.c_int32), ("first_sample", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("seed", ctypes.c_uint64)]
+
+
+class SgError(RuntimeError):
+    def __init__(self, code, what, cuda_error=0):
+        self.code, self.cuda_error = code, cuda_error
+        super().__init__("%s failed: %s (code %d, cudaError %d)" % (what, _strerror(code), code, cuda_error))
+
+
+_lib = None
+
+
+def load_library():
+    """Loads libsg_b200.so (built by paper_1309_1599_b200/build.py); fails loudly if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError("libsg_b200.so is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(_LIB_PATH)
+    vp, i, d = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    u64 = ctypes.c_uint64
+    shp = ctypes.POINTER(SgShape)
+    L.sg_workspace_bytes.argtypes = [shp]; L.sg_workspace_bytes.restype = ctypes.c_size_t
+    L.sg_create.argtypes = [ctypes.POINTER(vp), shp, vp, vp, ctypes.c_size_t, vp]; L.sg_create.restype = i
+    L.sg_destroy.argtypes = [vp]; L.sg_destroy.restype = i
+    L.sg_init_sample.argtypes = [vp, i, i, d, vp, vp]; L.sg_init_sample.restype = i
+    L.sg_sweep_or.argtypes = [vp, i]; L.sg_sweep_or.restype = i
+    L.sg_sweep_hb.argtypes = [vp, i]; L.sg_sweep_hb.restype = i
+    L.sg_pt_swap.argtypes = [vp]; L.sg_pt_swap.restype = i
+    L.sg_measure.argtypes = [vp, vp, vp, vp]; L.sg_measure.restype = i
+    L.sg_get_spins.argtypes = [vp, i, vp]; L.sg_get_spins.restype = i
+    L.sg_set_spins.argtypes = [vp, i, vp]; L.sg_set_spins.restype = i
+    L.sg_get_couplings.argtypes = [vp, i, vp]; L.sg_get_couplings.restype = i
+    L.sg_get_perm.argtypes = [vp, i, vp, vp]; L.sg_get_perm.restype = i
+    L.sg_set_perm.argtypes = [vp, i, vp]; L.sg_set_perm.restype = i
+    L.sg_get_energies.argtypes = [vp, vp]; L.sg_get_energies.restype = i
+    L.sg_set_energies.argtypes = [vp, vp]; L.sg_set_energies.restype = i
+    L.sg_get_counters.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]; L.sg_get_counters.restype = i
+    L.sg_set_counters.argtypes = [vp, u64, u64]; L.sg_set_counters.restype = i
+    L.sg_halfsweep.argtypes = [vp, i, i]; L.sg_halfsweep.restype = i
+    L.sg_pt_stats.argtypes = [vp, vp, vp]; L.sg_pt_stats.restype = i
+    L.sg_sync.argtypes = [vp]; L.sg_sync.restype = i
+    L.sg_kernel_launches.argtypes = [vp]; L.sg_kernel_launches.restype = u64
+    L.sg_last_cuda_error.argtypes = [vp]; L.sg_last_cuda_error.restype = i
+    L.sg_strerror.argtypes = [i]; L.sg_strerror.restype = ctypes.c_char_p
+    L.sg_philox4x32_10.argtypes = [ctypes.POINTER(ctypes.c_uint32)] * 3; L.sg_philox4x32_10.restype = None
+    _lib = L
+    return L
+
+
+def _strerror(code):
+    return load_library().sg_strerror(int(code)).decode()
+
+
+def _ptr(a):
+    return ctypes.c_void_p(a.ctypes.data) if a is not None else None
+
+
+def workspace_bytes(L, n_samples, n_replicas, n_temps, seed=0, first_sample=0):
+    shape = SgShape(L, n_samples, n_replicas, n_temps, first_sample, 0, seed)
+    return int(load_library().sg_workspace_bytes(ctypes.byref(shape)))
+
+
+def philox4x32_10(ctr, key):
+    c = (ctypes.c_uint32 * 4)(*[int(v) for v in ctr]); k = (ctypes.c_uint32 * 2)(*[int(v) for v in key])
+    o = (ctypes.c_uint32 * 4)()
+    load_library().sg_philox4x32_10(c, k, o)
+    return [int(v) for v in o]
+
+
+class SpinGlass:
+    """One context of the C-ABI library on the current CUDA device and torch's current stream."""
+
+    def __init__(self, L, n_samples, n_replicas, n_temps, betas, seed=1, first_sample=0, device=None, stream=None):
+        import torch
+        self._lib = load_library()
+        self.L, self.S, self.R, self.T = int(L), int(n_samples), int(n_replicas), int(n_temps)
+        self.N, self.C, self.P = self.L ** 3, self.R * self.T, self.R * (self.R - 1) // 2
+        self.shape = SgShape(self.L, self.S, self.R, self.T, int(first_sample), 0, int(seed))
+        nbytes = int(self._lib.sg_workspace_bytes(ctypes.byref(self.shape)))
+        if nbytes == 0:
+            raise SgError(SG_EINVAL, "sg_workspace_bytes")
+        if not torch.cuda.is_available():
+            raise SgError(SG_ECUDA, "sg_create (no CUDA device; there is no CPU fallback)")
+        self.device = torch.device(device if device is not None else "cuda:%d" % torch.cuda.current_device())
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        aligned = (base + 255) & ~255
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        betas = np.ascontiguousarray(betas, dtype=np.float64)
+        if betas.shape != (self.T,):
+            raise SgError(SG_EINVAL, "sg_create (betas must have n_temps entries)")
+        self._ctx = ctypes.c_void_p()
+        rc = self._lib.sg_create(ctypes.byref(self._ctx), ctypes.byref(self.shape), _ptr(betas), ctypes.c_void_p(aligned),
+                                 nbytes, ctypes.c_void_p(self.stream.cuda_stream))
+        if rc != SG_OK:
+            self._ctx = None
+            raise SgError(rc, "sg_create")
+        self.workspace_bytes = nbytes
+
+    def _check(self, rc, what):
+        if rc != SG_OK:
+            raise SgError(rc, what, self._lib.sg_last_cuda_error(self._ctx))
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            self._lib.sg_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- the five calls of the north star ----
+    def init_sample(self, sample, gen_mode=GEN_OFFDIAG_SYM, sigma_D=1.0, couplings=None, spins=None):
+        if couplings is not None:
+            couplings = np.ascontiguousarray(couplings, dtype=np.float32)
+            assert couplings.size == 27 * self.N
+        if spins is not None:
+            spins = np.ascontiguousarray(spins, dtype=np.float32)
+            assert spins.size == 3 * self.N * self.C
+        self._check(self._lib.sg_init_sample(self._ctx, int(sample), int(gen_mode), float(sigma_D), _ptr(couplings),
+                                             _ptr(spins)), "sg_init_sample")
+
+    def sweep_or(self, n_sweeps=1):
+        self._check(self._lib.sg_sweep_or(self._ctx, int(n_sweeps)), "sg_sweep_or")
+
+    def sweep_hb(self, n_sweeps=1):
+        self._check(self._lib.sg_sweep_hb(self._ctx, int(n_sweeps)), "sg_sweep_hb")
+
+    def pt_swap(self):
+        self._check(self._lib.sg_pt_swap(self._ctx), "sg_pt_swap")
+
+    def measure(self):
+        e = np.empty((self.S, self.R, self.T)); q0 = np.empty((self.S, self.P, self.T))
+        qk = np.empty((self.S, self.P, self.T, 3, 2))
+        self._check(self._lib.sg_measure(self._ctx, _ptr(e), _ptr(q0), _ptr(qk)), "sg_measure")
+        return e, q0, qk
+
+    def unit(self, n_or):
+        """One MCS: 1 HB sweep, n_or OR sweeps, 1 PT sweep."""
+        self.sweep_hb(1)
+        self.sweep_or(n_or)
+        self.pt_swap()
+
+    # ---- state access ----
+    def get_spins(self, sample):
+        out = np.empty((self.C, 3, self.N), dtype=np.float32)
+        self._check(self._lib.sg_get_spins(self._ctx, int(sample), _ptr(out)), "sg_get_spins")
+        return out
+
+    def set_spins(self, sample, spins):
+        spins = np.ascontiguousarray(spins, dtype=np.float32)
+        assert spins.size == 3 * self.N * self.C
+        self._check(self._lib.sg_set_spins(self._ctx, int(sample), _ptr(spins)), "sg_set_spins")
+
+    def get_couplings(self, sample):
+        out = np.empty((3, self.N, 3, 3), dtype=np.float32)
+        self._check(self._lib.sg_get_couplings(self._ctx, int(sample), _ptr(out)), "sg_get_couplings")
+        return out
+
+    def get_perm(self, sample):
+        tos = np.empty((self.R, self.T), dtype=np.int32); sot = np.empty((self.R, self.T), dtype=np.int32)
+        self._check(self._lib.sg_get_perm(self._ctx, int(sample), _ptr(tos), _ptr(sot)), "sg_get_perm")
+        return tos, sot
+
+    def set_perm(self, sample, temp_of_slot):
+        tos = np.ascontiguousarray(temp_of_slot, dtype=np.int32)
+        assert tos.shape == (self.R, self.T)
+        self._check(self._lib.sg_set_perm(self._ctx, int(sample), _ptr(tos)), "sg_set_perm")
+
+    def get_energies(self):
+        E = np.empty((self.S, self.C))
+        self._check(self._lib.sg_get_energies(self._ctx, _ptr(E)), "sg_get_energies")
+        return E
+
+    def set_energies(self, E):
+        E = np.ascontiguousarray(E, dtype=np.float64)
+        assert E.shape == (self.S, self.C)
+        self._check(self._lib.sg_set_energies(self._ctx, _ptr(E)), "sg_set_energies")
+
+    def get_counters(self):
+        hb, pt = ctypes.c_uint64(), ctypes.c_uint64()
+        self._check(self._lib.sg_get_counters(self._ctx, ctypes.byref(hb), ctypes.byref(pt)), "sg_get_counters")
+        return int(hb.value), int(pt.value)
+
+    def set_counters(self, hb, pt):
+        self._check(self._lib.sg_set_counters(self._ctx, int(hb), int(pt)), "sg_set_counters")
+
+    def halfsweep(self, kind, colour):
+        self._check(self._lib.sg_halfsweep(self._ctx, int(kind), int(colour)), "sg_halfsweep")
+
+    def pt_stats(self):
+        n = max(self.T - 1, 1)
+        att = np.zeros((self.S, self.R, n), dtype=np.uint64); acc = np.zeros((self.S, self.R, n), dtype=np.uint64)
+        self._check(self._lib.sg_pt_stats(self._ctx, _ptr(att), _ptr(acc)), "sg_pt_stats")
+        return att, acc
+
+    def sync(self):
+        self._check(self._lib.sg_sync(self._ctx), "sg_sync")
+
+    def kernel_launches(self):
+        return int(self._lib.sg_kernel_launches(self._ctx))

@@ -1,0 +1,600 @@
+// sg_api.cu -- host side of libsg_b200: the C ABI of include/sg_b200.h.
+// Context book-keeping, workspace carving, the coupling generator (host fp64 Philox + Box-Muller,
+// DESIGN.md section 3.2) and the kernel launches.  No CPU implementation of any sweep exists here:
+// without a device every compute call fails with SG_ECUDA.
+#include "../../include/sg_b200.h"
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "sg_kernels.cuh"
+
+using namespace sg;
+
+struct sg_ctx {
+    sg_shape shape;
+    int L, N, Nh, S, R, T, C, NG, Cp, P;
+    cudaStream_t stream;
+    // device arrays (carved from the caller's workspace)
+    float* spins; float* Jg; float* Mraw; float* staging; float* beta_slot;
+    double* betas; double* E; double* Epart; double* phase; double* Mpart; double* result;
+    int* slot_of_temp; int* temp_of_slot;
+    unsigned long long* attempts; unsigned long long* accepts;
+    // sweep geometry
+    int tile_sites, ntiles, log2L;
+    // measure geometry
+    int nchunk, chunk_sites, MS;
+    // host state
+    std::vector<double> h_betas;
+    std::vector<char> inited;
+    uint64_t hb_counter, pt_counter, launches;
+    bool energies_fresh;
+    int last_cuda;
+};
+
+namespace {
+
+size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+bool shape_ok(const sg_shape* s)
+{
+    if (!s) return false;
+    if (s->L < 2 || (s->L & 1) || s->L > 1024) return false;
+    if (s->n_samples <= 0 || s->n_replicas <= 0 || s->n_temps <= 0 || s->first_sample < 0) return false;
+    if (s->reserved != 0) return false;
+    const double N = (double)s->L * s->L * s->L;
+    const double C = (double)s->n_replicas * s->n_temps;
+    if (N > 2.0e9 || C > 1.0e6) return false;
+    if (((double)s->first_sample + s->n_samples) * C > 4.0e9) return false;   // copy ids are 32-bit counters
+    if ((double)s->n_samples * std::ceil(C / 32.0) * N * 96.0 > 4.0e11) return false;
+    return true;
+}
+
+struct Geometry {
+    int L, N, Nh, S, R, T, C, NG, Cp, P, tile_sites, ntiles, nchunk, chunk_sites, MS;
+};
+
+Geometry geometry(const sg_shape* s)
+{
+    Geometry g;
+    g.L = s->L; g.N = s->L * s->L * s->L; g.Nh = g.N / 2;
+    g.S = s->n_samples; g.R = s->n_replicas; g.T = s->n_temps; g.C = g.R * g.T;
+    g.NG = (g.C + G - 1) / G; g.Cp = g.NG * G; g.P = g.R * (g.R - 1) / 2;
+    // sweep tiles: 128 consecutive same-colour sites per CTA (4 passes of 32 site slots)
+    g.tile_sites = 128;
+    g.ntiles = (g.Nh + g.tile_sites - 1) / g.tile_sites;
+    // measure chunks
+    g.nchunk = g.N / 512; if (g.nchunk < 1) g.nchunk = 1; if (g.nchunk > 256) g.nchunk = 256;
+    g.chunk_sites = (g.N + g.nchunk - 1) / g.nchunk;
+    g.MS = 10240 / (3 * g.Cp); if (g.MS < 1) g.MS = 1; if (g.MS > 8) g.MS = 8;
+    return g;
+}
+
+struct Carve {
+    size_t off = 0;
+    size_t take(size_t bytes) { size_t o = off; off += align256(bytes); return o; }
+};
+
+struct Offsets {
+    size_t spins, Jg, Mraw, staging, beta_slot, betas, E, Epart, phase, Mpart, result, sot, tos, att, acc, total;
+};
+
+Offsets offsets(const Geometry& g)
+{
+    Carve c; Offsets o;
+    o.spins = c.take((size_t)g.S * g.NG * g.N * SITE_FLOATS * sizeof(float));
+    o.Jg = c.take((size_t)g.S * 2 * g.Nh * JG * sizeof(float));
+    o.Mraw = c.take((size_t)g.S * 3 * g.N * 9 * sizeof(float));
+    size_t stg = (size_t)G * 3 * g.N * sizeof(float);
+    o.staging = c.take(stg);
+    o.beta_slot = c.take((size_t)g.S * g.Cp * sizeof(float));
+    o.betas = c.take((size_t)g.T * sizeof(double));
+    o.E = c.take((size_t)g.S * g.Cp * sizeof(double));
+    o.Epart = c.take((size_t)g.S * g.NG * g.ntiles * G * sizeof(double));
+    o.phase = c.take((size_t)g.L * 2 * sizeof(double));
+    o.Mpart = c.take((size_t)g.S * g.nchunk * (g.P * g.T > 0 ? g.P * g.T : 1) * 7 * sizeof(double));
+    o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 7 + 1) * sizeof(double));
+    o.sot = c.take((size_t)g.S * g.R * g.T * sizeof(int));
+    o.tos = c.take((size_t)g.S * g.R * g.T * sizeof(int));
+    size_t st = (size_t)g.S * g.R * (g.T > 1 ? g.T - 1 : 1) * sizeof(unsigned long long);
+    o.att = c.take(st);
+    o.acc = c.take(st);
+    o.total = c.off;
+    return o;
+}
+
+int cuda_fail(sg_ctx* ctx, cudaError_t e)
+{
+    if (ctx) ctx->last_cuda = (int)e;
+    return SG_ECUDA;
+}
+
+#define SG_CUDA(ctx, call)                                    \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) return cuda_fail((ctx), e__); \
+    } while (0)
+
+#define SG_LAUNCHED(ctx)                                      \
+    do {                                                      \
+        (ctx)->launches += 1;                                 \
+        cudaError_t e__ = cudaGetLastError();                 \
+        if (e__ != cudaSuccess) return cuda_fail((ctx), e__); \
+    } while (0)
+
+int ilog2_exact(int L)
+{
+    int l = 0;
+    while ((1 << l) < L) ++l;
+    return ((1 << l) == L) ? l : 0;
+}
+
+// ---- coupling generator (host, fp64) ----
+const double kPi = 3.14159265358979323846;
+
+void link_normals(uint64_t seed, uint32_t link, uint32_t sample, double n[12], uint32_t w0[4])
+{
+    const uint32_t k0 = (uint32_t)(seed & 0xffffffffu), k1 = (uint32_t)(seed >> 32);
+    for (uint32_t j = 0; j < 3; ++j) {
+        uint32_t w[4];
+        philox4x32_10(link, sample, j, STREAM_COUPLINGS, k0, k1, w);
+        if (j == 0) std::memcpy(w0, w, sizeof(w));
+        for (int pair = 0; pair < 2; ++pair) {
+            const double u0 = ((double)w[2 * pair] + 0.5) / 4294967296.0;
+            const double u1 = ((double)w[2 * pair + 1] + 0.5) / 4294967296.0;
+            const double rad = std::sqrt(-2.0 * std::log(u0));
+            n[4 * j + 2 * pair] = rad * std::cos(2.0 * kPi * u1);
+            n[4 * j + 2 * pair + 1] = rad * std::sin(2.0 * kPi * u1);
+        }
+    }
+}
+
+void generate_couplings(int L, uint64_t seed, uint32_t sample, int mode, double sd, float* M)
+{
+    const int N = L * L * L;
+    for (int i = 0; i < N; ++i)
+        for (int mu = 0; mu < 3; ++mu) {
+            double n[12], m[9] = { 0, 0, 0, 0, 0, 0, 0, 0, 0 };
+            uint32_t w0[4];
+            link_normals(seed, (uint32_t)(3 * i + mu), sample, n, w0);
+            switch (mode) {
+            case SG_GEN_OFFDIAG_SYM:
+                m[0] = m[4] = m[8] = n[0];
+                m[1] = m[3] = sd * n[1]; m[2] = m[6] = sd * n[2]; m[5] = m[7] = sd * n[3];
+                break;
+            case SG_GEN_PAPER_SYM6:
+                m[0] = n[0] + sd * n[1]; m[4] = n[0] + sd * n[2]; m[8] = n[0] + sd * n[3];
+                m[1] = m[3] = sd * n[4]; m[2] = m[6] = sd * n[5]; m[5] = m[7] = sd * n[6];
+                break;
+            case SG_GEN_GENERAL9:
+                for (int e = 0; e < 9; ++e) m[e] = sd * n[e];
+                break;
+            case SG_GEN_BIMODAL: {
+                const double J = (w0[0] & 1u) ? 1.0 : -1.0;
+                double d[6];
+                for (int k = 0; k < 6; ++k) d[k] = ((w0[0] >> (k + 1)) & 1u) ? sd : -sd;
+                m[0] = J + d[0]; m[4] = J + d[1]; m[8] = J + d[2];
+                m[1] = m[3] = d[3]; m[2] = m[6] = d[4]; m[5] = m[7] = d[5];
+                break;
+            }
+            default:
+                m[0] = m[4] = m[8] = 1.0;
+            }
+            float* dst = M + ((size_t)mu * N + i) * 9;
+            for (int e = 0; e < 9; ++e) dst[e] = (float)m[e];
+        }
+}
+
+template <int KIND, bool WITH_E>
+void launch_sweep_l(sg_ctx* ctx, const SweepParams& p, dim3 grid)
+{
+    switch (ctx->log2L) {
+    case 1: k_sweep<KIND, WITH_E, 1><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(p); break;
+    case 2: k_sweep<KIND, WITH_E, 2><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(p); break;
+    case 3: k_sweep<KIND, WITH_E, 3><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(p); break;
+    case 4: k_sweep<KIND, WITH_E, 4><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(p); break;
+    case 5: k_sweep<KIND, WITH_E, 5><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(p); break;
+    case 6: k_sweep<KIND, WITH_E, 6><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(p); break;
+    case 7: k_sweep<KIND, WITH_E, 7><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(p); break;
+    default: k_sweep<KIND, WITH_E, 0><<<grid, SWEEP_THREADS, 0, ctx->stream>>>(p); break;
+    }
+}
+
+// one half-sweep of every copy; with_energy also reduces E (valid because a whole colour is swept)
+int half_sweep(sg_ctx* ctx, int kind, int colour, bool with_energy)
+{
+    SweepParams p;
+    p.spins = ctx->spins; p.Jg = ctx->Jg; p.beta_slot = ctx->beta_slot; p.Epart = ctx->Epart;
+    p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.ntiles = ctx->ntiles;
+    p.tile_sites = ctx->tile_sites; p.colour = colour; p.C = ctx->C;
+    p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
+    p.hb_counter = (uint32_t)ctx->hb_counter;
+    p.g_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->C;
+    const dim3 grid(ctx->ntiles, ctx->NG, ctx->S);
+    if (kind == KIND_OR) {
+        if (with_energy) launch_sweep_l<KIND_OR, true>(ctx, p, grid);
+        else launch_sweep_l<KIND_OR, false>(ctx, p, grid);
+    } else if (kind == KIND_HB) {
+        if (with_energy) launch_sweep_l<KIND_HB, true>(ctx, p, grid);
+        else launch_sweep_l<KIND_HB, false>(ctx, p, grid);
+    } else {
+        launch_sweep_l<KIND_ENERGY, true>(ctx, p, grid);
+    }
+    SG_LAUNCHED(ctx);
+    if (with_energy || kind == KIND_ENERGY) {
+        k_reduce_energy<<<ctx->S * ctx->NG, 256, 0, ctx->stream>>>(ctx->Epart, ctx->E, ctx->ntiles);
+        SG_LAUNCHED(ctx);
+        ctx->energies_fresh = true;
+    } else {
+        ctx->energies_fresh = false;
+    }
+    return SG_OK;
+}
+
+int all_inited(const sg_ctx* ctx)
+{
+    for (char c : ctx->inited)
+        if (!c) return SG_ESTATE;
+    return SG_OK;
+}
+
+int ensure_energies(sg_ctx* ctx)
+{
+    if (ctx->energies_fresh) return SG_OK;
+    return half_sweep(ctx, KIND_ENERGY, 0, true);
+}
+
+int fill_beta_slot(sg_ctx* ctx)
+{
+    const int n = ctx->S * ctx->Cp;
+    k_fill_beta_slot<<<(n + 255) / 256, 256, 0, ctx->stream>>>(ctx->betas, ctx->temp_of_slot, ctx->beta_slot, ctx->S,
+                                                              ctx->R, ctx->T, ctx->Cp);
+    SG_LAUNCHED(ctx);
+    return SG_OK;
+}
+
+int sweeps(sg_ctx* ctx, int kind, int n_sweeps)
+{
+    if (!ctx || n_sweeps < 0) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    for (int k = 0; k < n_sweeps; ++k) {
+        if (int rc = half_sweep(ctx, kind, 0, false)) return rc;
+        if (int rc = half_sweep(ctx, kind, 1, k == n_sweeps - 1)) return rc;
+        if (kind == KIND_HB) ctx->hb_counter += 1;
+    }
+    return SG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t sg_workspace_bytes(const sg_shape* shape)
+{
+    if (!shape_ok(shape)) return 0;
+    return offsets(geometry(shape)).total;
+}
+
+int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* dev_workspace, size_t bytes,
+              void* cuda_stream)
+{
+    if (!out) return SG_EINVAL;
+    *out = nullptr;
+    if (!shape_ok(shape) || !betas || !dev_workspace) return SG_EINVAL;
+    if (((uintptr_t)dev_workspace & 255) != 0) return SG_EINVAL;
+    for (int t = 0; t < shape->n_temps; ++t)
+        if (!std::isfinite(betas[t])) return SG_EINVAL;
+    if (shape->n_temps > 1) {
+        const bool up = betas[1] > betas[0];
+        for (int t = 1; t < shape->n_temps; ++t)
+            if (up ? !(betas[t] > betas[t - 1]) : !(betas[t] < betas[t - 1])) return SG_EINVAL;
+    }
+    const Geometry g = geometry(shape);
+    const Offsets o = offsets(g);
+    if (bytes < o.total) return SG_EINVAL;
+
+    sg_ctx* ctx = new (std::nothrow) sg_ctx();
+    if (!ctx) return SG_EINVAL;
+    ctx->shape = *shape;
+    ctx->L = g.L; ctx->N = g.N; ctx->Nh = g.Nh; ctx->S = g.S; ctx->R = g.R; ctx->T = g.T; ctx->C = g.C;
+    ctx->NG = g.NG; ctx->Cp = g.Cp; ctx->P = g.P;
+    ctx->tile_sites = g.tile_sites; ctx->ntiles = g.ntiles; ctx->log2L = ilog2_exact(g.L);
+    ctx->nchunk = g.nchunk; ctx->chunk_sites = g.chunk_sites; ctx->MS = g.MS;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    char* base = (char*)dev_workspace;
+    ctx->spins = (float*)(base + o.spins); ctx->Jg = (float*)(base + o.Jg); ctx->Mraw = (float*)(base + o.Mraw);
+    ctx->staging = (float*)(base + o.staging); ctx->beta_slot = (float*)(base + o.beta_slot);
+    ctx->betas = (double*)(base + o.betas); ctx->E = (double*)(base + o.E); ctx->Epart = (double*)(base + o.Epart);
+    ctx->phase = (double*)(base + o.phase); ctx->Mpart = (double*)(base + o.Mpart);
+    ctx->result = (double*)(base + o.result);
+    ctx->slot_of_temp = (int*)(base + o.sot); ctx->temp_of_slot = (int*)(base + o.tos);
+    ctx->attempts = (unsigned long long*)(base + o.att); ctx->accepts = (unsigned long long*)(base + o.acc);
+    ctx->h_betas.assign(betas, betas + g.T);
+    ctx->inited.assign(g.S, 0);
+    ctx->hb_counter = ctx->pt_counter = ctx->launches = 0;
+    ctx->energies_fresh = false;
+    ctx->last_cuda = 0;
+
+    // small tables: betas, Fourier phases, identity permutations, zeroed statistics
+    std::vector<double> phase(2 * (size_t)g.L);
+    for (int x = 0; x < g.L; ++x) {
+        phase[2 * x] = std::cos(2.0 * kPi * (double)x / (double)g.L);
+        phase[2 * x + 1] = std::sin(2.0 * kPi * (double)x / (double)g.L);
+    }
+    std::vector<int> ident((size_t)g.S * g.R * g.T);
+    for (size_t k = 0; k < ident.size(); ++k) ident[k] = (int)(k % g.T);
+    cudaError_t e = cudaMemcpyAsync(ctx->betas, betas, g.T * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->phase, phase.data(), phase.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->slot_of_temp, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->temp_of_slot, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
+    const size_t st = (size_t)g.S * g.R * (g.T > 1 ? g.T - 1 : 1) * sizeof(unsigned long long);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->attempts, 0, st, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->accepts, 0, st, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->E, 0, (size_t)g.S * g.Cp * sizeof(double), ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // the host vectors above go out of scope
+    if (e != cudaSuccess) { delete ctx; return SG_ECUDA; }
+    int rc = fill_beta_slot(ctx);
+    if (rc != SG_OK) { delete ctx; return rc; }
+    *out = ctx;
+    return SG_OK;
+}
+
+int sg_destroy(sg_ctx* ctx)
+{
+    if (!ctx) return SG_EINVAL;
+    cudaStreamSynchronize(ctx->stream);
+    delete ctx;
+    return SG_OK;
+}
+
+int sg_set_spins(sg_ctx* ctx, int sample, const float* in)
+{
+    if (!ctx || !in || sample < 0 || sample >= ctx->S) return SG_EINVAL;
+    const size_t copy_floats = (size_t)3 * ctx->N;
+    for (int grp = 0; grp < ctx->NG; ++grp) {
+        const int c0 = grp * G, nc = (ctx->C - c0 < G) ? ctx->C - c0 : G;
+        if (nc < G) SG_CUDA(ctx, cudaMemsetAsync(ctx->staging, 0, (size_t)G * copy_floats * sizeof(float), ctx->stream));
+        SG_CUDA(ctx, cudaMemcpyAsync(ctx->staging, in + (size_t)c0 * copy_floats, (size_t)nc * copy_floats * sizeof(float),
+                                     cudaMemcpyHostToDevice, ctx->stream));
+        float* dev = ctx->spins + ((size_t)(sample * ctx->NG + grp) * ctx->N) * SITE_FLOATS;
+        k_spins_from_staging<<<dim3((ctx->N + 31) / 32, 3), dim3(32, 8), 0, ctx->stream>>>(ctx->staging, dev, ctx->N);
+        SG_LAUNCHED(ctx);
+    }
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->energies_fresh = false;
+    return SG_OK;
+}
+
+int sg_get_spins(sg_ctx* ctx, int sample, float* out)
+{
+    if (!ctx || !out || sample < 0 || sample >= ctx->S) return SG_EINVAL;
+    if (!ctx->inited[sample]) return SG_ESTATE;
+    const size_t copy_floats = (size_t)3 * ctx->N;
+    for (int grp = 0; grp < ctx->NG; ++grp) {
+        const int c0 = grp * G, nc = (ctx->C - c0 < G) ? ctx->C - c0 : G;
+        const float* dev = ctx->spins + ((size_t)(sample * ctx->NG + grp) * ctx->N) * SITE_FLOATS;
+        k_spins_to_staging<<<dim3((ctx->N + 31) / 32, 3), dim3(32, 8), 0, ctx->stream>>>(dev, ctx->staging, ctx->N);
+        SG_LAUNCHED(ctx);
+        SG_CUDA(ctx, cudaMemcpyAsync(out + (size_t)c0 * copy_floats, ctx->staging, (size_t)nc * copy_floats * sizeof(float),
+                                     cudaMemcpyDeviceToHost, ctx->stream));
+        SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    }
+    return SG_OK;
+}
+
+int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const float* couplings, const float* spins)
+{
+    if (!ctx || sample < 0 || sample >= ctx->S) return SG_EINVAL;
+    if (!couplings && (gen_mode < SG_GEN_OFFDIAG_SYM || gen_mode > SG_GEN_FERRO || !std::isfinite(sigma_D))) return SG_EINVAL;
+    const size_t mfloats = (size_t)3 * ctx->N * 9;
+    float* Mdev = ctx->Mraw + (size_t)sample * mfloats;
+    std::vector<float> gen;
+    const float* src = couplings;
+    if (!src) {
+        gen.resize(mfloats);
+        generate_couplings(ctx->L, ctx->shape.seed, (uint32_t)(ctx->shape.first_sample + sample), gen_mode, sigma_D, gen.data());
+        src = gen.data();
+    }
+    SG_CUDA(ctx, cudaMemcpyAsync(Mdev, src, mfloats * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    k_gather_couplings<<<(ctx->N + 127) / 128, 128, 0, ctx->stream>>>(Mdev, ctx->Jg + (size_t)sample * 2 * ctx->Nh * JG, ctx->L);
+    SG_LAUNCHED(ctx);
+
+    if (spins) {
+        if (int rc = sg_set_spins(ctx, sample, spins)) return rc;
+    } else {
+        const size_t nthr = (size_t)ctx->NG * ctx->N * 8;
+        const uint32_t g_sample = (uint32_t)(ctx->shape.first_sample + sample) * (uint32_t)ctx->C;
+        k_init_spins<<<(unsigned)((nthr + 255) / 256), 256, 0, ctx->stream>>>(
+            ctx->spins + (size_t)sample * ctx->NG * ctx->N * SITE_FLOATS, ctx->N, ctx->NG, ctx->C, g_sample,
+            (uint32_t)(ctx->shape.seed & 0xffffffffu), (uint32_t)(ctx->shape.seed >> 32));
+        SG_LAUNCHED(ctx);
+    }
+    // identity temperature assignment for this sample
+    std::vector<int> ident((size_t)ctx->R * ctx->T);
+    for (size_t k = 0; k < ident.size(); ++k) ident[k] = (int)(k % ctx->T);
+    const size_t off = (size_t)sample * ctx->R * ctx->T;
+    SG_CUDA(ctx, cudaMemcpyAsync(ctx->slot_of_temp + off, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+    SG_CUDA(ctx, cudaMemcpyAsync(ctx->temp_of_slot + off, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (int rc = fill_beta_slot(ctx)) return rc;
+    ctx->inited[sample] = 1;
+    ctx->energies_fresh = false;
+    return SG_OK;
+}
+
+int sg_sweep_or(sg_ctx* ctx, int n_sweeps) { return sweeps(ctx, KIND_OR, n_sweeps); }
+int sg_sweep_hb(sg_ctx* ctx, int n_sweeps) { return sweeps(ctx, KIND_HB, n_sweeps); }
+
+int sg_halfsweep(sg_ctx* ctx, int kind, int colour)
+{
+    if (!ctx || (kind != SG_KIND_OR && kind != SG_KIND_HB) || (colour != 0 && colour != 1)) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    return half_sweep(ctx, kind, colour, false);
+}
+
+int sg_pt_swap(sg_ctx* ctx)
+{
+    if (!ctx) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    if (int rc = ensure_energies(ctx)) return rc;
+    PtParams p;
+    p.betas = ctx->betas; p.E = ctx->E; p.slot_of_temp = ctx->slot_of_temp; p.temp_of_slot = ctx->temp_of_slot;
+    p.beta_slot = ctx->beta_slot; p.attempts = ctx->attempts; p.accepts = ctx->accepts;
+    p.S = ctx->S; p.R = ctx->R; p.T = ctx->T; p.Cp = ctx->Cp;
+    p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
+    p.pt_counter = (uint32_t)ctx->pt_counter;
+    p.chain_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->R;
+    const int chains = ctx->S * ctx->R;
+    k_pt_swap<<<(chains + 63) / 64, 64, 0, ctx->stream>>>(p);
+    SG_LAUNCHED(ctx);
+    ctx->pt_counter += 1;
+    return SG_OK;
+}
+
+int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
+{
+    if (!ctx) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    if (int rc = ensure_energies(ctx)) return rc;
+    const int PT = ctx->P * ctx->T;
+    if (PT > 0 && (q0 || qk)) {
+        MeasureParams p;
+        p.spins = ctx->spins; p.slot_of_temp = ctx->slot_of_temp; p.phase = ctx->phase; p.Mpart = ctx->Mpart;
+        p.L = ctx->L; p.N = ctx->N; p.NG = ctx->NG; p.Cp = ctx->Cp; p.R = ctx->R; p.T = ctx->T; p.P = ctx->P;
+        p.nchunk = ctx->nchunk; p.chunk_sites = ctx->chunk_sites; p.MS = ctx->MS;
+        int threads = ((PT + 31) / 32) * 32;
+        if (threads > 512) threads = 512;
+        const int nbatch = (PT + threads - 1) / threads;
+        const size_t smem = (size_t)ctx->MS * 3 * ctx->Cp * sizeof(float);
+        if (smem > 48 * 1024) return SG_EINVAL;
+        k_measure<<<dim3(ctx->nchunk, ctx->S, nbatch), threads, smem, ctx->stream>>>(p);
+        SG_LAUNCHED(ctx);
+    }
+    const int nE = ctx->S * ctx->R * ctx->T, nQ = ctx->S * PT;
+    const int total = nE + nQ * 7;
+    k_reduce_measure<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->Mpart, ctx->E, ctx->slot_of_temp, ctx->result, ctx->S,
+                                                                 ctx->R, ctx->T, ctx->P, ctx->Cp, ctx->nchunk, ctx->N);
+    SG_LAUNCHED(ctx);
+    if (e) SG_CUDA(ctx, cudaMemcpyAsync(e, ctx->result, (size_t)nE * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    if (q0 && nQ) SG_CUDA(ctx, cudaMemcpyAsync(q0, ctx->result + nE, (size_t)nQ * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    if (qk && nQ) SG_CUDA(ctx, cudaMemcpyAsync(qk, ctx->result + nE + nQ, (size_t)nQ * 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_get_couplings(sg_ctx* ctx, int sample, float* out)
+{
+    if (!ctx || !out || sample < 0 || sample >= ctx->S) return SG_EINVAL;
+    if (!ctx->inited[sample]) return SG_ESTATE;
+    const size_t mfloats = (size_t)3 * ctx->N * 9;
+    SG_CUDA(ctx, cudaMemcpyAsync(out, ctx->Mraw + (size_t)sample * mfloats, mfloats * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_get_perm(sg_ctx* ctx, int sample, int32_t* temp_of_slot, int32_t* slot_of_temp)
+{
+    if (!ctx || sample < 0 || sample >= ctx->S) return SG_EINVAL;
+    const size_t n = (size_t)ctx->R * ctx->T, off = (size_t)sample * n;
+    if (temp_of_slot) SG_CUDA(ctx, cudaMemcpyAsync(temp_of_slot, ctx->temp_of_slot + off, n * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    if (slot_of_temp) SG_CUDA(ctx, cudaMemcpyAsync(slot_of_temp, ctx->slot_of_temp + off, n * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_set_perm(sg_ctx* ctx, int sample, const int32_t* temp_of_slot)
+{
+    if (!ctx || !temp_of_slot || sample < 0 || sample >= ctx->S) return SG_EINVAL;
+    const int R = ctx->R, T = ctx->T;
+    std::vector<int> tos(temp_of_slot, temp_of_slot + (size_t)R * T), sot((size_t)R * T, -1);
+    for (int r = 0; r < R; ++r)
+        for (int s = 0; s < T; ++s) {
+            const int t = tos[(size_t)r * T + s];
+            if (t < 0 || t >= T || sot[(size_t)r * T + t] != -1) return SG_EINVAL;
+            sot[(size_t)r * T + t] = s;
+        }
+    const size_t off = (size_t)sample * R * T;
+    SG_CUDA(ctx, cudaMemcpyAsync(ctx->temp_of_slot + off, tos.data(), tos.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+    SG_CUDA(ctx, cudaMemcpyAsync(ctx->slot_of_temp + off, sot.data(), sot.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return fill_beta_slot(ctx);
+}
+
+int sg_get_energies(sg_ctx* ctx, double* E)
+{
+    if (!ctx || !E) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    if (int rc = ensure_energies(ctx)) return rc;
+    SG_CUDA(ctx, cudaMemcpy2DAsync(E, (size_t)ctx->C * sizeof(double), ctx->E, (size_t)ctx->Cp * sizeof(double),
+                                   (size_t)ctx->C * sizeof(double), ctx->S, cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_set_energies(sg_ctx* ctx, const double* E)
+{
+    if (!ctx || !E) return SG_EINVAL;
+    SG_CUDA(ctx, cudaMemcpy2DAsync(ctx->E, (size_t)ctx->Cp * sizeof(double), E, (size_t)ctx->C * sizeof(double),
+                                   (size_t)ctx->C * sizeof(double), ctx->S, cudaMemcpyHostToDevice, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->energies_fresh = true;
+    return SG_OK;
+}
+
+int sg_get_counters(sg_ctx* ctx, uint64_t* hb_counter, uint64_t* pt_counter)
+{
+    if (!ctx) return SG_EINVAL;
+    if (hb_counter) *hb_counter = ctx->hb_counter;
+    if (pt_counter) *pt_counter = ctx->pt_counter;
+    return SG_OK;
+}
+
+int sg_set_counters(sg_ctx* ctx, uint64_t hb_counter, uint64_t pt_counter)
+{
+    if (!ctx) return SG_EINVAL;
+    ctx->hb_counter = hb_counter;
+    ctx->pt_counter = pt_counter;
+    return SG_OK;
+}
+
+int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts)
+{
+    if (!ctx) return SG_EINVAL;
+    if (ctx->T < 2) return SG_OK;
+    const size_t n = (size_t)ctx->S * ctx->R * (ctx->T - 1) * sizeof(unsigned long long);
+    if (attempts) SG_CUDA(ctx, cudaMemcpyAsync(attempts, ctx->attempts, n, cudaMemcpyDeviceToHost, ctx->stream));
+    if (accepts) SG_CUDA(ctx, cudaMemcpyAsync(accepts, ctx->accepts, n, cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_sync(sg_ctx* ctx)
+{
+    if (!ctx) return SG_EINVAL;
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+uint64_t sg_kernel_launches(const sg_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int sg_last_cuda_error(const sg_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
+
+const char* sg_strerror(int code)
+{
+    switch (code) {
+    case SG_OK: return "ok";
+    case SG_EINVAL: return "invalid argument";
+    case SG_ESTATE: return "sample not initialised";
+    case SG_ECUDA: return "CUDA call failed (see sg_last_cuda_error)";
+    default: return "unknown error";
+    }
+}
+
+void sg_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    philox4x32_10(ctr[0], ctr[1], ctr[2], ctr[3], key[0], key[1], out);
+}
+
+}  // extern "C"

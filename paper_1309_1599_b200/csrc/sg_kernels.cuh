@@ -1,0 +1,394 @@
+// sg_kernels.cuh -- the CUDA kernels of libsg_b200 (sm_100a).  DESIGN.md section 10 states, for each
+// kernel, the roofline that bounds it and its algorithmic bytes per spin update.
+#pragma once
+#include "sg_device.cuh"
+
+namespace sg {
+
+// ------------------------------------------------------------------------------------------------
+// Sweep kernel (S1, S2, S3): one checkerboard half-sweep of every copy of every sample.
+//
+// Work decomposition.  A CTA owns TILE consecutive same-colour sites (h-order: along x1, then x2, x3)
+// of ONE (sample, copy group); its 256 threads are 32 site slots x 8 lanes, a lane holding the float4 of
+// 4 consecutive copies.  Every spin access of a warp instruction is four full, aligned 128-byte lines
+// (one per site), for every L, with no colour-split arrays; stores are full lines.  The six matrices
+// of a site are shared by the 8 lanes (one broadcast LDG.128 per 4 floats) and used for 4 copies each.
+// ------------------------------------------------------------------------------------------------
+constexpr int SWEEP_THREADS = 256;
+constexpr int SLOTS = SWEEP_THREADS / 8;   // site slots per pass
+
+enum : int { KIND_OR = 0, KIND_HB = 1, KIND_ENERGY = 2 };
+
+struct SweepParams {
+    float* spins;            // [S][NG][N][3][G]
+    const float* Jg;         // [S][2][Nh][JG]
+    const float* beta_slot;  // [S][Cp]
+    double* Epart;           // [S][NG][ntiles][G]
+    int L, N, Nh, NG, ntiles, tile_sites;
+    int colour;
+    int C;                   // copies per sample (R*T); Cp = NG*G
+    uint32_t key0, key1, hb_counter;
+    uint32_t g_first;        // global copy id of (local sample 0, copy 0) = first_sample*C
+};
+
+template <int KIND, bool WITH_E, int LOG2L>
+__global__ void __launch_bounds__(SWEEP_THREADS) k_sweep(const SweepParams p)
+{
+    const int tid = threadIdx.x;
+    const int q = tid & 7;        // copy quad: copies 4q..4q+3 of the group
+    const int slot = tid >> 3;    // site slot
+    const int tile = blockIdx.x, grp = blockIdx.y, sample = blockIdx.z;
+    const int L = p.L;
+
+    float* const sp = p.spins + ((size_t)(sample * p.NG + grp) * p.N) * SITE_FLOATS + q * 4;
+    const float* const Jc = p.Jg + ((size_t)(sample * 2 + p.colour) * p.Nh) * JG;
+
+    float4 beta4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (KIND == KIND_HB) beta4 = ldg4(p.beta_slot + (size_t)sample * p.NG * G + grp * G + q * 4);
+
+    float eacc[4] = { 0.f, 0.f, 0.f, 0.f };
+
+    const int h_end = min(p.Nh, (tile + 1) * p.tile_sites);
+    for (int h = tile * p.tile_sites + slot; h < h_end; h += SLOTS) {
+        int x, y, z;
+        site_of<LOG2L>(h, p.colour, L, x, y, z);
+        const int xp = (x + 1 == L) ? 0 : x + 1, xm = (x == 0) ? L - 1 : x - 1;
+        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+        const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+        const int row = L * (y + L * z);
+        const int i = x + row;
+        int nb[6];
+        nb[0] = xp + row;            nb[1] = xm + row;
+        nb[2] = x + L * (yp + L * z); nb[3] = x + L * (ym + L * z);
+        nb[4] = x + L * (y + L * zp); nb[5] = x + L * (y + L * zm);
+
+        // couplings of this site: 14 broadcast 16-byte loads (54 floats + 2 pad)
+        float J[JG];
+        {
+            const float* jp = Jc + (size_t)h * JG;
+#pragma unroll
+            for (int v = 0; v < JG / 4; ++v) {
+                const float4 t4 = ldg4(jp + 4 * v);
+                J[4 * v] = t4.x; J[4 * v + 1] = t4.y; J[4 * v + 2] = t4.z; J[4 * v + 3] = t4.w;
+            }
+        }
+        float* const own = sp + (size_t)i * SITE_FLOATS;
+        float s[3][4];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const float4 t4 = ld4(own + a * G);
+            s[a][0] = t4.x; s[a][1] = t4.y; s[a][2] = t4.z; s[a][3] = t4.w;
+        }
+        float hf[3][4];
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) hf[a][j] = 0.f;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const float* np_ = sp + (size_t)nb[k] * SITE_FLOATS;
+            float n[3][4];
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const float4 t4 = ld4(np_ + b * G);
+                n[b][0] = t4.x; n[b][1] = t4.y; n[b][2] = t4.z; n[b][3] = t4.w;
+            }
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * k + 3 * a + b], n[b][j], hf[a][j]);
+        }
+
+        if (KIND == KIND_OR) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
+                or_update(hf[0][j], hf[1][j], hf[2][j], s[0][j], s[1][j], s[2][j]);
+            }
+        } else if (KIND == KIND_HB) {
+            const float bt[4] = { beta4.x, beta4.y, beta4.z, beta4.w };
+            const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.C + (uint32_t)(grp * G + q * 4);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                uint32_t w[4];
+                philox4x32_10((uint32_t)i, g0 + j, p.hb_counter, STREAM_HB, p.key0, p.key1, w);
+                hb_update(hf[0][j], hf[1][j], hf[2][j], bt[j], uniform23(w[0]), uniform23(w[1]),
+                          s[0][j], s[1][j], s[2][j]);
+                if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
+        }
+        if (KIND != KIND_ENERGY) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) st4(own + a * G, make_float4(s[a][0], s[a][1], s[a][2], s[a][3]));
+        }
+    }
+
+    if (WITH_E || KIND == KIND_ENERGY) {
+        // per-copy sum over the CTA's sites: fixed order, fp64 across threads (no float atomics)
+        __shared__ double red[SLOTS][G + 1];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) red[slot][q * 4 + j] = (double)eacc[j];
+        __syncthreads();
+        if (tid < G) {
+            double acc = 0.0;
+            for (int r = 0; r < SLOTS; ++r) acc += red[r][tid];
+            p.Epart[((size_t)(sample * p.NG + grp) * p.ntiles + tile) * G + tid] = acc;
+        }
+    }
+}
+
+// E[sample][copy] = - sum over tiles of the per-CTA partial sums of s.h over ONE colour
+// (every link joins the two colours, so one colour's sum of s_x.h_x counts each link once).
+__global__ void k_reduce_energy(const double* __restrict__ Epart, double* __restrict__ E, int ntiles)
+{
+    // grid = S*NG blocks of 256 threads = 8 tile ranges x 32 copies
+    __shared__ double part[8][G];
+    const int col = threadIdx.x & 31, rng = threadIdx.x >> 5;
+    const double* src = Epart + (size_t)blockIdx.x * ntiles * G;
+    const int per = (ntiles + 7) / 8;
+    double acc = 0.0;
+    for (int t = rng * per; t < min(ntiles, (rng + 1) * per); ++t) acc += src[(size_t)t * G + col];
+    part[rng][col] = acc;
+    __syncthreads();
+    if (rng == 0) {
+        double tot = 0.0;
+        for (int r = 0; r < 8; ++r) tot += part[r][col];
+        E[(size_t)blockIdx.x * G + col] = -tot;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S0: initial spins uniform on S^2, Philox stream 3, counter (i, g, 0, 3)
+// ------------------------------------------------------------------------------------------------
+__global__ void k_init_spins(float* __restrict__ spins_sample /* [NG][N][3][G] of one sample */, int N, int NG,
+                             int C, uint32_t g_sample, uint32_t key0, uint32_t key1)
+{
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;   // over NG*N*8 (site, quad)
+    if (t >= (size_t)NG * N * 8) return;
+    const int q = (int)(t & 7);
+    const size_t si = t >> 3;
+    const int i = (int)(si % N), grp = (int)(si / N);
+    float out[3][4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int c = grp * G + q * 4 + j;
+        uint32_t w[4];
+        philox4x32_10((uint32_t)i, g_sample + (uint32_t)c, 0u, STREAM_SPINS, key0, key1, w);
+        const float zc = 1.0f - 2.0f * uniform23(w[0]);
+        const float rho = sqrtf(fmaxf(1.0f - zc * zc, 0.0f));
+        float sn, cs;
+        sincospif(2.0f * uniform23(w[1]), &sn, &cs);
+        const bool live = c < C;     // padding copies of the last group stay zero
+        out[0][j] = live ? rho * cs : 0.f;
+        out[1][j] = live ? rho * sn : 0.f;
+        out[2][j] = live ? zc : 0.f;
+    }
+    float* dst = spins_sample + ((size_t)grp * N + i) * SITE_FLOATS + q * 4;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) st4(dst + a * G, make_float4(out[a][0], out[a][1], out[a][2], out[a][3]));
+}
+
+// host layout [c][3][N] (32 copies of one group, staged on the device) <-> device layout [N][3][G]
+// block (32, 8); tile = 32 sites x 32 copies per component
+__global__ void k_spins_from_staging(const float* __restrict__ stg, float* __restrict__ dev, int N)
+{
+    __shared__ float tile[32][33];
+    const int comp = blockIdx.y;
+    const int i0 = blockIdx.x * 32;
+    for (int c = threadIdx.y; c < 32; c += 8) {
+        const int i = i0 + threadIdx.x;
+        tile[c][threadIdx.x] = (i < N) ? stg[((size_t)c * 3 + comp) * N + i] : 0.f;
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += 8) {
+        const int i = i0 + r;
+        if (i < N) dev[(size_t)i * SITE_FLOATS + comp * G + threadIdx.x] = tile[threadIdx.x][r];
+    }
+}
+
+__global__ void k_spins_to_staging(const float* __restrict__ dev, float* __restrict__ stg, int N)
+{
+    __shared__ float tile[32][33];
+    const int comp = blockIdx.y;
+    const int i0 = blockIdx.x * 32;
+    for (int r = threadIdx.y; r < 32; r += 8) {
+        const int i = i0 + r;
+        tile[r][threadIdx.x] = (i < N) ? dev[(size_t)i * SITE_FLOATS + comp * G + threadIdx.x] : 0.f;
+    }
+    __syncthreads();
+    for (int c = threadIdx.y; c < 32; c += 8) {
+        const int i = i0 + threadIdx.x;
+        if (i < N) stg[((size_t)c * 3 + comp) * N + i] = tile[threadIdx.x][c];
+    }
+}
+
+// raw couplings M[3][N][9] of one sample -> gathered per-site blocks Jg[2][Nh][JG]
+__global__ void k_gather_couplings(const float* __restrict__ M, float* __restrict__ Jg_sample, int L)
+{
+    const int N = L * L * L, Nh = N >> 1;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int x = i % L, y = (i / L) % L, z = i / (L * L);
+    const int colour = (x + y + z) & 1;
+    float* dst = Jg_sample + ((size_t)colour * Nh + (i >> 1)) * JG;
+    const int bw[3] = { ((x == 0) ? L - 1 : x - 1) + L * (y + L * z), x + L * (((y == 0) ? L - 1 : y - 1) + L * z),
+                        x + L * (y + L * ((z == 0) ? L - 1 : z - 1)) };
+    for (int mu = 0; mu < 3; ++mu) {
+        const float* mf = M + ((size_t)mu * N + i) * 9;        // link (x, mu): acts as M
+        const float* mb = M + ((size_t)mu * N + bw[mu]) * 9;   // link (x-e_mu, mu): acts as M^T
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+                dst[(2 * mu) * 9 + 3 * a + b] = mf[3 * a + b];
+                dst[(2 * mu + 1) * 9 + 3 * a + b] = mb[3 * b + a];
+            }
+    }
+    dst[54] = 0.f; dst[55] = 0.f;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S4: parallel tempering.  One thread per chain (sample, replica); pairs in order.
+// ------------------------------------------------------------------------------------------------
+struct PtParams {
+    const double* betas;   // [T]
+    const double* E;       // [S][Cp]
+    int* slot_of_temp;     // [S][R][T]
+    int* temp_of_slot;     // [S][R][T]
+    float* beta_slot;      // [S][Cp]
+    unsigned long long* attempts;  // [S][R][T-1]
+    unsigned long long* accepts;
+    int S, R, T, Cp;
+    uint32_t key0, key1, pt_counter, chain_first;   // chain id of (local sample 0, r = 0) = first_sample*R
+};
+
+__global__ void k_pt_swap(const PtParams p)
+{
+    const int chain = blockIdx.x * blockDim.x + threadIdx.x;
+    if (chain >= p.S * p.R) return;
+    const int sample = chain / p.R, r = chain % p.R;
+    int* sot = p.slot_of_temp + (size_t)chain * p.T;
+    int* tos = p.temp_of_slot + (size_t)chain * p.T;
+    const double* E = p.E + (size_t)sample * p.Cp + r * p.T;
+    float* bs = p.beta_slot + (size_t)sample * p.Cp + r * p.T;
+    for (int t = 0; t + 1 < p.T; ++t) {
+        const int i = sot[t], j = sot[t + 1];
+        const double delta = (p.betas[t] - p.betas[t + 1]) * (E[i] - E[j]);
+        uint32_t w[4];
+        philox4x32_10((uint32_t)t, p.chain_first + (uint32_t)chain, p.pt_counter, STREAM_PT, p.key0, p.key1, w);
+        const double rr = ((double)(w[0] >> 9) + 0.5) * (1.0 / 8388608.0);
+        const bool accept = (delta >= 0.0) || (rr < exp(delta));
+        p.attempts[(size_t)chain * (p.T - 1) + t] += 1ull;
+        if (accept) {
+            sot[t] = j; sot[t + 1] = i;
+            tos[j] = t; tos[i] = t + 1;
+            bs[j] = (float)p.betas[t]; bs[i] = (float)p.betas[t + 1];
+            p.accepts[(size_t)chain * (p.T - 1) + t] += 1ull;
+        }
+    }
+}
+
+// beta_slot[sample][r*T + slot] = beta[temp_of_slot], for all chains (after init / set_perm)
+__global__ void k_fill_beta_slot(const double* __restrict__ betas, const int* __restrict__ temp_of_slot,
+                                 float* __restrict__ beta_slot, int S, int R, int T, int Cp)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= S * Cp) return;
+    const int sample = t / Cp, c = t % Cp;
+    float b = 0.f;
+    if (c < R * T) b = (float)betas[temp_of_slot[(size_t)sample * R * T + c]];
+    beta_slot[t] = b;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S5: overlap and k_min Fourier modes.  One work item = (replica pair, temperature);
+// a CTA stages MS sites of all Cp copies in shared memory, every thread looks its two copies up
+// through the temperature permutation.  Partial sums per site chunk, reduced in fixed order.
+// ------------------------------------------------------------------------------------------------
+struct MeasureParams {
+    const float* spins;        // [S][NG][N][3][G]
+    const int* slot_of_temp;   // [S][R][T]
+    const double* phase;       // [L][2] cos, sin of 2 pi x / L
+    double* Mpart;             // [S][nchunk][PT][7]
+    int L, N, NG, Cp, R, T, P, nchunk, chunk_sites, MS;
+};
+
+__global__ void k_measure(const MeasureParams p)
+{
+    extern __shared__ float sm[];   // [MS][3][Cp]
+    const int chunk = blockIdx.x, sample = blockIdx.y;
+    const int PT = p.P * p.T;
+    const int item = blockIdx.z * blockDim.x + threadIdx.x;
+    int ca = 0, cb = 0;
+    const bool live = item < PT;
+    if (live) {
+        const int pr = item / p.T, t = item % p.T;
+        int a = 0, rem = pr;                       // pair index -> (a, b), a < b, lexicographic
+        while (rem >= p.R - 1 - a) { rem -= p.R - 1 - a; ++a; }
+        const int b = a + 1 + rem;
+        ca = a * p.T + p.slot_of_temp[((size_t)sample * p.R + a) * p.T + t];
+        cb = b * p.T + p.slot_of_temp[((size_t)sample * p.R + b) * p.T + t];
+    }
+    double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };
+    const int i_begin = chunk * p.chunk_sites, i_end = min(p.N, i_begin + p.chunk_sites);
+    const float* base = p.spins + (size_t)sample * p.NG * p.N * SITE_FLOATS;
+    const int row = 3 * p.Cp;
+    for (int i0 = i_begin; i0 < i_end; i0 += p.MS) {
+        const int ms = min(p.MS, i_end - i0);
+        __syncthreads();
+        for (int e = threadIdx.x; e < ms * p.NG * SITE_FLOATS; e += blockDim.x) {
+            const int lane = e % G, comp = (e / G) % 3, grp = (e / SITE_FLOATS) % p.NG, m = e / (SITE_FLOATS * p.NG);
+            sm[m * row + comp * p.Cp + grp * G + lane] =
+                base[((size_t)grp * p.N + (i0 + m)) * SITE_FLOATS + comp * G + lane];
+        }
+        __syncthreads();
+        if (live) {
+            for (int m = 0; m < ms; ++m) {
+                const float* s = sm + m * row;
+                const float qf = fmaf(s[ca], s[cb], fmaf(s[p.Cp + ca], s[p.Cp + cb], s[2 * p.Cp + ca] * s[2 * p.Cp + cb]));
+                const double qx = (double)qf;
+                const int i = i0 + m;
+                const int x[3] = { i % p.L, (i / p.L) % p.L, i / (p.L * p.L) };
+                acc[0] += qx;
+#pragma unroll
+                for (int mu = 0; mu < 3; ++mu) {
+                    acc[1 + 2 * mu] = fma(qx, p.phase[2 * x[mu]], acc[1 + 2 * mu]);
+                    acc[2 + 2 * mu] = fma(qx, p.phase[2 * x[mu] + 1], acc[2 + 2 * mu]);
+                }
+            }
+        }
+    }
+    if (live) {
+        double* dst = p.Mpart + (((size_t)sample * p.nchunk + chunk) * PT + item) * 7;
+#pragma unroll
+        for (int k = 0; k < 7; ++k) dst[k] = acc[k];
+    }
+}
+
+// result = [ e[S][R][T] | q0[S][P][T] | qk[S][P][T][3][2] ]
+__global__ void k_reduce_measure(const double* __restrict__ Mpart, const double* __restrict__ E,
+                                 const int* __restrict__ slot_of_temp, double* __restrict__ result,
+                                 int S, int R, int T, int P, int Cp, int nchunk, int N)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nE = S * R * T, PT = P * T, nQ = S * PT;
+    const double invN = 1.0 / (double)N;
+    if (t < nE) {
+        const int sample = t / (R * T), r = (t / T) % R;
+        result[t] = E[(size_t)sample * Cp + r * T + slot_of_temp[t]] * invN;
+    } else if (t < nE + nQ * 7) {
+        const int u = t - nE;
+        const int k = u % 7, item = (u / 7) % PT, sample = u / (7 * PT);
+        double acc = 0.0;
+        for (int c = 0; c < nchunk; ++c) acc += Mpart[(((size_t)sample * nchunk + c) * PT + item) * 7 + k];
+        acc *= invN;
+        if (k == 0) result[nE + (size_t)sample * PT + item] = acc;
+        else result[nE + nQ + ((size_t)sample * PT + item) * 6 + (k - 1)] = acc;
+    }
+}
+
+}  // namespace sg

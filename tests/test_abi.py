@@ -1,0 +1,99 @@
+"""CPU-only checks of the boundary: the library builds, loads, exports every symbol the header
+declares, validates arguments, and fails loudly (no CPU fallback) when there is no device."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1309_1599_b200 import build, binding
+    build.build()
+    return binding.load_library()
+
+
+def header_symbols():
+    text = open(os.path.join(ROOT, "include", "sg_b200.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(sg_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    from paper_1309_1599_b200 import binding
+    syms = header_symbols()
+    assert sorted(binding.DECLARED_SYMBOLS) == syms
+    for s in syms:
+        assert hasattr(lib, s), s
+
+
+def test_host_philox_known_answers(lib):
+    from paper_1309_1599_b200 import binding
+    rows = [l.split() for l in open(os.path.join(ROOT, "tests", "golden", "philox4x32_10_kat.txt")) if not l.startswith("#")]
+    for r in rows:
+        v = [int(t, 16) for t in r if t != "->"]
+        assert binding.philox4x32_10(v[0:4], v[4:6]) == v[6:10]
+
+
+def test_workspace_bytes_and_shape_validation(lib):
+    from paper_1309_1599_b200 import binding
+    wb = binding.workspace_bytes
+    assert wb(4, 1, 2, 4) > 0
+    # cfg 4: spins 2.42 GB + gathered couplings + raw couplings + staging, well under 180 GB
+    b4 = wb(64, 4, 4, 48)
+    assert 2.4e9 < b4 < 4e9
+    assert wb(5, 1, 2, 4) == 0          # odd L: no periodic checkerboard (reading R4)
+    assert wb(0, 1, 2, 4) == 0 and wb(4, 0, 2, 4) == 0 and wb(4, 1, 0, 4) == 0 and wb(4, 1, 2, 0) == 0
+    assert wb(4, 1, 2, 4, first_sample=-1) == 0
+    assert wb(2, 1, 1, 1) > 0           # smallest legal shape
+
+
+def test_create_rejects_bad_arguments_without_a_device(lib):
+    from paper_1309_1599_b200 import binding
+    shape = binding.SgShape(4, 1, 2, 4, 0, 0, 1)
+    ctx = ctypes.c_void_p()
+    betas = np.array([0.6, 0.9, 1.2, 1.6])
+    fake = ctypes.c_void_p(256 * 1000)
+    big = 1 << 30
+    call = lambda sh, b, ws, n: lib.sg_create(ctypes.byref(ctx), ctypes.byref(sh), b, ws, n, None)
+    bp = lambda a: ctypes.c_void_p(a.ctypes.data)
+    assert call(shape, None, fake, big) == binding.SG_EINVAL
+    assert call(shape, bp(betas), None, big) == binding.SG_EINVAL
+    assert call(shape, bp(betas), ctypes.c_void_p(256 * 1000 + 4), big) == binding.SG_EINVAL      # misaligned
+    assert call(shape, bp(betas), fake, 16) == binding.SG_EINVAL                                   # too small
+    assert call(shape, bp(np.array([0.6, 0.9, 0.9, 1.6])), fake, big) == binding.SG_EINVAL         # not strictly monotone
+    assert call(shape, bp(np.array([0.6, np.nan, 1.2, 1.6])), fake, big) == binding.SG_EINVAL
+    assert call(shape, bp(np.array([0.6, 1.2, 0.9, 1.6])), fake, big) == binding.SG_EINVAL
+    assert call(binding.SgShape(3, 1, 2, 4, 0, 0, 1), bp(betas), fake, big) == binding.SG_EINVAL
+    assert ctx.value is None
+    for fn in (lib.sg_sweep_or, lib.sg_sweep_hb):
+        assert fn(None, 1) == binding.SG_EINVAL
+    assert lib.sg_pt_swap(None) == binding.SG_EINVAL
+    assert lib.sg_measure(None, None, None, None) == binding.SG_EINVAL
+    assert lib.sg_strerror(binding.SG_ECUDA).decode().startswith("CUDA")
+
+
+def test_no_cpu_fallback():
+    """Without a CUDA device the product path must fail loudly, not compute on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    import paper_1309_1599_b200 as sg
+    with pytest.raises(sg.SgError):
+        sg.SpinGlass(4, 1, 2, 4, [0.6, 0.9, 1.2, 1.6])
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1309_1599_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "sg_oracle" not in text and "import oracle" not in text and "from oracle" not in text, f
+    otext = open(os.path.join(ROOT, "oracle", "sg_oracle.py")).read() + open(os.path.join(ROOT, "oracle", "sg_oracle.c")).read()
+    assert "paper_1309_1599_b200" not in otext and "sg_device" not in otext and "sg_kernels" not in otext
+    assert not re.search(r"#include\s+\"[^\"]*sg_b200", otext) and "libsg_b200" not in otext

@@ -1,0 +1,342 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerances are the north star's: spins after one sweep <= 1e-5 absolute per
+component (ill-conditioned sites excluded by the oracle's flags), energy per
+spin within 1e-6*max(1,|e|), identical PT decisions on identical energies."""
+import numpy as np
+import pytest
+
+import sg_workloads as W
+from tests.util import gpu_spins, make_pair, neighbour_dilate, oracle_spins
+
+pytestmark = pytest.mark.gpu
+
+SPIN_TOL = 1e-5
+MAX_FLAG_FRACTION = 1e-4
+
+
+@pytest.fixture(scope="module")
+def sg():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1309_1599_b200 import build
+    build.build()
+    import paper_1309_1599_b200 as mod
+    return mod
+
+
+# shapes: cfg 0; the generic (non power-of-two) path with a ragged tile and a padded copy group; L = 2;
+# several tiles with a ragged tail (L = 10: 500 sites per colour = 3 tiles of 128 + 116); cfg-1-like
+SHAPES = [
+    dict(L=4, S=1, R=2, T=4, b=(0.6, 1.6)),
+    dict(L=2, S=2, R=2, T=3, b=(0.5, 1.5)),
+    dict(L=6, S=2, R=4, T=10, b=(0.5, 2.0)),
+    dict(L=10, S=1, R=3, T=11, b=(0.4, 2.4)),
+    dict(L=8, S=3, R=4, T=16, b=(0.5, 2.0)),
+    dict(L=16, S=1, R=2, T=20, b=(0.5, 2.2)),
+]
+
+
+def betas_of(sh):
+    return np.linspace(sh["b"][0], sh["b"][1], sh["T"])
+
+
+def colour_mask(L):
+    idx = np.arange(L ** 3)
+    return (idx % L + (idx // L) % L + idx // (L * L)) % 2
+
+
+def assert_spins_close(got, want, exclude, what):
+    """got, want [S][C][3][N]; exclude [S][C][N] bool."""
+    frac = exclude.mean()
+    assert frac <= max(MAX_FLAG_FRACTION * 6, 2.0 / exclude.size), (what, "flagged fraction", frac)
+    err = np.abs(got - want).max(axis=2)
+    err = np.where(exclude, 0.0, err)
+    assert err.max() <= SPIN_TOL, (what, err.max(), np.unravel_index(err.argmax(), err.shape))
+
+
+# ---------------------------------------------------------------------------------------------
+# S0
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode,sigma", [(0, 1.0), (0, 2 ** 0.5), (1, 0.5), (2, 1.0), (3, 0.5), (4, 0.0)])
+def test_coupling_generator_matches_oracle(sg, oracle, mode, sigma):
+    L, S = 6, 2
+    gpu = sg.SpinGlass(L, S, 2, 3, [0.5, 1.0, 1.5], seed=12345678901234, first_sample=7)
+    for s in range(S):
+        gpu.init_sample(s, mode, sigma)
+        want = oracle.gen_couplings(L, 12345678901234, 7 + s, mode, sigma)
+        got = gpu.get_couplings(s).astype(np.float64)
+        # same Philox words, same fp64 formulae, rounded to fp32 on both sides: bit-exact up to the
+        # last fp32 bit of libm's last-ulp freedom
+        assert np.abs(got - want).max() <= 1.2e-7 * max(1.0, np.abs(want).max())
+        assert (got != want).mean() < 1e-3
+
+
+@pytest.mark.parametrize("sh", SHAPES[:4])
+def test_initial_spins_match_oracle(sg, oracle, sh):
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    gpu = sg.SpinGlass(L, S, R, T, betas_of(sh), seed=99, first_sample=3)
+    for s in range(S):
+        gpu.init_sample(s)
+        got = gpu.get_spins(s).astype(np.float64)
+        want = np.stack([oracle.gen_spins(L, 99, (3 + s) * R * T + c) for c in range(R * T)])
+        assert np.abs(got - want).max() <= 5e-7
+        tos, sot = gpu.get_perm(s)
+        assert np.array_equal(tos, np.tile(np.arange(T), (R, 1))) and np.array_equal(sot, tos)
+
+
+@pytest.mark.parametrize("sh", SHAPES)
+def test_set_get_spins_roundtrip(sg, sh):
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    rng = np.random.default_rng(L)
+    gpu = sg.SpinGlass(L, S, R, T, betas_of(sh))
+    data = [W.random_spins(rng, R * T, L ** 3).astype(np.float32) for _ in range(S)]
+    for s in range(S):
+        gpu.init_sample(s, spins=data[s])
+    for s in range(S):
+        assert np.array_equal(gpu.get_spins(s), data[s])
+    gpu.set_spins(0, data[-1])
+    assert np.array_equal(gpu.get_spins(0), data[-1])
+
+
+# ---------------------------------------------------------------------------------------------
+# S1, S2: half-sweeps and sweeps, element by element
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("sh", SHAPES)
+@pytest.mark.parametrize("kind", [0, 1])
+@pytest.mark.parametrize("gen_mode", [0, 2])
+def test_half_sweeps_match_oracle(sg, oracle, sh, kind, gen_mode):
+    """Each colour separately, each compared from the oracle's state (no error propagation)."""
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=5, gen_mode=gen_mode)
+    sim.hb_counter = 17
+    gpu.set_counters(17, 0)
+    col = colour_mask(L)
+    for colour in (0, 1):
+        before = oracle_spins(sim)
+        for s in range(S):
+            gpu.set_spins(s, sim.spins[s].astype(np.float32))      # restart from the oracle's state
+        flags = sim.halfsweep(kind, colour, want_flags=True)
+        gpu.halfsweep(kind, colour)
+        got, want = gpu_spins(gpu), oracle_spins(sim)
+        assert_spins_close(got, want, flags != 0, ("half", kind, colour))
+        other = col != colour
+        assert np.array_equal(got[..., other], before[..., other])       # the other colour is untouched
+        assert np.abs(want[..., ~other] - before[..., ~other]).max() > 0.1
+    assert gpu.get_counters() == (17, 0)
+
+
+@pytest.mark.parametrize("sh", SHAPES)
+@pytest.mark.parametrize("kind", [0, 1])
+def test_full_sweep_matches_oracle(sg, oracle, sh, kind):
+    """north_star: spins after one sweep within 1e-5 absolute per component; energy per spin within 1e-6."""
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    N = L ** 3
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=6)
+    f0 = sim.halfsweep(kind, 0, want_flags=True)
+    f1 = sim.halfsweep(kind, 1, want_flags=True)
+    if kind == 1:
+        sim.hb_counter += 1
+        gpu.sweep_hb(1)
+    else:
+        gpu.sweep_or(1)
+    exclude = (f0 != 0) | (f1 != 0) | neighbour_dilate(f0 != 0, L)
+    assert_spins_close(gpu_spins(gpu), oracle_spins(sim), exclude, ("sweep", kind))
+    # fused energy of the sweep's last half-sweep against Eq. (1) on the oracle's spins
+    e_gpu, e_ref = gpu.get_energies() / N, sim.energies() / N
+    assert np.all(np.abs(e_gpu - e_ref) <= 1e-6 * np.maximum(1.0, np.abs(e_ref)) + 2e-5 * exclude.any())
+    assert gpu.get_counters()[0] == (1 if kind == 1 else 0)
+
+
+def test_or_conserves_energy_and_norm_on_gpu(sg, oracle):
+    sh = SHAPES[4]
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    N = L ** 3
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=8)
+    e0 = gpu.get_energies() / N                   # standalone energy kernel
+    assert np.all(np.abs(e0 - sim.energies() / N) <= 1e-6 * np.maximum(1.0, np.abs(e0)))
+    gpu.sweep_or(8)
+    e1 = gpu.get_energies() / N                   # fused into the last half-sweep
+    assert np.abs(e1 - e0).max() < 2e-5           # fp32 reflections: drift ~ sqrt(sweeps) * 1e-7 * |h|
+    s = gpu_spins(gpu)
+    assert np.abs(np.sum(s * s, axis=2) - 1.0).max() < 2e-5
+    for smp in range(S):                          # fused vs standalone reduction on the same state
+        gpu.set_spins(smp, gpu.get_spins(smp))
+    e2 = gpu.get_energies() / N
+    assert np.abs(e2 - e1).max() < 1e-6
+
+
+def test_time_reversal_and_involution_on_gpu(sg, oracle):
+    sh = SHAPES[2]
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=9, gen_mode=2)
+    s0 = gpu_spins(gpu)
+    gpu.halfsweep(0, 0)
+    s1 = gpu_spins(gpu)
+    gpu.halfsweep(0, 0)
+    assert np.abs(gpu_spins(gpu) - s0).max() < 5e-5       # reflection twice = identity (up to fp32; small |h| sites)
+    for s in range(S):
+        gpu.set_spins(s, (-s0[s]).astype(np.float32))
+    gpu.halfsweep(0, 0)
+    assert np.array_equal(gpu_spins(gpu), -s1)            # OR(-s) = -OR(s) exactly
+
+
+# ---------------------------------------------------------------------------------------------
+# S3, S5: energies and overlaps
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("sh", SHAPES)
+def test_measure_matches_oracle(sg, oracle, sh):
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=10)
+    rng = np.random.default_rng(3)
+    for s in range(S):                                    # a non-trivial temperature assignment
+        tos = np.stack([rng.permutation(T) for _ in range(R)]).astype(np.int32)
+        gpu.set_perm(s, tos)
+        sim.temp_of_slot[s] = tos
+        sim.slot_of_temp[s] = np.argsort(tos, axis=1).astype(np.int32)
+        got_tos, got_sot = gpu.get_perm(s)
+        assert np.array_equal(got_tos, tos) and np.array_equal(got_sot, sim.slot_of_temp[s])
+    e, q0, qk = gpu.measure()
+    e_ref, q0_ref, qk_ref = sim.measure()
+    assert np.all(np.abs(e - e_ref) <= 1e-6 * np.maximum(1.0, np.abs(e_ref)))
+    assert np.abs(q0 - q0_ref).max() <= 1e-6 and np.abs(qk - qk_ref).max() <= 1e-6
+
+
+def test_measure_closed_forms_on_gpu(sg):
+    """Identical replicas: q(0) = 1, q(k) = 0; a cosine modulation along x_mu: q(k_mu) = 1/2."""
+    L, R, T = 8, 2, 2
+    N = L ** 3
+    rng = np.random.default_rng(4)
+    gpu = sg.SpinGlass(L, 1, R, T, [0.5, 1.0])
+    idx = np.arange(N)
+    coords = [idx % L, (idx // L) % L, idx // (L * L)]
+    base = W.random_spins(rng, 1, N)[0]
+    spins = np.zeros((R * T, 3, N))
+    spins[0] = base; spins[2] = base                       # replica 0 and 1 at temperature 0: identical
+    spins[1, 2] = 1.0                                      # temperature 1: z^ against a modulation along x2
+    th = 2 * np.pi * coords[1] / L
+    spins[3, 0] = np.sin(th); spins[3, 2] = np.cos(th)
+    gpu.init_sample(0, couplings=np.zeros((3, N, 3, 3)), spins=spins)
+    e, q0, qk = gpu.measure()
+    assert np.all(e == 0)
+    assert abs(q0[0, 0, 0] - 1) < 1e-6 and np.abs(qk[0, 0, 0]).max() < 1e-6
+    want = np.zeros((3, 2)); want[1, 0] = 0.5
+    assert abs(q0[0, 0, 1]) < 1e-6 and np.abs(qk[0, 0, 1] - want).max() < 1e-6
+
+
+def test_ferromagnet_energy_on_gpu(sg):
+    """The paper's own cross-check: ferromagnetic couplings, exact energies."""
+    L = 8
+    N = L ** 3
+    gpu = sg.SpinGlass(L, 1, 1, 2, [0.5, 1.0])
+    spins = np.zeros((2, 3, N))
+    spins[0, 1] = 1.0
+    idx = np.arange(N)
+    spins[1, 2] = 1.0 - 2.0 * ((idx % L + (idx // L) % L + idx // (L * L)) % 2)
+    gpu.init_sample(0, sg.GEN_FERRO, 0.0, spins=spins)
+    E = gpu.get_energies()[0] / N
+    assert E[0] == -3.0 and E[1] == 3.0
+
+
+# ---------------------------------------------------------------------------------------------
+# S4: parallel tempering
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("sh", [SHAPES[0], SHAPES[2], SHAPES[4]])
+def test_pt_decisions_identical_on_identical_energies(sg, oracle, sh):
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=11, first_sample=2)
+    rng = np.random.default_rng(5)
+    for k in range(40):
+        # energies spaced so that acceptance is neither 0 nor 1
+        E = rng.normal(0.0, 3.0 / (betas_of(sh)[1] - betas_of(sh)[0]) / 4, size=(S, R * T))
+        gpu.set_energies(E)
+        gpu.pt_swap()
+        sim.pt_swap(energies=E)
+        for s in range(S):
+            tos, sot = gpu.get_perm(s)
+            assert np.array_equal(tos, sim.temp_of_slot[s]) and np.array_equal(sot, sim.slot_of_temp[s]), k
+    att, acc = gpu.pt_stats()
+    assert np.array_equal(att, sim.attempts) and np.array_equal(acc, sim.accepts)
+    assert 0 < acc.sum() < att.sum()
+    assert gpu.get_counters() == (0, 40)
+
+
+def test_pt_moves_temperatures_not_spins_and_hb_follows(sg, oracle):
+    """After PT the heat bath must use each slot's *new* temperature (beta by slot follows the swap)."""
+    sh = SHAPES[0]
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=12)
+    before = gpu_spins(gpu)
+    E = np.array([[0.0, -50.0, -20.0, -90.0, 5.0, 1.0, -3.0, 2.0]])     # forces some swaps
+    gpu.set_energies(E); gpu.pt_swap(); sim.pt_swap(energies=E)
+    assert np.array_equal(gpu_spins(gpu), before)
+    tos, _ = gpu.get_perm(0)
+    assert np.array_equal(tos, sim.temp_of_slot[0]) and not np.array_equal(tos, np.tile(np.arange(T), (R, 1)))
+    f0 = sim.halfsweep(1, 0, want_flags=True)
+    gpu.halfsweep(1, 0)
+    assert_spins_close(gpu_spins(gpu), oracle_spins(sim), f0 != 0, "hb after pt")
+
+
+def test_unit_sequence_with_resync(sg, oracle):
+    """Three units of cfg 0 (1 HB + 4 OR + PT): every sweep is compared from the oracle's state, PT is
+    compared on the GPU's own energies (decisions may differ only at a near-tie)."""
+    cfg = W.CONFIGS[0]
+    L, S, R, T = cfg.L, cfg.n_samples, cfg.n_replicas, cfg.n_temps
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, cfg.betas, seed=cfg.seed)
+    N = L ** 3
+    for unit in range(3):
+        for kind, n in ((1, 1), (0, cfg.n_or)):
+            for _ in range(n):
+                for s in range(S):
+                    gpu.set_spins(s, sim.spins[s].astype(np.float32))
+                f0 = sim.halfsweep(kind, 0, want_flags=True)
+                f1 = sim.halfsweep(kind, 1, want_flags=True)
+                if kind == 1:
+                    sim.hb_counter += 1
+                    gpu.sweep_hb(1)
+                else:
+                    gpu.sweep_or(1)
+                exclude = (f0 != 0) | (f1 != 0) | neighbour_dilate(f0 != 0, L)
+                assert_spins_close(gpu_spins(gpu), oracle_spins(sim), exclude, ("unit", unit, kind))
+        E_gpu, E_ref = gpu.get_energies(), sim.energies()
+        assert np.all(np.abs(E_gpu - E_ref) / N <= 1e-6 * np.maximum(1.0, np.abs(E_ref) / N))
+        gpu.pt_swap()
+        sim.pt_swap(energies=E_gpu)              # same energies -> the decisions must be identical
+        tos, sot = gpu.get_perm(0)
+        assert np.array_equal(tos, sim.temp_of_slot[0])
+        assert gpu.get_counters() == (sim.hb_counter, sim.pt_counter)
+
+
+def test_sharded_samples_draw_the_single_process_numbers(sg, oracle):
+    """first_sample shifts every Philox counter: a context holding samples [2,4) reproduces samples 2, 3 of
+    a context holding [0,4) (weak-scaling shard by sample)."""
+    L, R, T = 4, 2, 4
+    betas = np.linspace(0.6, 1.6, T)
+    full = sg.SpinGlass(L, 4, R, T, betas, seed=21)
+    part = sg.SpinGlass(L, 2, R, T, betas, seed=21, first_sample=2)
+    for s in range(4):
+        full.init_sample(s)
+    for s in range(2):
+        part.init_sample(s)
+    for g in (full, part):
+        g.unit(3); g.unit(3)
+    for s in range(2):
+        assert np.array_equal(part.get_couplings(s), full.get_couplings(2 + s))
+        assert np.array_equal(part.get_spins(s), full.get_spins(2 + s))
+        assert np.array_equal(part.get_perm(s)[0], full.get_perm(2 + s)[0])
+    assert np.array_equal(part.get_energies(), full.get_energies()[2:])
+
+
+def test_errors_on_gpu(sg):
+    gpu = sg.SpinGlass(4, 2, 2, 4, np.linspace(0.6, 1.6, 4))
+    gpu.init_sample(0)
+    with pytest.raises(sg.SgError) as ei:
+        gpu.sweep_or(1)                          # sample 1 not initialised
+    assert ei.value.code == -2
+    with pytest.raises(sg.SgError):
+        gpu.init_sample(5)
+    with pytest.raises(sg.SgError):
+        gpu.set_perm(0, np.zeros((2, 4), dtype=np.int32))
+    gpu.init_sample(1)
+    n0 = gpu.kernel_launches()
+    gpu.sweep_or(2)
+    assert gpu.kernel_launches() == n0 + 5       # 4 half-sweeps + 1 energy reduction
