@@ -310,10 +310,11 @@ static uint8_t sgo_flag(const double h[3], int kind)
  * r1 = u23(w0), r2 = u23(w1).  store_fp32 != 0 rounds each new spin component to the nearest fp32
  * (the state precision of reading R20); 0 keeps full doubles (used by the invariance pins).
  * flags (may be NULL): per-site ill-conditioning flag of the sites updated, others untouched.
+ * hnorm (may be NULL): |h_x| of the sites updated (the tests propagate measured errors with it).
  * sd (may be NULL): accumulates over the updated sites sum s_new.h, sum h.h, sum (s_new.h)^2 (Eq. (A6)). */
 void sgo_halfsweep(int L, const double* M, double* s, int kind, int colour, double beta,
                    uint64_t seed, uint32_t g, uint32_t hb_counter, int store_fp32,
-                   uint8_t* flags, double sd[3])
+                   uint8_t* flags, double* hnorm, double sd[3])
 {
     int N = L * L * L;
     for (int i = 0; i < N; ++i) {
@@ -329,6 +330,7 @@ void sgo_halfsweep(int L, const double* M, double* s, int kind, int colour, doub
         }
         for (int a = 0; a < 3; ++a) s[a * N + i] = store_fp32 ? (double)(float)sx[a] : sx[a];
         if (flags) flags[i] = sgo_flag(h, kind);
+        if (hnorm) hnorm[i] = sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
         if (sd) {
             double sh = sx[0] * h[0] + sx[1] * h[1] + sx[2] * h[2];
             sd[0] += sh;
@@ -352,7 +354,7 @@ void sgo_sweep_copies(int L, const double* M, double* spins, int n_copies, int k
         for (int k = 0; k < n_sweeps; ++k)
             for (int colour = 0; colour < 2; ++colour)
                 sgo_halfsweep(L, M, spins + c * stride, kind, colour, kind ? beta_of_copy[c] : 0.0,
-                              seed, g0 + (uint32_t)c, hb_counter0 + (uint32_t)k, store_fp32, NULL, NULL);
+                              seed, g0 + (uint32_t)c, hb_counter0 + (uint32_t)k, store_fp32, NULL, NULL, NULL);
 }
 
 void sgo_energy_copies(int L, const double* M, const double* spins, int n_copies, double* E)

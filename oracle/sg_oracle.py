@@ -57,7 +57,7 @@ def lib():
         L.sgo_energy_from_fields.argtypes = [i, dp, dp, i]; L.sgo_energy_from_fields.restype = d
         L.sgo_or_update.argtypes = [dp, dp]
         L.sgo_hb_update.argtypes = [dp, d, d, d, dp]
-        L.sgo_halfsweep.argtypes = [i, dp, dp, i, i, d, u64, u32, u32, i, u8p, dp]
+        L.sgo_halfsweep.argtypes = [i, dp, dp, i, i, d, u64, u32, u32, i, u8p, dp, dp]
         L.sgo_sweep_copies.argtypes = [i, dp, dp, i, i, i, dp, u64, u32, u32, i]
         L.sgo_energy_copies.argtypes = [i, dp, dp, i, dp]
         L.sgo_num_threads.restype = i
@@ -146,13 +146,15 @@ def hb_update(h, beta, r1, r2):
 
 
 def halfsweep(L, M, s, kind, colour, beta=0.0, seed=0, g=0, hb_counter=0, store_fp32=False,
-              want_flags=False, want_sd=False):
-    """In-place half-sweep of one copy `s` ([3][N] float64).  Returns (flags or None, sd or None)."""
+              want_flags=False, want_sd=False, hnorm_out=None):
+    """In-place half-sweep of one copy `s` ([3][N] float64).  Returns (flags or None, sd or None);
+    hnorm_out ([N] float64, optional) receives |h_x| of the updated sites."""
     flags = np.zeros(L ** 3, dtype=np.uint8) if want_flags else None
     sd = np.zeros(3) if want_sd else None
     lib().sgo_halfsweep(L, _dp(M), _dp(s), int(kind), int(colour), float(beta), int(seed), int(g),
                         int(hb_counter), int(bool(store_fp32)),
                         flags.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8)) if want_flags else None,
+                        _dp(hnorm_out) if hnorm_out is not None else None,
                         _dp(sd) if want_sd else None)
     return flags, sd
 
@@ -250,17 +252,20 @@ class OracleSim:
                          self.g0(s), self.hb_counter, self.store_fp32)
         self.hb_counter += n_sweeps
 
-    def halfsweep(self, kind, colour, want_flags=False):
-        """One colour of every copy with the current HB counter (not advanced).  Returns flags [S][C][N]."""
+    def halfsweep(self, kind, colour, want_flags=False, want_hnorm=False):
+        """One colour of every copy with the current HB counter (not advanced).  Returns flags [S][C][N]
+        (and, with want_hnorm, also |h_x| [S][C][N] of the updated sites, 0 elsewhere)."""
         out = np.zeros((self.S, self.C, self.N), dtype=np.uint8) if want_flags else None
+        hn = np.zeros((self.S, self.C, self.N)) if want_hnorm else None
         for s in range(self.S):
             b = self.beta_of_copy(s)
             for c in range(self.C):
                 f, _ = halfsweep(self.L, self.M[s], self.spins[s][c], kind, colour, b[c], self.seed,
-                                 self.g0(s) + c, self.hb_counter, self.store_fp32, want_flags=want_flags)
+                                 self.g0(s) + c, self.hb_counter, self.store_fp32, want_flags=want_flags,
+                                 hnorm_out=hn[s, c] if want_hnorm else None)
                 if want_flags:
                     out[s, c] = f
-        return out
+        return (out, hn) if want_hnorm else out
 
     def energies(self):
         """Total H of every slot, [S][C]."""

@@ -1,0 +1,55 @@
+"""Host logic of the weak-scaling run (paper_1309_1599_b200/multi.py) with two gloo processes on CPU:
+sample sharding, the barrier, max-over-ranks timing and the whole-job rate.  No GPU, no oracle."""
+import os
+import socket
+
+import pytest
+import torch.multiprocessing as mp
+
+from paper_1309_1599_b200 import multi
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    assert multi.env_rank() == (rank, rank, world)
+    assert multi.init_process_group("gloo", world)
+    multi.barrier()
+    first = multi.first_sample_of_rank(rank, 4)
+    seconds = 1.0 + rank                       # rank 1 is the slow one
+    rate, total, slowest = multi.whole_job_rate(100.0 * (rank + 1), seconds)
+    out.put((rank, first, multi.max_over_ranks(seconds), multi.sum_over_ranks(first), rate, total, slowest))
+    multi.barrier()
+    import torch.distributed as dist
+    dist.destroy_process_group()
+
+
+def test_two_rank_gloo_sharding_and_reduction():
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted(out.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert [g[1] for g in got] == [0, 4]                       # disjoint, contiguous sample ranges
+    for g in got:
+        assert g[2] == 2.0 and g[3] == 4.0                     # max / sum agree on every rank
+        assert g[5] == 300.0 and g[6] == 2.0 and g[4] == 150.0  # all units / slowest rank
+
+
+def test_single_process_passthrough():
+    assert multi.max_over_ranks(3.5) == 3.5 and multi.sum_over_ranks(2.0) == 2.0
+    assert multi.whole_job_rate(10.0, 2.0) == (5.0, 10.0, 2.0)
+    assert multi.first_sample_of_rank(3, 4) == 12
+    with pytest.raises(ValueError):
+        multi.first_sample_of_rank(-1, 4)

@@ -31,3 +31,4 @@ def gpu_spins(gpu):
 
 def oracle_spins(sim):
     return np.stack(sim.spins)
+
