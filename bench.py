@@ -176,6 +176,9 @@ def run_ours(args, cfg):
 
     S, R, T, L, N, C = cfg.n_samples, cfg.n_replicas, cfg.n_temps, cfg.L, cfg.n_sites, cfg.n_copies
     gpu = sg.SpinGlass(L, S, R, T, cfg.betas, seed=cfg.seed, first_sample=multi.first_sample_of_rank(rank, S))
+    gpu.tune(sg.TUNE_SWEEP_IMPL, {"auto": sg.SWEEP_AUTO, "tiled": sg.SWEEP_TILED, "zmarch": sg.SWEEP_ZMARCH}[args.sweep_impl])
+    if args.zchunk:
+        gpu.tune(sg.TUNE_ZCHUNK, args.zchunk)
     for s in range(S):
         gpu.init_sample(s, sg.GEN_OFFDIAG_SYM, cfg.sigma_D)
     state_bytes = S * C * N * 12
@@ -262,7 +265,8 @@ def run_ours(args, cfg):
                 "steps": e2e_steps, "what": "per step: sg_set_spins of every sample from pinned host memory, "
                                             "one unit, sg_measure to host"},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "kernel": "k_sweep<OR> (one checkerboard half-sweep of all copies)",
+        "roofline": {"bound": "hbm", "kernel": "OR half-sweep (k_sweep_zm<OR> for L %% 8 == 0, else k_sweep<OR>), sweep_impl=%s zchunk=%d"
+                                                  % (args.sweep_impl, args.zchunk),
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                      "peak_source": peak_src, "alg_bytes_per_update": algorithmic_bytes_per_update(C),
                      "updates_per_launch": updates_per_launch, "launch_us": or_launch_s * 1e6,
@@ -291,6 +295,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (default: the headline cfg 4)")
+    ap.add_argument("--sweep-impl", default="auto", choices=["auto", "tiled", "zmarch"],
+                    help="sg_tune(SG_TUNE_SWEEP_IMPL): which half-sweep kernel serves the sweeps (default: the library's choice)")
+    ap.add_argument("--zchunk", type=int, default=0, help="sg_tune(SG_TUNE_ZCHUNK): planes per CTA of the z-marching kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (profiling runs)")
     args = ap.parse_args()
     if args.impl == "ours":

@@ -126,6 +126,16 @@ int sg_halfsweep(sg_ctx* ctx, int kind, int colour);
 /* PT statistics since creation, uint64 [S][R][T-1] each (either may be NULL). */
 int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts);
 
+/* ---- tuning (results do not depend on it beyond floating-point summation order) ----
+ * SG_TUNE_SWEEP_IMPL: which half-sweep kernel serves sg_sweep_or / sg_sweep_hb / the energy pass.
+ *   SG_SWEEP_AUTO   z-marching kernel when L is a multiple of 8, else the tiled kernel (default)
+ *   SG_SWEEP_TILED  the tiled kernel (any even L)
+ *   SG_SWEEP_ZMARCH the z-marching kernel; SG_EINVAL unless L is a multiple of 8
+ * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else >= 4 and a divisor of L. */
+enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1 };
+enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2 };
+int sg_tune(sg_ctx* ctx, int knob, int value);
+
 /* ---- utilities ---- */
 int sg_sync(sg_ctx* ctx);                       /* cudaStreamSynchronize on the context's stream        */
 uint64_t sg_kernel_launches(const sg_ctx* ctx); /* kernels launched by this context so far              */

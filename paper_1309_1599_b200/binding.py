@@ -12,13 +12,15 @@ _LIB_PATH = os.path.join(_HERE, "libsg_b200.so")
 GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2, 3, 4
 KIND_OR, KIND_HB = 0, 1
 SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
+TUNE_SWEEP_IMPL, TUNE_ZCHUNK = 0, 1
+SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH = 0, 1, 2
 
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_sweep_or", "sg_sweep_hb",
     "sg_pt_swap", "sg_measure", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
-    "sg_halfsweep", "sg_pt_stats", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
+    "sg_halfsweep", "sg_pt_stats", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
 ]
 
@@ -69,6 +71,7 @@ def load_library():
     L.sg_set_counters.argtypes = [vp, u64, u64]; L.sg_set_counters.restype = i
     L.sg_halfsweep.argtypes = [vp, i, i]; L.sg_halfsweep.restype = i
     L.sg_pt_stats.argtypes = [vp, vp, vp]; L.sg_pt_stats.restype = i
+    L.sg_tune.argtypes = [vp, i, i]; L.sg_tune.restype = i
     L.sg_sync.argtypes = [vp]; L.sg_sync.restype = i
     L.sg_kernel_launches.argtypes = [vp]; L.sg_kernel_launches.restype = u64
     L.sg_last_cuda_error.argtypes = [vp]; L.sg_last_cuda_error.restype = i
@@ -227,6 +230,9 @@ class SpinGlass:
         att = np.zeros((self.S, self.R, n), dtype=np.uint64); acc = np.zeros((self.S, self.R, n), dtype=np.uint64)
         self._check(self._lib.sg_pt_stats(self._ctx, _ptr(att), _ptr(acc)), "sg_pt_stats")
         return att, acc
+
+    def tune(self, knob, value):
+        self._check(self._lib.sg_tune(self._ctx, int(knob), int(value)), "sg_tune")
 
     def sync(self):
         self._check(self._lib.sg_sync(self._ctx), "sg_sync")

@@ -24,6 +24,10 @@ struct sg_ctx {
     unsigned long long* attempts; unsigned long long* accepts;
     // sweep geometry
     int tile_sites, ntiles, log2L;
+    // z-marching sweep (L a multiple of 8): tuning knobs and the derived chunking
+    int sweep_impl;   // SG_SWEEP_AUTO / SG_SWEEP_TILED / SG_SWEEP_ZMARCH
+    int zm_zc_req;    // requested planes per chunk, 0 = automatic
+    int zm_ok, zm_ZC, zm_nzc;
     // measure geometry
     int nchunk, chunk_sites, MS;
     // host state
@@ -202,9 +206,74 @@ void launch_sweep_l(sg_ctx* ctx, const SweepParams& p, dim3 grid)
     }
 }
 
+// ---- z-marching sweep: 8 x 8 columns, ring of NST other-colour planes and NJ coupling stages ----
+constexpr int ZM_TX = 8, ZM_TY = 8, ZM_NST = 5, ZM_NJ = 3;
+
+void zm_plan(sg_ctx* ctx)
+{
+    const int L = ctx->L;
+    ctx->zm_ok = (L % 8 == 0) ? 1 : 0;
+    ctx->zm_ZC = 0; ctx->zm_nzc = 0;
+    if (!ctx->zm_ok) return;
+    int ZC = 0;
+    if (ctx->zm_zc_req > 0) {
+        ZC = ctx->zm_zc_req;
+    } else {
+        // the longest chunk that still gives every SM several CTAs' worth of work in turn (2 CTAs per SM x 148 SMs
+        // per wave); a chunk re-reads 2 planes of other-colour sites per ZC planes
+        const long per_plane_col = (long)ctx->S * ctx->NG * (L / ZM_TX) * (L / ZM_TY);
+        ZC = L;
+        while (ZC > 8 && per_plane_col * (L / ZC) < 6 * 296) ZC /= 2;
+    }
+    ctx->zm_ZC = ZC; ctx->zm_nzc = L / ZC;
+}
+
+template <int KIND, bool WITH_E>
+int launch_zm(sg_ctx* ctx, const ZmParams& p, dim3 grid)
+{
+    auto kern = k_sweep_zm<KIND, WITH_E, ZM_TX, ZM_TY, ZM_NST, ZM_NJ>;
+    constexpr size_t smem = zm_smem_bytes<ZM_TX, ZM_TY, ZM_NST, ZM_NJ>();
+    static bool attr_done = false;   // per process and template instance; the attribute is per function
+    if (!attr_done) {
+        SG_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    kern<<<grid, ZmGeom<ZM_TX, ZM_TY>::THREADS, smem, ctx->stream>>>(p);
+    return SG_OK;
+}
+
+int half_sweep_zm(sg_ctx* ctx, int kind, int colour, bool with_energy)
+{
+    ZmParams p;
+    p.spins = ctx->spins; p.Jg = ctx->Jg; p.beta_slot = ctx->beta_slot; p.Epart = ctx->Epart;
+    p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.C = ctx->C;
+    p.ntx = ctx->L / ZM_TX; p.nty = ctx->L / ZM_TY; p.nzc = ctx->zm_nzc; p.ZC = ctx->zm_ZC;
+    p.colour = colour;
+    p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
+    p.hb_counter = (uint32_t)ctx->hb_counter;
+    p.g_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->C;
+    const int nblk = p.ntx * p.nty * p.nzc;
+    const dim3 grid(nblk * ctx->NG, ctx->S);
+    int rc;
+    if (kind == KIND_OR) rc = with_energy ? launch_zm<KIND_OR, true>(ctx, p, grid) : launch_zm<KIND_OR, false>(ctx, p, grid);
+    else if (kind == KIND_HB) rc = with_energy ? launch_zm<KIND_HB, true>(ctx, p, grid) : launch_zm<KIND_HB, false>(ctx, p, grid);
+    else rc = launch_zm<KIND_ENERGY, true>(ctx, p, grid);
+    if (rc != SG_OK) return rc;
+    SG_LAUNCHED(ctx);
+    if (with_energy || kind == KIND_ENERGY) {
+        k_reduce_energy<<<ctx->S * ctx->NG, 256, 0, ctx->stream>>>(ctx->Epart, ctx->E, nblk);
+        SG_LAUNCHED(ctx);
+        ctx->energies_fresh = true;
+    } else {
+        ctx->energies_fresh = false;
+    }
+    return SG_OK;
+}
+
 // one half-sweep of every copy; with_energy also reduces E (valid because a whole colour is swept)
 int half_sweep(sg_ctx* ctx, int kind, int colour, bool with_energy)
 {
+    if (ctx->zm_ok && ctx->sweep_impl != SG_SWEEP_TILED) return half_sweep_zm(ctx, kind, colour, with_energy);
     SweepParams p;
     p.spins = ctx->spins; p.Jg = ctx->Jg; p.beta_slot = ctx->beta_slot; p.Epart = ctx->Epart;
     p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.ntiles = ctx->ntiles;
@@ -212,7 +281,7 @@ int half_sweep(sg_ctx* ctx, int kind, int colour, bool with_energy)
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.hb_counter = (uint32_t)ctx->hb_counter;
     p.g_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->C;
-    const dim3 grid(ctx->ntiles, ctx->NG, ctx->S);
+    const dim3 grid(ctx->ntiles * ctx->NG, ctx->S);
     if (kind == KIND_OR) {
         if (with_energy) launch_sweep_l<KIND_OR, true>(ctx, p, grid);
         else launch_sweep_l<KIND_OR, false>(ctx, p, grid);
@@ -314,6 +383,8 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->h_betas.assign(betas, betas + g.T);
     ctx->inited.assign(g.S, 0);
     ctx->hb_counter = ctx->pt_counter = ctx->launches = 0;
+    ctx->sweep_impl = SG_SWEEP_AUTO; ctx->zm_zc_req = 0;
+    zm_plan(ctx);
     ctx->energies_fresh = false;
     ctx->last_cuda = 0;
 
@@ -569,6 +640,26 @@ int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts)
     if (accepts) SG_CUDA(ctx, cudaMemcpyAsync(accepts, ctx->accepts, n, cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
+}
+
+int sg_tune(sg_ctx* ctx, int knob, int value)
+{
+    if (!ctx) return SG_EINVAL;
+    switch (knob) {
+    case SG_TUNE_SWEEP_IMPL:
+        if (value != SG_SWEEP_AUTO && value != SG_SWEEP_TILED && value != SG_SWEEP_ZMARCH) return SG_EINVAL;
+        if (value == SG_SWEEP_ZMARCH && ctx->L % 8 != 0) return SG_EINVAL;
+        ctx->sweep_impl = value;
+        return SG_OK;
+    case SG_TUNE_ZCHUNK:
+        if (value < 0) return SG_EINVAL;
+        if (value > 0 && (ctx->L % 8 != 0 || value < 4 || ctx->L % value != 0)) return SG_EINVAL;
+        ctx->zm_zc_req = value;
+        zm_plan(ctx);
+        return SG_OK;
+    default:
+        return SG_EINVAL;
+    }
 }
 
 int sg_sync(sg_ctx* ctx)

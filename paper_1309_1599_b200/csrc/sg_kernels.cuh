@@ -2,6 +2,7 @@
 // kernel, the roofline that bounds it and its algorithmic bytes per spin update.
 #pragma once
 #include "sg_device.cuh"
+#include "sg_sweep_zm.cuh"
 
 namespace sg {
 
@@ -16,8 +17,6 @@ namespace sg {
 // ------------------------------------------------------------------------------------------------
 constexpr int SWEEP_THREADS = 256;
 constexpr int SLOTS = SWEEP_THREADS / 8;   // site slots per pass
-
-enum : int { KIND_OR = 0, KIND_HB = 1, KIND_ENERGY = 2 };
 
 struct SweepParams {
     float* spins;            // [S][NG][N][3][G]
@@ -37,7 +36,8 @@ __global__ void __launch_bounds__(SWEEP_THREADS) k_sweep(const SweepParams p)
     const int tid = threadIdx.x;
     const int q = tid & 7;        // copy quad: copies 4q..4q+3 of the group
     const int slot = tid >> 3;    // site slot
-    const int tile = blockIdx.x, grp = blockIdx.y, sample = blockIdx.z;
+    // the copy group is the fastest block index: the CTAs that share a tile's couplings run together
+    const int grp = blockIdx.x % p.NG, tile = blockIdx.x / p.NG, sample = blockIdx.y;
     const int L = p.L;
 
     float* const sp = p.spins + ((size_t)(sample * p.NG + grp) * p.N) * SITE_FLOATS + q * 4;

@@ -1,0 +1,319 @@
+// sg_sweep_zm.cuh -- the z-marching half-sweep kernel (S1, S2, S3) of libsg_b200 for L a multiple of 8.
+//
+// Why.  A half-sweep is HBM-bound at 36 + 216/C bytes per update, but only if every
+// spin is fetched from L2 about once: the first kernel (k_sweep, sg_kernels.cuh) pulled 78 B per update
+// through the L2 -> SM crossbar, which saturates near 6300 B/clk on this chip, before HBM does.  Here a CTA
+// owns a TX x TY column of one copy group and marches along x3.  Per plane it needs the 32-copy lines of
+//   * the TX*TY/2 sites it updates (read once, by the updating thread, prefetched into registers), and
+//   * the other-colour sites of that plane, tile plus a one-site halo (TX*TY/2 + TX + TY lines),
+// and every other-colour plane serves three consecutive steps (as the x3+1 neighbours, the in-plane
+// neighbours, the x3-1 neighbours).  A producer warp streams those planes, and the per-site coupling
+// blocks, into a shared-memory ring with bulk asynchronous copies (cp.async.bulk -> UBLKCP) that complete
+// on mbarriers; the consumer warps read neighbours and couplings from shared memory only.
+// L2 -> SM traffic: 12 (own) + 12 (TX*TY/2+TX+TY)/(TX*TY/2) (other) + 7 (couplings) + 12 (write) = 49 B
+// per update for 8 x 8 columns.
+#pragma once
+#include "sg_device.cuh"
+
+namespace sg {
+
+enum : int { KIND_OR = 0, KIND_HB = 1, KIND_ENERGY = 2 };
+
+// ---- mbarrier / bulk-copy primitives (PTX; sm_90+) ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) {}
+}
+// global -> shared bulk copy of `bytes` (multiple of 16, 16-byte aligned both sides), completing on `bar`
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ float4 lds4(const unsigned char* p) { return *reinterpret_cast<const float4*>(p); }
+
+// Geometry of one ring stage: the other-colour sites of a plane, tile + halo.
+//   interior row yy (0..TY-1): ROW = TX/2+1 slots, slot = yy*ROW + ((xx+1)>>1), xx in [-1, TX]
+//   halo rows yy = -1, TY     : TX/2 slots each, slot = TY*ROW + (yy<0 ? 0 : TX/2) + (xx>>1)
+template <int TX, int TY>
+struct ZmGeom {
+    static constexpr int ROW = TX / 2 + 1;
+    static constexpr int SLOTS = TY * ROW + TX;
+    static constexpr int OWN = TX * TY / 2;
+    static constexpr int SITE_BYTES = SITE_FLOATS * 4;            // 384
+    static constexpr int STAGE_BYTES = SLOTS * SITE_BYTES;        // 18432 for 8 x 8
+    static constexpr int JSITE_BYTES = JG * 4;                    // 224
+    static constexpr int JSTAGE_BYTES = OWN * JSITE_BYTES;        // 7168 for 8 x 8
+    static constexpr int CONSUMERS = OWN * 8;                     // threads: (site, copy quad)
+    static constexpr int THREADS = CONSUMERS + 32;                // + one producer warp
+    static constexpr int NWARPS_C = CONSUMERS / 32;
+};
+
+template <int TX, int TY, int NST, int NJ>
+constexpr size_t zm_smem_bytes()
+{
+    return (size_t)NST * ZmGeom<TX, TY>::STAGE_BYTES + (size_t)NJ * ZmGeom<TX, TY>::JSTAGE_BYTES + 8 * (2 * NST + 2 * NJ) + 128;
+}
+
+struct ZmParams {
+    float* spins;            // [S][NG][N][3][G]
+    const float* Jg;         // [S][2][Nh][JG]
+    const float* beta_slot;  // [S][Cp]
+    double* Epart;           // [S][NG][nblk][G]
+    int L, N, Nh, NG, C;
+    int ntx, nty, nzc, ZC;   // tiles along x1, x2; chunks along x3 of ZC planes each
+    int colour;
+    uint32_t key0, key1, hb_counter, g_first;
+};
+
+// the single-site update of 4 copies held by one thread (shared by the update kinds)
+template <int KIND, bool WITH_E>
+__device__ __forceinline__ void zm_update(const float (&hf)[3][4], float (&s)[3][4], float (&eacc)[4], const float4& beta4,
+                                          uint32_t i, uint32_t g0, const ZmParams& p)
+{
+    if (KIND == KIND_OR) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
+            or_update(hf[0][j], hf[1][j], hf[2][j], s[0][j], s[1][j], s[2][j]);
+        }
+    } else if (KIND == KIND_HB) {
+        const float bt[4] = { beta4.x, beta4.y, beta4.z, beta4.w };
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            uint32_t w[4];
+            philox4x32_10(i, g0 + j, p.hb_counter, STREAM_HB, p.key0, p.key1, w);
+            hb_update(hf[0][j], hf[1][j], hf[2][j], bt[j], uniform23(w[0]), uniform23(w[1]), s[0][j], s[1][j], s[2][j]);
+            if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
+    }
+}
+
+template <int KIND, bool WITH_E, int TX, int TY, int NST, int NJ>
+__global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS) k_sweep_zm(const ZmParams p)
+{
+    using Gm = ZmGeom<TX, TY>;
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned char* const ring = smem;                                       // NST stages of other-colour planes
+    unsigned char* const jring = smem + (size_t)NST * Gm::STAGE_BYTES;      // NJ stages of coupling blocks
+    const uint32_t bars = smem_u32(jring + (size_t)NJ * Gm::JSTAGE_BYTES);  // full_o[NST] empty_o[NST] full_j[NJ] empty_j[NJ]
+    auto full_o = [&](int s) { return bars + 8u * s; };
+    auto empty_o = [&](int s) { return bars + 8u * (NST + s); };
+    auto full_j = [&](int s) { return bars + 8u * (2 * NST + s); };
+    auto empty_j = [&](int s) { return bars + 8u * (2 * NST + NJ + s); };
+
+    const int tid = threadIdx.x;
+    // block -> (tile, chunk, group): the group is fastest so that the CTAs that share a tile's couplings
+    // run next to each other in time (one DRAM read of the couplings per tile, not per group)
+    int b = blockIdx.x;
+    const int grp = b % p.NG; b /= p.NG;
+    const int zc = b % p.nzc; b /= p.nzc;
+    const int X0 = (b % p.ntx) * TX, Y0 = (b / p.ntx) * TY;
+    const int sample = blockIdx.y;
+    const int L = p.L, z0 = zc * p.ZC, ZC = p.ZC;
+
+    if (tid == 0) {
+        for (int s = 0; s < NST; ++s) { mbar_init(full_o(s), 1); mbar_init(empty_o(s), Gm::NWARPS_C); }
+        for (int s = 0; s < NJ; ++s) { mbar_init(full_j(s), 1); mbar_init(empty_j(s), Gm::NWARPS_C); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    const float* const spins_grp = p.spins + ((size_t)(sample * p.NG + grp) * p.N) * SITE_FLOATS;
+    const float* const Jc = p.Jg + ((size_t)(sample * 2 + p.colour) * p.Nh) * JG;
+
+    if (tid >= Gm::CONSUMERS) {
+        // ---------------- producer warp ----------------
+        const int lane = tid - Gm::CONSUMERS;
+        for (int n = 0; n < ZC + 2; ++n) {
+            // other-colour plane n of the chunk: x3 = z0 - 1 + n (periodic)
+            {
+                const int st = n % NST;
+                if (n >= NST) mbar_wait(empty_o(st), ((n / NST) - 1) & 1);
+                if (lane == 0) mbar_expect_tx(full_o(st), Gm::STAGE_BYTES);
+                __syncwarp();
+                int z = z0 - 1 + n;
+                z = (z < 0) ? z + L : ((z >= L) ? z - L : z);
+                const uint32_t dst0 = smem_u32(ring + (size_t)st * Gm::STAGE_BYTES);
+                for (int c = lane; c < Gm::SLOTS; c += 32) {
+                    int xx, yy;
+                    if (c < TY * Gm::ROW) {
+                        yy = c / Gm::ROW;
+                        const int j = c - yy * Gm::ROW;
+                        xx = 2 * j - 1 + ((yy + z + p.colour) & 1);
+                    } else {
+                        const int h = c - TY * Gm::ROW;
+                        yy = (h < TX / 2) ? -1 : TY;
+                        const int j = (h < TX / 2) ? h : h - TX / 2;
+                        xx = 2 * j + ((yy + z + p.colour + 1) & 1);
+                    }
+                    int x = X0 + xx, y = Y0 + yy;
+                    x = (x < 0) ? x + L : ((x >= L) ? x - L : x);
+                    y = (y < 0) ? y + L : ((y >= L) ? y - L : y);
+                    const size_t i = (size_t)x + (size_t)L * (y + (size_t)L * z);
+                    bulk_g2s(dst0 + c * Gm::SITE_BYTES, spins_grp + i * SITE_FLOATS, Gm::SITE_BYTES, full_o(st));
+                }
+            }
+            // coupling blocks of step k = n - 2: one bulk copy per tile row (TX/2 consecutive sites of the colour)
+            const int k = n - 2;
+            if (k >= 0) {
+                const int st = k % NJ;
+                if (k >= NJ) mbar_wait(empty_j(st), ((k / NJ) - 1) & 1);
+                if (lane == 0) mbar_expect_tx(full_j(st), Gm::JSTAGE_BYTES);
+                __syncwarp();
+                const int z = z0 + k;
+                const uint32_t dst0 = smem_u32(jring + (size_t)st * Gm::JSTAGE_BYTES);
+                for (int r = lane; r < TY; r += 32) {
+                    const size_t h0 = ((size_t)X0 + (size_t)L * (Y0 + r + (size_t)L * z)) >> 1;
+                    bulk_g2s(dst0 + r * (TX / 2) * Gm::JSITE_BYTES, Jc + h0 * JG, (TX / 2) * Gm::JSITE_BYTES, full_j(st));
+                }
+            }
+        }
+        return;
+    }
+
+    // ---------------- consumer warps: thread = (own-colour site of the plane, copy quad) ----------------
+    const int q = tid & 7, ks = tid >> 3;
+    const int ky = ks / (TX / 2), kx = ks - ky * (TX / 2);
+    const int Y = Y0 + ky;
+    float4 beta4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (KIND == KIND_HB) beta4 = ldg4(p.beta_slot + (size_t)sample * p.NG * G + grp * G + q * 4);
+    const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.C + (uint32_t)(grp * G + q * 4);
+    float eacc[4] = { 0.f, 0.f, 0.f, 0.f };
+
+    // own spin of step k: site (X0 + 2 kx + ((ky + z + colour) & 1), Y, z)
+    auto own_ptr = [&](int k) -> float* {
+        const int z = z0 + k;
+        const int x = X0 + 2 * kx + ((ky + z + p.colour) & 1);
+        return const_cast<float*>(spins_grp) + ((size_t)x + (size_t)L * (Y + (size_t)L * z)) * SITE_FLOATS + q * 4;
+    };
+    float4 pre[2][3];   // register prefetch of the own spins, two steps deep
+#pragma unroll
+    for (int d = 0; d < 2; ++d)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) pre[d][a] = (d < ZC) ? ld4(own_ptr(d) + a * G) : make_float4(0.f, 0.f, 0.f, 0.f);
+
+    mbar_wait(full_o(0 % NST), 0);
+    mbar_wait(full_o(1 % NST), 0);
+
+    for (int k2 = 0; k2 < ZC; k2 += 2) {
+#pragma unroll
+        for (int d = 0; d < 2; ++d) {
+            const int k = k2 + d;
+            if (k >= ZC) break;
+            const int z = z0 + k;
+            const int off = (ky + z + p.colour) & 1;
+            float* const own = own_ptr(k);
+            float s[3][4];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { s[a][0] = pre[d][a].x; s[a][1] = pre[d][a].y; s[a][2] = pre[d][a].z; s[a][3] = pre[d][a].w; }
+            if (k + 2 < ZC) {
+                const float* nx = own_ptr(k + 2);
+#pragma unroll
+                for (int a = 0; a < 3; ++a) pre[d][a] = ld4(nx + a * G);
+            }
+            // planes n = k (x3-1), k+1 (in-plane), k+2 (x3+1)
+            const int sm_ = k % NST, s0_ = (k + 1) % NST, sp_ = (k + 2) % NST;
+            mbar_wait(full_o(sp_), ((k + 2) / NST) & 1);
+            mbar_wait(full_j(k % NJ), (k / NJ) & 1);
+            const unsigned char* const Pm = ring + (size_t)sm_ * Gm::STAGE_BYTES + q * 16;
+            const unsigned char* const P0 = ring + (size_t)s0_ * Gm::STAGE_BYTES + q * 16;
+            const unsigned char* const Pp = ring + (size_t)sp_ * Gm::STAGE_BYTES + q * 16;
+            const int sl_z = ky * Gm::ROW + kx + off;
+            const int sl_xm = ky * Gm::ROW + kx;
+            const int sl_ym = (ky > 0) ? (ky - 1) * Gm::ROW + kx + off : TY * Gm::ROW + kx;
+            const int sl_yp = (ky < TY - 1) ? (ky + 1) * Gm::ROW + kx + off : TY * Gm::ROW + TX / 2 + kx;
+            const unsigned char* nbp[6] = { P0 + (sl_xm + 1) * Gm::SITE_BYTES, P0 + sl_xm * Gm::SITE_BYTES,
+                                            P0 + sl_yp * Gm::SITE_BYTES,       P0 + sl_ym * Gm::SITE_BYTES,
+                                            Pp + sl_z * Gm::SITE_BYTES,        Pm + sl_z * Gm::SITE_BYTES };
+            const unsigned char* const Jp = jring + (size_t)(k % NJ) * Gm::JSTAGE_BYTES + ks * Gm::JSITE_BYTES;
+
+            float hf[3][4];
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) hf[a][j] = 0.f;
+            float J[JG];
+#pragma unroll
+            for (int v = 0; v < JG / 4; ++v) {
+                const float4 t4 = lds4(Jp + 16 * v);
+                J[4 * v] = t4.x; J[4 * v + 1] = t4.y; J[4 * v + 2] = t4.z; J[4 * v + 3] = t4.w;
+            }
+#pragma unroll
+            for (int nbk = 0; nbk < 6; ++nbk) {
+                float n[3][4];
+#pragma unroll
+                for (int bb = 0; bb < 3; ++bb) {
+                    const float4 t4 = lds4(nbp[nbk] + bb * (G * 4));
+                    n[bb][0] = t4.x; n[bb][1] = t4.y; n[bb][2] = t4.z; n[bb][3] = t4.w;
+                }
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int bb = 0; bb < 3; ++bb)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * nbk + 3 * a + bb], n[bb][j], hf[a][j]);
+            }
+            // the stage of plane k and the coupling stage are dead for this warp once the loads above retire
+            __syncwarp();
+            if ((tid & 31) == 0) { mbar_arrive(empty_o(sm_)); mbar_arrive(empty_j(k % NJ)); }
+
+            const uint32_t i = (uint32_t)((own - q * 4 - spins_grp) / SITE_FLOATS);
+            zm_update<KIND, WITH_E>(hf, s, eacc, beta4, i, g0, p);
+            if (KIND != KIND_ENERGY) {
+#pragma unroll
+                for (int a = 0; a < 3; ++a) st4(own + a * G, make_float4(s[a][0], s[a][1], s[a][2], s[a][3]));
+            }
+        }
+    }
+
+    if (WITH_E || KIND == KIND_ENERGY) {
+        // per-copy sum over the CTA's sites: fixed order, fp64 across threads (no float atomics).
+        // The ring is dead by now for every consumer warp (all full barriers were waited, all reads retired
+        // before the named barrier below), so its first bytes serve as the reduction scratch.
+        asm volatile("bar.sync 1, %0;" ::"r"(Gm::CONSUMERS) : "memory");
+        double* red = reinterpret_cast<double*>(ring);   // [OWN][G+1]
+#pragma unroll
+        for (int j = 0; j < 4; ++j) red[ks * (G + 1) + q * 4 + j] = (double)eacc[j];
+        asm volatile("bar.sync 1, %0;" ::"r"(Gm::CONSUMERS) : "memory");
+        if (tid < G) {
+            double acc = 0.0;
+            for (int r = 0; r < Gm::OWN; ++r) acc += red[r * (G + 1) + tid];
+            const int nblk = p.ntx * p.nty * p.nzc;
+            const int blk = blockIdx.x / p.NG;
+            p.Epart[((size_t)(sample * p.NG + grp) * nblk + blk) * G + tid] = acc;
+        }
+    }
+}
+
+}  // namespace sg

@@ -33,6 +33,13 @@ SHAPES = [
     dict(L=10, S=1, R=3, T=11, b=(0.4, 2.4)),
     dict(L=8, S=3, R=4, T=16, b=(0.5, 2.0)),
     dict(L=16, S=1, R=2, T=20, b=(0.5, 2.2)),
+    # the same two shapes through the tiled kernel (L = 8, 16 go to the z-marching kernel by default), and the
+    # z-marching kernel with several chunks per column, one chunk of all planes, and 3 x 3 tiles (L = 24)
+    dict(L=8, S=3, R=4, T=16, b=(0.5, 2.0), tune=((0, 1),)),
+    dict(L=16, S=1, R=2, T=20, b=(0.5, 2.2), tune=((0, 1),)),
+    dict(L=16, S=2, R=2, T=17, b=(0.5, 2.2), tune=((0, 2), (1, 4))),
+    dict(L=16, S=1, R=1, T=33, b=(0.5, 2.2), tune=((0, 2), (1, 16))),
+    dict(L=24, S=1, R=2, T=5, b=(0.5, 2.2), tune=((0, 2), (1, 6))),
 ]
 
 
@@ -107,7 +114,7 @@ def test_set_get_spins_roundtrip(sg, sh):
 def test_half_sweeps_match_oracle(sg, oracle, sh, kind, gen_mode):
     """Each colour separately, each compared from the oracle's state (no error propagation)."""
     L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
-    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=5, gen_mode=gen_mode)
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=5, gen_mode=gen_mode, tune=sh.get("tune"))
     sim.hb_counter = 17
     gpu.set_counters(17, 0)
     col = colour_mask(L)
@@ -179,7 +186,7 @@ def test_full_sweep_matches_oracle(sg, oracle, sh, kind):
     """north_star: spins after one sweep within 1e-5 absolute per component; energy per spin within 1e-6."""
     L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
     N = L ** 3
-    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=6)
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=6, tune=sh.get("tune"))
     sweep_both(sim, gpu, kind, L)
     # fused energy of the sweep's last half-sweep against Eq. (1) on the oracle's spins
     e_gpu, e_ref = gpu.get_energies() / N, sim.energies() / N
@@ -191,7 +198,7 @@ def test_or_conserves_energy_and_norm_on_gpu(sg, oracle):
     sh = SHAPES[4]
     L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
     N = L ** 3
-    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=8)
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=8, tune=sh.get("tune"))
     e0 = gpu.get_energies() / N                   # standalone energy kernel
     assert np.all(np.abs(e0 - sim.energies() / N) <= 1e-6 * np.maximum(1.0, np.abs(e0)))
     gpu.sweep_or(8)
@@ -208,7 +215,7 @@ def test_or_conserves_energy_and_norm_on_gpu(sg, oracle):
 def test_time_reversal_and_involution_on_gpu(sg, oracle):
     sh = SHAPES[2]
     L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
-    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=9, gen_mode=2)
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=9, gen_mode=2, tune=sh.get("tune"))
     s0 = gpu_spins(gpu)
     gpu.halfsweep(0, 0)
     s1 = gpu_spins(gpu)
@@ -226,7 +233,7 @@ def test_time_reversal_and_involution_on_gpu(sg, oracle):
 @pytest.mark.parametrize("sh", SHAPES)
 def test_measure_matches_oracle(sg, oracle, sh):
     L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
-    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=10)
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=10, tune=sh.get("tune"))
     rng = np.random.default_rng(3)
     for s in range(S):                                    # a non-trivial temperature assignment
         tos = np.stack([rng.permutation(T) for _ in range(R)]).astype(np.int32)
@@ -283,7 +290,7 @@ def test_ferromagnet_energy_on_gpu(sg):
 @pytest.mark.parametrize("sh", [SHAPES[0], SHAPES[2], SHAPES[4]])
 def test_pt_decisions_identical_on_identical_energies(sg, oracle, sh):
     L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
-    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=11, first_sample=2)
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=11, first_sample=2, tune=sh.get("tune"))
     rng = np.random.default_rng(5)
     for k in range(40):
         # energies spaced so that acceptance is neither 0 nor 1
@@ -304,7 +311,7 @@ def test_pt_moves_temperatures_not_spins_and_hb_follows(sg, oracle):
     """After PT the heat bath must use each slot's *new* temperature (beta by slot follows the swap)."""
     sh = SHAPES[0]
     L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
-    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=12)
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=12, tune=sh.get("tune"))
     before = gpu_spins(gpu)
     E = np.array([[0.0, -50.0, -20.0, -90.0, 5.0, 1.0, -3.0, 2.0]])     # forces some swaps
     gpu.set_energies(E); gpu.pt_swap(); sim.pt_swap(energies=E)

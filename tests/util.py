@@ -12,11 +12,13 @@ def neighbour_dilate(mask, L):
 
 
 def make_pair(oracle, sgmod, L, S, R, T, betas, seed=1, gen_mode=0, sigma_D=1.0, first_sample=0,
-              couplings=None, spins=None):
+              couplings=None, spins=None, tune=None):
     """Oracle chain and CUDA context with identical inputs.  Inputs flow oracle -> CUDA, never back:
     couplings / spins are drawn by the oracle's generators (or passed in) and copied to the device."""
     sim = oracle.OracleSim(L, S, R, T, betas, seed, store_fp32=True, first_sample=first_sample)
     gpu = sgmod.SpinGlass(L, S, R, T, betas, seed=seed, first_sample=first_sample)
+    for knob, value in (tune or ()):           # (sg_tune knob, value) pairs: which sweep kernel serves the calls
+        gpu.tune(knob, value)
     for s in range(S):
         sim.init_sample(s, gen_mode, sigma_D,
                         couplings=None if couplings is None else couplings[s],
