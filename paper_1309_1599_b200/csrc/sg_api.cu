@@ -18,7 +18,7 @@ struct sg_ctx {
     int L, N, Nh, S, R, T, C, NG, Cp, P;
     cudaStream_t stream;
     // device arrays (carved from the caller's workspace)
-    float* spins; float* Jg; float* Mraw; float* staging; float* beta_slot;
+    float* spins; float* Jg; float* Jt; float* Mraw; float* staging; float* beta_slot;
     double* betas; double* E; double* Epart; double* phase; double* Mpart; double* result;
     int* slot_of_temp; int* temp_of_slot;
     unsigned long long* attempts; unsigned long long* accepts;
@@ -82,7 +82,7 @@ struct Carve {
 };
 
 struct Offsets {
-    size_t spins, Jg, Mraw, staging, beta_slot, betas, E, Epart, phase, Mpart, result, sot, tos, att, acc, total;
+    size_t spins, Jg, Jt, Mraw, staging, beta_slot, betas, E, Epart, phase, Mpart, result, sot, tos, att, acc, total;
 };
 
 Offsets offsets(const Geometry& g)
@@ -90,6 +90,7 @@ Offsets offsets(const Geometry& g)
     Carve c; Offsets o;
     o.spins = c.take((size_t)g.S * g.NG * g.N * SITE_FLOATS * sizeof(float));
     o.Jg = c.take((size_t)g.S * 2 * g.Nh * JG * sizeof(float));
+    o.Jt = c.take((g.L % 8 == 0) ? (size_t)g.S * 2 * g.Nh * JG * sizeof(float) : 0);
     o.Mraw = c.take((size_t)g.S * 3 * g.N * 9 * sizeof(float));
     size_t stg = (size_t)G * 3 * g.N * sizeof(float);
     o.staging = c.take(stg);
@@ -245,7 +246,7 @@ int launch_zm(sg_ctx* ctx, const ZmParams& p, dim3 grid)
 int half_sweep_zm(sg_ctx* ctx, int kind, int colour, bool with_energy)
 {
     ZmParams p;
-    p.spins = ctx->spins; p.Jg = ctx->Jg; p.beta_slot = ctx->beta_slot; p.Epart = ctx->Epart;
+    p.spins = ctx->spins; p.Jt = ctx->Jt; p.beta_slot = ctx->beta_slot; p.Epart = ctx->Epart;
     p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.C = ctx->C;
     p.ntx = ctx->L / ZM_TX; p.nty = ctx->L / ZM_TY; p.nzc = ctx->zm_nzc; p.ZC = ctx->zm_ZC;
     p.colour = colour;
@@ -373,7 +374,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->nchunk = g.nchunk; ctx->chunk_sites = g.chunk_sites; ctx->MS = g.MS;
     ctx->stream = (cudaStream_t)cuda_stream;
     char* base = (char*)dev_workspace;
-    ctx->spins = (float*)(base + o.spins); ctx->Jg = (float*)(base + o.Jg); ctx->Mraw = (float*)(base + o.Mraw);
+    ctx->spins = (float*)(base + o.spins); ctx->Jg = (float*)(base + o.Jg); ctx->Jt = (g.L % 8 == 0) ? (float*)(base + o.Jt) : nullptr; ctx->Mraw = (float*)(base + o.Mraw);
     ctx->staging = (float*)(base + o.staging); ctx->beta_slot = (float*)(base + o.beta_slot);
     ctx->betas = (double*)(base + o.betas); ctx->E = (double*)(base + o.E); ctx->Epart = (double*)(base + o.Epart);
     ctx->phase = (double*)(base + o.phase); ctx->Mpart = (double*)(base + o.Mpart);
@@ -430,7 +431,7 @@ int sg_set_spins(sg_ctx* ctx, int sample, const float* in)
         SG_CUDA(ctx, cudaMemcpyAsync(ctx->staging, in + (size_t)c0 * copy_floats, (size_t)nc * copy_floats * sizeof(float),
                                      cudaMemcpyHostToDevice, ctx->stream));
         float* dev = ctx->spins + ((size_t)(sample * ctx->NG + grp) * ctx->N) * SITE_FLOATS;
-        k_spins_from_staging<<<dim3((ctx->N + 31) / 32, 3), dim3(32, 8), 0, ctx->stream>>>(ctx->staging, dev, ctx->N);
+        k_spins_from_staging<<<dim3((ctx->N + 31) / 32, 3), dim3(32, 8), 0, ctx->stream>>>(ctx->staging, dev, ctx->N, ctx->L);
         SG_LAUNCHED(ctx);
     }
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -446,7 +447,7 @@ int sg_get_spins(sg_ctx* ctx, int sample, float* out)
     for (int grp = 0; grp < ctx->NG; ++grp) {
         const int c0 = grp * G, nc = (ctx->C - c0 < G) ? ctx->C - c0 : G;
         const float* dev = ctx->spins + ((size_t)(sample * ctx->NG + grp) * ctx->N) * SITE_FLOATS;
-        k_spins_to_staging<<<dim3((ctx->N + 31) / 32, 3), dim3(32, 8), 0, ctx->stream>>>(dev, ctx->staging, ctx->N);
+        k_spins_to_staging<<<dim3((ctx->N + 31) / 32, 3), dim3(32, 8), 0, ctx->stream>>>(dev, ctx->staging, ctx->N, ctx->L);
         SG_LAUNCHED(ctx);
         SG_CUDA(ctx, cudaMemcpyAsync(out + (size_t)c0 * copy_floats, ctx->staging, (size_t)nc * copy_floats * sizeof(float),
                                      cudaMemcpyDeviceToHost, ctx->stream));
@@ -470,7 +471,8 @@ int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const 
     }
     SG_CUDA(ctx, cudaMemcpyAsync(Mdev, src, mfloats * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    k_gather_couplings<<<(ctx->N + 127) / 128, 128, 0, ctx->stream>>>(Mdev, ctx->Jg + (size_t)sample * 2 * ctx->Nh * JG, ctx->L);
+    k_gather_couplings<<<(ctx->N + 127) / 128, 128, 0, ctx->stream>>>(Mdev, ctx->Jg + (size_t)sample * 2 * ctx->Nh * JG,
+                                                                           ctx->Jt ? ctx->Jt + (size_t)sample * 2 * ctx->Nh * JG : nullptr, ctx->L);
     SG_LAUNCHED(ctx);
 
     if (spins) {
@@ -479,7 +481,7 @@ int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const 
         const size_t nthr = (size_t)ctx->NG * ctx->N * 8;
         const uint32_t g_sample = (uint32_t)(ctx->shape.first_sample + sample) * (uint32_t)ctx->C;
         k_init_spins<<<(unsigned)((nthr + 255) / 256), 256, 0, ctx->stream>>>(
-            ctx->spins + (size_t)sample * ctx->NG * ctx->N * SITE_FLOATS, ctx->N, ctx->NG, ctx->C, g_sample,
+            ctx->spins + (size_t)sample * ctx->NG * ctx->N * SITE_FLOATS, ctx->L, ctx->N, ctx->NG, ctx->C, g_sample,
             (uint32_t)(ctx->shape.seed & 0xffffffffu), (uint32_t)(ctx->shape.seed >> 32));
         SG_LAUNCHED(ctx);
     }

@@ -9,11 +9,17 @@ namespace sg {
 
 // ------------------------------------------------------------------------------------------------
 // HBM layout (private)
-//   spins  float [S][NG][N][3][G]   G = 32 consecutive copy ids: one aligned 128-byte line per
-//                                   (site, component, group); a site of a group is 384 contiguous bytes
+//   spins  float [S][NG][2][N/2][3][G]  G = 32 consecutive copy ids: one aligned 128-byte line per
+//                                   (site, component, group); a site of a group is 384 contiguous bytes.
+//                                   Sites are split by colour, then ordered by h = i>>1, so that the
+//                                   same-colour sites of a lattice row (x2, x3) are L/2 contiguous
+//                                   384-byte blocks: one bulk copy fetches a whole row segment.
 //   Jg     float [S][2][N/2][JG]    per-site gathered couplings, by colour then h = i>>1:
 //                                   A_k, k = (+x,-x,+y,-y,+z,-z), with h_x = sum_k A_k s_{nbr k}
 //                                   (forward: M_{x,mu}; backward: M_{x-e_mu,mu}^T), 54 floats + 2 pad
+//   Jt     float [S][2][L/8][L/8][L][8][4][JG]  (L a multiple of 8 only) the same blocks ordered by
+//                                   8 x 8 column tile, plane, row, site: the couplings one CTA of the
+//                                   z-marching sweep needs for one plane are 7168 contiguous bytes
 // ------------------------------------------------------------------------------------------------
 constexpr int G = 32;
 constexpr int SITE_FLOATS = 3 * G;
@@ -115,6 +121,13 @@ __device__ __forceinline__ void site_of(int h, int colour, int L, int& x, int& y
         z = r / L;
         x = 2 * xh + ((y + z + colour) & 1);
     }
+}
+
+// position of site i in the colour-split site order of the spin array (units of one site = SITE_FLOATS floats)
+__device__ __forceinline__ size_t site_slot(int i, int L, int Nh)
+{
+    const int x = i % L, y = (i / L) % L, z = i / (L * L);
+    return (size_t)((x + y + z) & 1) * Nh + (size_t)(i >> 1);
 }
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }

@@ -19,7 +19,7 @@ constexpr int SWEEP_THREADS = 256;
 constexpr int SLOTS = SWEEP_THREADS / 8;   // site slots per pass
 
 struct SweepParams {
-    float* spins;            // [S][NG][N][3][G]
+    float* spins;            // [S][NG][2][Nh][3][G]
     const float* Jg;         // [S][2][Nh][JG]
     const float* beta_slot;  // [S][Cp]
     double* Epart;           // [S][NG][ntiles][G]
@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS) k_sweep(const SweepParams p)
                 J[4 * v] = t4.x; J[4 * v + 1] = t4.y; J[4 * v + 2] = t4.z; J[4 * v + 3] = t4.w;
             }
         }
-        float* const own = sp + (size_t)i * SITE_FLOATS;
+        float* const own = sp + ((size_t)p.colour * p.Nh + h) * SITE_FLOATS;
         float s[3][4];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS) k_sweep(const SweepParams p)
             for (int j = 0; j < 4; ++j) hf[a][j] = 0.f;
 #pragma unroll
         for (int k = 0; k < 6; ++k) {
-            const float* np_ = sp + (size_t)nb[k] * SITE_FLOATS;
+            const float* np_ = sp + ((size_t)(1 - p.colour) * p.Nh + (nb[k] >> 1)) * SITE_FLOATS;
             float n[3][4];
 #pragma unroll
             for (int b = 0; b < 3; ++b) {
@@ -166,7 +166,7 @@ __global__ void k_reduce_energy(const double* __restrict__ Epart, double* __rest
 // ------------------------------------------------------------------------------------------------
 // S0: initial spins uniform on S^2, Philox stream 3, counter (i, g, 0, 3)
 // ------------------------------------------------------------------------------------------------
-__global__ void k_init_spins(float* __restrict__ spins_sample /* [NG][N][3][G] of one sample */, int N, int NG,
+__global__ void k_init_spins(float* __restrict__ spins_sample /* [NG][2][Nh][3][G] of one sample */, int L, int N, int NG,
                              int C, uint32_t g_sample, uint32_t key0, uint32_t key1)
 {
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;   // over NG*N*8 (site, quad)
@@ -189,14 +189,14 @@ __global__ void k_init_spins(float* __restrict__ spins_sample /* [NG][N][3][G] o
         out[1][j] = live ? rho * sn : 0.f;
         out[2][j] = live ? zc : 0.f;
     }
-    float* dst = spins_sample + ((size_t)grp * N + i) * SITE_FLOATS + q * 4;
+    float* dst = spins_sample + ((size_t)grp * N + site_slot(i, L, N >> 1)) * SITE_FLOATS + q * 4;
 #pragma unroll
     for (int a = 0; a < 3; ++a) st4(dst + a * G, make_float4(out[a][0], out[a][1], out[a][2], out[a][3]));
 }
 
-// host layout [c][3][N] (32 copies of one group, staged on the device) <-> device layout [N][3][G]
+// host layout [c][3][N] (32 copies of one group, staged on the device) <-> device layout [2][Nh][3][G]
 // block (32, 8); tile = 32 sites x 32 copies per component
-__global__ void k_spins_from_staging(const float* __restrict__ stg, float* __restrict__ dev, int N)
+__global__ void k_spins_from_staging(const float* __restrict__ stg, float* __restrict__ dev, int N, int L)
 {
     __shared__ float tile[32][33];
     const int comp = blockIdx.y;
@@ -208,18 +208,18 @@ __global__ void k_spins_from_staging(const float* __restrict__ stg, float* __res
     __syncthreads();
     for (int r = threadIdx.y; r < 32; r += 8) {
         const int i = i0 + r;
-        if (i < N) dev[(size_t)i * SITE_FLOATS + comp * G + threadIdx.x] = tile[threadIdx.x][r];
+        if (i < N) dev[site_slot(i, L, N >> 1) * SITE_FLOATS + comp * G + threadIdx.x] = tile[threadIdx.x][r];
     }
 }
 
-__global__ void k_spins_to_staging(const float* __restrict__ dev, float* __restrict__ stg, int N)
+__global__ void k_spins_to_staging(const float* __restrict__ dev, float* __restrict__ stg, int N, int L)
 {
     __shared__ float tile[32][33];
     const int comp = blockIdx.y;
     const int i0 = blockIdx.x * 32;
     for (int r = threadIdx.y; r < 32; r += 8) {
         const int i = i0 + r;
-        tile[r][threadIdx.x] = (i < N) ? dev[(size_t)i * SITE_FLOATS + comp * G + threadIdx.x] : 0.f;
+        tile[r][threadIdx.x] = (i < N) ? dev[site_slot(i, L, N >> 1) * SITE_FLOATS + comp * G + threadIdx.x] : 0.f;
     }
     __syncthreads();
     for (int c = threadIdx.y; c < 32; c += 8) {
@@ -229,7 +229,8 @@ __global__ void k_spins_to_staging(const float* __restrict__ dev, float* __restr
 }
 
 // raw couplings M[3][N][9] of one sample -> gathered per-site blocks Jg[2][Nh][JG]
-__global__ void k_gather_couplings(const float* __restrict__ M, float* __restrict__ Jg_sample, int L)
+// (and, when Jt_sample != nullptr, the tile-major copy Jt[2][L/8][L/8][L][8][4][JG] of the z-marching sweep)
+__global__ void k_gather_couplings(const float* __restrict__ M, float* __restrict__ Jg_sample, float* __restrict__ Jt_sample, int L)
 {
     const int N = L * L * L, Nh = N >> 1;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -249,6 +250,12 @@ __global__ void k_gather_couplings(const float* __restrict__ M, float* __restric
             }
     }
     dst[54] = 0.f; dst[55] = 0.f;
+    if (Jt_sample) {
+        const int nt = L >> 3;
+        const size_t t = ((((size_t)colour * nt + (y >> 3)) * nt + (x >> 3)) * L + z) * 32 + (y & 7) * 4 + ((x & 7) >> 1);
+        float* d2 = Jt_sample + t * JG;
+        for (int e = 0; e < JG; ++e) d2[e] = dst[e];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -310,7 +317,7 @@ __global__ void k_fill_beta_slot(const double* __restrict__ betas, const int* __
 // through the temperature permutation.  Partial sums per site chunk, reduced in fixed order.
 // ------------------------------------------------------------------------------------------------
 struct MeasureParams {
-    const float* spins;        // [S][NG][N][3][G]
+    const float* spins;        // [S][NG][2][Nh][3][G]
     const int* slot_of_temp;   // [S][R][T]
     const double* phase;       // [L][2] cos, sin of 2 pi x / L
     double* Mpart;             // [S][nchunk][PT][7]
@@ -343,7 +350,7 @@ __global__ void k_measure(const MeasureParams p)
         for (int e = threadIdx.x; e < ms * p.NG * SITE_FLOATS; e += blockDim.x) {
             const int lane = e % G, comp = (e / G) % 3, grp = (e / SITE_FLOATS) % p.NG, m = e / (SITE_FLOATS * p.NG);
             sm[m * row + comp * p.Cp + grp * G + lane] =
-                base[((size_t)grp * p.N + (i0 + m)) * SITE_FLOATS + comp * G + lane];
+                base[((size_t)grp * p.N + site_slot(i0 + m, p.L, p.N >> 1)) * SITE_FLOATS + comp * G + lane];
         }
         __syncthreads();
         if (live) {

@@ -82,8 +82,8 @@ constexpr size_t zm_smem_bytes()
 }
 
 struct ZmParams {
-    float* spins;            // [S][NG][N][3][G]
-    const float* Jg;         // [S][2][Nh][JG]
+    float* spins;            // [S][NG][2][Nh][3][G]
+    const float* Jt;         // [S][2][L/TY][L/TX][L][TY][TX/2][JG]
     const float* beta_slot;  // [S][Cp]
     double* Epart;           // [S][NG][nblk][G]
     int L, N, Nh, NG, C;
@@ -150,11 +150,16 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS) k_sweep_zm(const ZmPa
     __syncthreads();
 
     const float* const spins_grp = p.spins + ((size_t)(sample * p.NG + grp) * p.N) * SITE_FLOATS;
-    const float* const Jc = p.Jg + ((size_t)(sample * 2 + p.colour) * p.Nh) * JG;
+    const int Lh = L >> 1;
 
     if (tid >= Gm::CONSUMERS) {
         // ---------------- producer warp ----------------
+        // Other-colour sites of a lattice row are contiguous in HBM (colour-split site order), so a plane is
+        // TY row segments of ROW sites (split in two where the x1 halo wraps), two halo rows of TX/2 sites,
+        // and the couplings of a plane are one block of the tile-major array: 11 to 19 bulk copies per step.
         const int lane = tid - Gm::CONSUMERS;
+        const float* const other = spins_grp + (size_t)(1 - p.colour) * p.Nh * SITE_FLOATS;
+        const float* const Jtile = p.Jt + ((((size_t)(sample * 2 + p.colour) * p.nty + Y0 / TY) * p.ntx + X0 / TX) * L) * (size_t)(Gm::OWN * JG);
         for (int n = 0; n < ZC + 2; ++n) {
             // other-colour plane n of the chunk: x3 = z0 - 1 + n (periodic)
             {
@@ -165,38 +170,48 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS) k_sweep_zm(const ZmPa
                 int z = z0 - 1 + n;
                 z = (z < 0) ? z + L : ((z >= L) ? z - L : z);
                 const uint32_t dst0 = smem_u32(ring + (size_t)st * Gm::STAGE_BYTES);
-                for (int c = lane; c < Gm::SLOTS; c += 32) {
-                    int xx, yy;
-                    if (c < TY * Gm::ROW) {
-                        yy = c / Gm::ROW;
-                        const int j = c - yy * Gm::ROW;
-                        xx = 2 * j - 1 + ((yy + z + p.colour) & 1);
+                if (lane < TY) {
+                    const int yy = lane;
+                    const int e = (yy + z + p.colour) & 1;          // first other-colour x1 of the row: X0 - 1 + e
+                    const size_t rowh = (size_t)Lh * (Y0 + yy + (size_t)L * z);
+                    const uint32_t dst = dst0 + yy * Gm::ROW * Gm::SITE_BYTES;
+                    if (e == 0) {
+                        // sites X0-1, X0+1, .., X0+TX-1: the first one wraps for the leftmost tile
+                        if (X0 == 0) {
+                            bulk_g2s(dst, other + (rowh + (Lh - 1)) * SITE_FLOATS, Gm::SITE_BYTES, full_o(st));
+                            bulk_g2s(dst + Gm::SITE_BYTES, other + (rowh + 0) * SITE_FLOATS, (Gm::ROW - 1) * Gm::SITE_BYTES, full_o(st));
+                        } else {
+                            bulk_g2s(dst, other + (rowh + ((X0 - 1) >> 1)) * SITE_FLOATS, Gm::ROW * Gm::SITE_BYTES, full_o(st));
+                        }
                     } else {
-                        const int h = c - TY * Gm::ROW;
-                        yy = (h < TX / 2) ? -1 : TY;
-                        const int j = (h < TX / 2) ? h : h - TX / 2;
-                        xx = 2 * j + ((yy + z + p.colour + 1) & 1);
+                        // sites X0, X0+2, .., X0+TX: the last one wraps for the rightmost tile
+                        if (X0 + TX == L) {
+                            bulk_g2s(dst, other + (rowh + (X0 >> 1)) * SITE_FLOATS, (Gm::ROW - 1) * Gm::SITE_BYTES, full_o(st));
+                            bulk_g2s(dst + (Gm::ROW - 1) * Gm::SITE_BYTES, other + rowh * SITE_FLOATS, Gm::SITE_BYTES, full_o(st));
+                        } else {
+                            bulk_g2s(dst, other + (rowh + (X0 >> 1)) * SITE_FLOATS, Gm::ROW * Gm::SITE_BYTES, full_o(st));
+                        }
                     }
-                    int x = X0 + xx, y = Y0 + yy;
-                    x = (x < 0) ? x + L : ((x >= L) ? x - L : x);
+                } else if (lane < TY + 2) {
+                    // halo rows x2 = Y0-1 and Y0+TY (periodic): TX/2 sites X0 + e, X0 + e + 2, ..
+                    const int up = lane - TY;
+                    int y = up ? Y0 + TY : Y0 - 1;
                     y = (y < 0) ? y + L : ((y >= L) ? y - L : y);
-                    const size_t i = (size_t)x + (size_t)L * (y + (size_t)L * z);
-                    bulk_g2s(dst0 + c * Gm::SITE_BYTES, spins_grp + i * SITE_FLOATS, Gm::SITE_BYTES, full_o(st));
+                    const size_t rowh = (size_t)Lh * (y + (size_t)L * z);
+                    bulk_g2s(dst0 + (TY * Gm::ROW + up * (TX / 2)) * Gm::SITE_BYTES, other + (rowh + (X0 >> 1)) * SITE_FLOATS,
+                             (TX / 2) * Gm::SITE_BYTES, full_o(st));
                 }
             }
-            // coupling blocks of step k = n - 2: one bulk copy per tile row (TX/2 consecutive sites of the colour)
+            // coupling blocks of step k = n - 2: one contiguous block of the tile-major array
             const int k = n - 2;
             if (k >= 0) {
                 const int st = k % NJ;
                 if (k >= NJ) mbar_wait(empty_j(st), ((k / NJ) - 1) & 1);
-                if (lane == 0) mbar_expect_tx(full_j(st), Gm::JSTAGE_BYTES);
-                __syncwarp();
-                const int z = z0 + k;
-                const uint32_t dst0 = smem_u32(jring + (size_t)st * Gm::JSTAGE_BYTES);
-                for (int r = lane; r < TY; r += 32) {
-                    const size_t h0 = ((size_t)X0 + (size_t)L * (Y0 + r + (size_t)L * z)) >> 1;
-                    bulk_g2s(dst0 + r * (TX / 2) * Gm::JSITE_BYTES, Jc + h0 * JG, (TX / 2) * Gm::JSITE_BYTES, full_j(st));
+                if (lane == 0) {
+                    mbar_expect_tx(full_j(st), Gm::JSTAGE_BYTES);
+                    bulk_g2s(smem_u32(jring + (size_t)st * Gm::JSTAGE_BYTES), Jtile + (size_t)(z0 + k) * (Gm::OWN * JG), Gm::JSTAGE_BYTES, full_j(st));
                 }
+                __syncwarp();
             }
         }
         return;
@@ -215,7 +230,7 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS) k_sweep_zm(const ZmPa
     auto own_ptr = [&](int k) -> float* {
         const int z = z0 + k;
         const int x = X0 + 2 * kx + ((ky + z + p.colour) & 1);
-        return const_cast<float*>(spins_grp) + ((size_t)x + (size_t)L * (Y + (size_t)L * z)) * SITE_FLOATS + q * 4;
+        return const_cast<float*>(spins_grp) + ((size_t)p.colour * p.Nh + (((size_t)x + (size_t)L * (Y + (size_t)L * z)) >> 1)) * SITE_FLOATS + q * 4;
     };
     float4 pre[2][3];   // register prefetch of the own spins, two steps deep
 #pragma unroll
@@ -288,7 +303,7 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS) k_sweep_zm(const ZmPa
             __syncwarp();
             if ((tid & 31) == 0) { mbar_arrive(empty_o(sm_)); mbar_arrive(empty_j(k % NJ)); }
 
-            const uint32_t i = (uint32_t)((own - q * 4 - spins_grp) / SITE_FLOATS);
+            const uint32_t i = (uint32_t)(X0 + 2 * kx + off + L * (Y + L * z));
             zm_update<KIND, WITH_E>(hf, s, eacc, beta4, i, g0, p);
             if (KIND != KIND_ENERGY) {
 #pragma unroll

@@ -38,7 +38,7 @@ SHAPES = [
     dict(L=8, S=3, R=4, T=16, b=(0.5, 2.0), tune=((0, 1),)),
     dict(L=16, S=1, R=2, T=20, b=(0.5, 2.2), tune=((0, 1),)),
     dict(L=16, S=2, R=2, T=17, b=(0.5, 2.2), tune=((0, 2), (1, 4))),
-    dict(L=16, S=1, R=1, T=33, b=(0.5, 2.2), tune=((0, 2), (1, 16))),
+    dict(L=16, S=1, R=2, T=17, b=(0.5, 2.2), tune=((0, 2), (1, 16))),
     dict(L=24, S=1, R=2, T=5, b=(0.5, 2.2), tune=((0, 2), (1, 6))),
 ]
 
