@@ -131,7 +131,7 @@ int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts);
  *   SG_SWEEP_AUTO   z-marching kernel when L is a multiple of 8, else the tiled kernel (default)
  *   SG_SWEEP_TILED  the tiled kernel (any even L)
  *   SG_SWEEP_ZMARCH the z-marching kernel; SG_EINVAL unless L is a multiple of 8
- * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else >= 4 and a divisor of L. */
+ * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else even, >= 4 and a divisor of L. */
 enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1 };
 enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2 };
 int sg_tune(sg_ctx* ctx, int knob, int value);

@@ -655,7 +655,7 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
         return SG_OK;
     case SG_TUNE_ZCHUNK:
         if (value < 0) return SG_EINVAL;
-        if (value > 0 && (ctx->L % 8 != 0 || value < 4 || ctx->L % value != 0)) return SG_EINVAL;
+        if (value > 0 && (ctx->L % 8 != 0 || value < 4 || (value & 1) || ctx->L % value != 0)) return SG_EINVAL;
         ctx->zm_zc_req = value;
         zm_plan(ctx);
         return SG_OK;

@@ -58,7 +58,7 @@ __device__ __forceinline__ void or_update(float hx, float hy, float hz, float& s
     const float hh = fmaf(hx, hx, fmaf(hy, hy, hz * hz));
     const float hs = fmaf(hx, sx, fmaf(hy, sy, hz * sz));
     if (hh >= 1e-30f) {
-        const float f = 2.0f * hs / hh;
+        const float f = __fdividef(2.0f * hs, hh);   // MUFU.RCP + FMUL (2 ulp): the drift it adds to |s| and to s.h is of the order of the fp32 rounding of the reflection itself
         sx = fmaf(f, hx, -sx);
         sy = fmaf(f, hy, -sy);
         sz = fmaf(f, hz, -sz);

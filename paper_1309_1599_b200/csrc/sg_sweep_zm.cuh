@@ -119,7 +119,7 @@ __device__ __forceinline__ void zm_update(const float (&hf)[3][4], float (&s)[3]
 }
 
 template <int KIND, bool WITH_E, int TX, int TY, int NST, int NJ>
-__global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS) k_sweep_zm(const ZmParams p)
+__global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const ZmParams p)
 {
     using Gm = ZmGeom<TX, TY>;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -226,52 +226,57 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS) k_sweep_zm(const ZmPa
     const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.C + (uint32_t)(grp * G + q * 4);
     float eacc[4] = { 0.f, 0.f, 0.f, 0.f };
 
-    // own spin of step k: site (X0 + 2 kx + ((ky + z + colour) & 1), Y, z)
-    auto own_ptr = [&](int k) -> float* {
-        const int z = z0 + k;
-        const int x = X0 + 2 * kx + ((ky + z + p.colour) & 1);
-        return const_cast<float*>(spins_grp) + ((size_t)p.colour * p.Nh + (((size_t)x + (size_t)L * (Y + (size_t)L * z)) >> 1)) * SITE_FLOATS + q * 4;
-    };
+    // Own spin of step k: site (X0 + 2 kx + off, Y, z0 + k), off = (ky + z + colour) & 1.  In the colour-split
+    // order its position is (X0/2 + kx) + (L/2)(Y + L z) whatever off is: a constant stride per plane.
+    const size_t plane = (size_t)Lh * L * SITE_FLOATS;
+    float* own = const_cast<float*>(spins_grp) +
+                 ((size_t)p.colour * p.Nh + (size_t)(X0 >> 1) + kx + (size_t)Lh * (Y + (size_t)L * z0)) * SITE_FLOATS + q * 4;
     float4 pre[2][3];   // register prefetch of the own spins, two steps deep
 #pragma unroll
     for (int d = 0; d < 2; ++d)
 #pragma unroll
-        for (int a = 0; a < 3; ++a) pre[d][a] = (d < ZC) ? ld4(own_ptr(d) + a * G) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int a = 0; a < 3; ++a) pre[d][a] = (d < ZC) ? ld4(own + d * plane + a * G) : make_float4(0.f, 0.f, 0.f, 0.f);
+
+    // Byte offsets of the six neighbours inside a stage, for even and odd steps (z0 and ZC are even, so the
+    // parity of the step is the parity of x3 - z0): +x1, -x1, +x2, -x2 in the plane's own stage, x3 +- 1 in
+    // the next / previous stage at the slot of (x1, x2).
+    uint32_t o_xm[2], o_yp[2], o_ym[2], o_z[2];
+#pragma unroll
+    for (int d = 0; d < 2; ++d) {
+        const int off = (ky + z0 + d + p.colour) & 1;
+        o_xm[d] = (uint32_t)((ky * Gm::ROW + kx) * Gm::SITE_BYTES + q * 16);
+        o_z[d] = (uint32_t)((ky * Gm::ROW + kx + off) * Gm::SITE_BYTES + q * 16);
+        o_ym[d] = (uint32_t)(((ky > 0) ? (ky - 1) * Gm::ROW + kx + off : TY * Gm::ROW + kx) * Gm::SITE_BYTES + q * 16);
+        o_yp[d] = (uint32_t)(((ky < TY - 1) ? (ky + 1) * Gm::ROW + kx + off : TY * Gm::ROW + TX / 2 + kx) * Gm::SITE_BYTES + q * 16);
+    }
+    const uint32_t i0 = (uint32_t)(X0 + 2 * kx + L * (Y + L * z0));   // site index of step k: i0 + off + L^2 k (heat bath only)
 
     mbar_wait(full_o(0 % NST), 0);
     mbar_wait(full_o(1 % NST), 0);
+    // rotating stage indices and phase parities: planes k (x3-1), k+1 (in-plane), k+2 (x3+1); coupling stage of step k
+    int sm_ = 0, s0_ = 1 % NST, sp_ = 2 % NST, sj_ = 0;
+    uint32_t par_p = (2 / NST) & 1, par_j = 0;
 
     for (int k2 = 0; k2 < ZC; k2 += 2) {
 #pragma unroll
         for (int d = 0; d < 2; ++d) {
             const int k = k2 + d;
             if (k >= ZC) break;
-            const int z = z0 + k;
-            const int off = (ky + z + p.colour) & 1;
-            float* const own = own_ptr(k);
             float s[3][4];
 #pragma unroll
             for (int a = 0; a < 3; ++a) { s[a][0] = pre[d][a].x; s[a][1] = pre[d][a].y; s[a][2] = pre[d][a].z; s[a][3] = pre[d][a].w; }
             if (k + 2 < ZC) {
-                const float* nx = own_ptr(k + 2);
 #pragma unroll
-                for (int a = 0; a < 3; ++a) pre[d][a] = ld4(nx + a * G);
+                for (int a = 0; a < 3; ++a) pre[d][a] = ld4(own + 2 * plane + a * G);
             }
-            // planes n = k (x3-1), k+1 (in-plane), k+2 (x3+1)
-            const int sm_ = k % NST, s0_ = (k + 1) % NST, sp_ = (k + 2) % NST;
-            mbar_wait(full_o(sp_), ((k + 2) / NST) & 1);
-            mbar_wait(full_j(k % NJ), (k / NJ) & 1);
-            const unsigned char* const Pm = ring + (size_t)sm_ * Gm::STAGE_BYTES + q * 16;
-            const unsigned char* const P0 = ring + (size_t)s0_ * Gm::STAGE_BYTES + q * 16;
-            const unsigned char* const Pp = ring + (size_t)sp_ * Gm::STAGE_BYTES + q * 16;
-            const int sl_z = ky * Gm::ROW + kx + off;
-            const int sl_xm = ky * Gm::ROW + kx;
-            const int sl_ym = (ky > 0) ? (ky - 1) * Gm::ROW + kx + off : TY * Gm::ROW + kx;
-            const int sl_yp = (ky < TY - 1) ? (ky + 1) * Gm::ROW + kx + off : TY * Gm::ROW + TX / 2 + kx;
-            const unsigned char* nbp[6] = { P0 + (sl_xm + 1) * Gm::SITE_BYTES, P0 + sl_xm * Gm::SITE_BYTES,
-                                            P0 + sl_yp * Gm::SITE_BYTES,       P0 + sl_ym * Gm::SITE_BYTES,
-                                            Pp + sl_z * Gm::SITE_BYTES,        Pm + sl_z * Gm::SITE_BYTES };
-            const unsigned char* const Jp = jring + (size_t)(k % NJ) * Gm::JSTAGE_BYTES + ks * Gm::JSITE_BYTES;
+            mbar_wait(full_o(sp_), par_p);
+            mbar_wait(full_j(sj_), par_j);
+            const unsigned char* const Pm = ring + sm_ * Gm::STAGE_BYTES;
+            const unsigned char* const P0 = ring + s0_ * Gm::STAGE_BYTES;
+            const unsigned char* const Pp = ring + sp_ * Gm::STAGE_BYTES;
+            const unsigned char* nbp[6] = { P0 + o_xm[d] + Gm::SITE_BYTES, P0 + o_xm[d], P0 + o_yp[d], P0 + o_ym[d],
+                                            Pp + o_z[d], Pm + o_z[d] };
+            const unsigned char* const Jp = jring + sj_ * Gm::JSTAGE_BYTES + ks * Gm::JSITE_BYTES;
 
             float hf[3][4];
 #pragma unroll
@@ -301,14 +306,18 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS) k_sweep_zm(const ZmPa
             }
             // the stage of plane k and the coupling stage are dead for this warp once the loads above retire
             __syncwarp();
-            if ((tid & 31) == 0) { mbar_arrive(empty_o(sm_)); mbar_arrive(empty_j(k % NJ)); }
+            if ((tid & 31) == 0) { mbar_arrive(empty_o(sm_)); mbar_arrive(empty_j(sj_)); }
+            sm_ = s0_; s0_ = sp_;
+            sp_ = (sp_ + 1 == NST) ? 0 : sp_ + 1; par_p ^= (sp_ == 0) ? 1u : 0u;
+            sj_ = (sj_ + 1 == NJ) ? 0 : sj_ + 1; par_j ^= (sj_ == 0) ? 1u : 0u;
 
-            const uint32_t i = (uint32_t)(X0 + 2 * kx + off + L * (Y + L * z));
+            const uint32_t i = i0 + (uint32_t)((ky + z0 + d + p.colour) & 1) + (uint32_t)(L * L) * (uint32_t)k;
             zm_update<KIND, WITH_E>(hf, s, eacc, beta4, i, g0, p);
             if (KIND != KIND_ENERGY) {
 #pragma unroll
                 for (int a = 0; a < 3; ++a) st4(own + a * G, make_float4(s[a][0], s[a][1], s[a][2], s[a][3]));
             }
+            own += plane;
         }
     }
 
