@@ -349,7 +349,7 @@ void sgo_sweep_copies(int L, const double* M, double* spins, int n_copies, int k
                       int store_fp32)
 {
     size_t stride = (size_t)3 * L * L * L;
-#pragma omp parallel for schedule(dynamic, 1) if ((size_t)n_copies * stride > 100000)
+#pragma omp parallel for schedule(dynamic, 1) if (n_copies >= 4 && (size_t)n_copies * stride > 20000)
     for (int c = 0; c < n_copies; ++c)
         for (int k = 0; k < n_sweeps; ++k)
             for (int colour = 0; colour < 2; ++colour)
@@ -360,7 +360,7 @@ void sgo_sweep_copies(int L, const double* M, double* spins, int n_copies, int k
 void sgo_energy_copies(int L, const double* M, const double* spins, int n_copies, double* E)
 {
     size_t stride = (size_t)3 * L * L * L;
-#pragma omp parallel for schedule(dynamic, 1) if ((size_t)n_copies * stride > 100000)
+#pragma omp parallel for schedule(dynamic, 1) if (n_copies >= 4 && (size_t)n_copies * stride > 20000)
     for (int c = 0; c < n_copies; ++c) E[c] = sgo_energy(L, M, spins + c * stride);
 }
 
