@@ -65,35 +65,74 @@ __device__ __forceinline__ void or_update(float hx, float hy, float hz, float& s
     }
 }
 
-// Heat bath, Eq. (A1): s drawn from exp(beta s.h).  Exact inverse CDF of the polar
-// cosine about n = h/|h|, evaluated hemisphere by hemisphere so that whichever of w = 1-u, w' = 1+u is
-// small carries a few-ulp relative error (reading R23); uniform azimuth in the frame of
-// Duff et al. (JCGT 2017).
+// MUFU approximations (1-2 ulp): reciprocal, reciprocal square root, square root, 2^x
+__device__ __forceinline__ float rcp_approx(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rsqrt_approx(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float sqrt_approx(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float ex2_approx(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
+// ln(u), u a normal positive float, to a few ulp RELATIVE also next to u = 1 (MUFU.LG2 is only absolutely
+// accurate there): u = m 2^e with m in [sqrt(1/2), sqrt(2)), ln m = 2 atanh(s), s = (m-1)/(m+1), |s| < 0.1716,
+// odd series up to s^9 (next term 2 s^11/11 < 7e-10 ln m).
+__device__ __forceinline__ float log_rel(float u)
+{
+    const int iu = __float_as_int(u);
+    const int e = (iu - 0x3f3504f3) >> 23;
+    const float f = __int_as_float(iu - (e << 23)) - 1.0f;       // exact
+    const float s = f * rcp_approx(2.0f + f);
+    const float z = s * s;
+    const float p = fmaf(z, fmaf(z, fmaf(z, 1.0f / 9.0f, 1.0f / 7.0f), 0.2f), 1.0f / 3.0f);
+    const float s2 = s + s;
+    return fmaf((float)e, 0.69314718f, fmaf(s2 * z, p, s2));
+}
+
+// Heat bath, Eq. (A1): s drawn from exp(beta s.h).  Exact inverse CDF of the polar cosine
+// about n = h/|h|, evaluated so that whichever of w = 1-u (distance from the north
+// pole) and w' = 1+u (from the south pole) is small carries a few-ulp relative error (reading R23), branch-free:
+//   E = e^{-2 kappa}, d = 1 - E, x = r1 d, x' = (1-r1) d / E, y = (1-r1) + r1 E      (1-r1 is exact in fp32)
+//   w  = -ln(1 - x)/kappa = -ln(y)/kappa,      w' = ln(1 + x')/kappa,      w + w' = 2
+// the smaller of x, x' (if <= 1/2) goes through log1p (= ln of the rounded sum plus the first-order correction
+// for that rounding), otherwise ln(y) is well conditioned; uniform azimuth in the frame of Duff et al. (JCGT 2017).
 __device__ __forceinline__ void hb_update(float hx, float hy, float hz, float beta, float r1, float r2,
                                           float& sx, float& sy, float& sz)
 {
     const float hh = fmaf(hx, hx, fmaf(hy, hy, hz * hz));
     float nx = 0.0f, ny = 0.0f, nz = 1.0f, kappa = 0.0f;
     if (hh >= 1e-30f) {
-        const float hn = sqrtf(hh);
-        nx = hx / hn; ny = hy / hn; nz = hz / hn;
-        kappa = beta * hn;
+        const float rs = rsqrt_approx(hh);
+        nx = hx * rs; ny = hy * rs; nz = hz * rs;
+        kappa = beta * (hh * rs);
     }
-    float w, wp, u;                    // w = 1 - u (from the north pole), wp = 1 + u (from the south pole)
+    float w, wp, u;                    // w = 1 - u, wp = 1 + u
     if (kappa < 1e-15f) {              // uniform law
         w = 2.0f * r1; wp = 2.0f - w; u = 1.0f - w;
-    } else if (r1 <= 1.0f / (1.0f + expf(-kappa))) {      // u >= 0
-        const float x = -r1 * expm1f(-2.0f * kappa);       // r1 (1 - e^{-2 kappa}) in [0,1)
-        const float lg = (x <= 0.5f) ? log1pf(-x) : logf((1.0f - r1) + r1 * expf(-2.0f * kappa));
-        w = -lg / kappa; wp = 2.0f - w; u = 1.0f - w;
-    } else {                                               // u < 0; only reachable for kappa < 16.7
-        wp = log1pf((1.0f - r1) * expm1f(2.0f * kappa)) / kappa; w = 2.0f - wp; u = wp - 1.0f;
+    } else {
+        const float a2 = 2.0f * kappa;
+        const float E = ex2_approx(-1.44269504f * a2);            // 0 for kappa > 43.6: then x' = inf, y = 1 - r1
+        float dp = fmaf(a2, 1.0f / 5040.0f, -1.0f / 720.0f);      // 1 - e^{-a} by its series for a < 0.3 (7 terms: 2e-8)
+        dp = fmaf(dp, a2, 1.0f / 120.0f); dp = fmaf(dp, a2, -1.0f / 24.0f); dp = fmaf(dp, a2, 1.0f / 6.0f);
+        dp = fmaf(dp, a2, -0.5f); dp = fmaf(dp, a2, 1.0f); dp *= a2;
+        const float d = (a2 < 0.3f) ? dp : 1.0f - E;
+        const float q1 = 1.0f - r1;
+        const float x = r1 * d;
+        const float xs = q1 * (d * rcp_approx(E));
+        const float y = fmaf(r1, E, q1);
+        const bool south = xs < x;
+        const bool mid = fminf(x, xs) > 0.5f;
+        const float zs = south ? xs : -x;
+        const float arg = mid ? y : 1.0f + zs;
+        float lg = log_rel(arg);
+        lg += mid ? 0.0f : (zs - (arg - 1.0f)) * rcp_approx(arg);  // arg - 1 is exact for arg in [1/2, 2]
+        const float v = lg * rcp_approx(kappa);
+        if (south && !mid) { wp = v; w = 2.0f - v; u = v - 1.0f; }
+        else { w = -v; wp = 2.0f + v; u = 1.0f + v; }
     }
-    const float t = sqrtf(fmaxf(w * wp, 0.0f));
-    float sp, cp;
-    sincospif(2.0f * r2, &sp, &cp);
+    const float t = sqrt_approx(fmaxf(w * wp, 0.0f));
+    // phi = 2 pi r2 reduced exactly to [-pi, pi); MUFU sine / cosine (absolute error 2^-21.4 on that range)
+    const float ph = 6.2831853f * (r2 - (r2 >= 0.5f ? 1.0f : 0.0f));
+    const float sp = __sinf(ph), cp = __cosf(ph);
     const float sg = copysignf(1.0f, nz);
-    const float a = -1.0f / (sg + nz);
+    const float a = -rcp_approx(sg + nz);
     const float b = nx * ny * a;
     const float e1x = 1.0f + sg * nx * nx * a, e1y = sg * b, e1z = -sg * nx;
     const float e2x = b, e2y = sg + ny * ny * a, e2z = -ny;
