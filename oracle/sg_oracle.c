@@ -23,7 +23,9 @@
  * against a dense numpy matrix and the exhaustive L=2 enumeration, ferromagnetic closed forms,
  * gauge / rotation / time-reversal invariance, OR energy conservation and involution, Langevin
  * moments and the KS test of the heat-bath law, Schwinger-Dyson (Eq. (A6)), exact Heisenberg ring
- * energies, Fourier closed forms, PT acceptance frequencies.  What stays "parity unpinned": the
+ * energies, Fourier closed forms, PT acceptance frequencies; chirality (Eq. (2)) against orthonormal triads,
+ * numpy determinants / FFT, the conical-spiral closed form and its symmetries; Eq. (4) against the lattice
+ * Ornstein-Zernike propagator.  What stays "parity unpinned": the
  * literal spin values after a seeded sweep (the paper prints none); the oracle defines them.
  */
 #include <math.h>
@@ -422,4 +424,49 @@ void sgo_overlap(int L, const double* sa, const double* sb, double out[7])
         }
     }
     for (int k = 0; k < 7; ++k) out[k] /= (double)N;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* Chirality observables (Sect. II.B, Eq. (2)):                                  */
+/*   zeta_{x,mu} = s_{x+e_mu} . (s_x x s_{x-e_mu}),  kappa_{x,mu} = zeta^a_{x,mu} zeta^b_{x,mu},  */
+/*   q^_CG^mu(k) = sum_x kappa_{x,mu} e^{i k.x} / N   at k = 0 and k_min + permutations.          */
+/* ------------------------------------------------------------------------------------------ */
+double sgo_chirality(int L, const double* s, int i, int mu)
+{
+    int N = L * L * L;
+    int ip = sgo_neighbour(L, i, mu, +1), im = sgo_neighbour(L, i, mu, -1);
+    double a[3], b[3], c[3];          /* a = s_{x+e_mu}, b = s_x, c = s_{x-e_mu} */
+    for (int k = 0; k < 3; ++k) { a[k] = s[k * N + ip]; b[k] = s[k * N + i]; c[k] = s[k * N + im]; }
+    double cr[3] = { b[1] * c[2] - b[2] * c[1], b[2] * c[0] - b[0] * c[2], b[0] * c[1] - b[1] * c[0] };
+    return a[0] * cr[0] + a[1] * cr[1] + a[2] * cr[2];
+}
+
+/* out[mu] = q^_CG^mu(0); out[3 + 2*(3*mu + nu)], out[4 + 2*(3*mu + nu)] = Re, Im of q^_CG^mu(k_nu),
+ * k_nu = 2 pi e_nu / L; mu, nu = 0,1,2 (21 numbers). */
+void sgo_chiral_overlap(int L, const double* sa, const double* sb, double out[21])
+{
+    int N = L * L * L;
+    for (int k = 0; k < 21; ++k) out[k] = 0.0;
+    for (int i = 0; i < N; ++i) {
+        int x[3];
+        sgo_coords(L, i, x);
+        for (int mu = 0; mu < 3; ++mu) {
+            double kap = sgo_chirality(L, sa, i, mu) * sgo_chirality(L, sb, i, mu);
+            out[mu] += kap;
+            for (int nu = 0; nu < 3; ++nu) {
+                double ang = 2.0 * SGO_PI * (double)x[nu] / (double)L;
+                out[3 + 2 * (3 * mu + nu)] += kap * cos(ang);
+                out[4 + 2 * (3 * mu + nu)] += kap * sin(ang);
+            }
+        }
+    }
+    for (int k = 0; k < 21; ++k) out[k] /= (double)N;
+}
+
+/* Second-moment correlation length, Eq. (4) PAPER.md:93-97:
+ *   xi = sqrt(chi(0)/chi(k_min) - 1) / (2 sin(k_min/2)),  k_min = 2 pi / L;
+ * chi = N <|q^(k)|^2> (Eq. (3)).  A ratio below 1 (possible for noisy estimates) gives NaN. */
+double sgo_xi(int L, double chi0, double chik)
+{
+    return sqrt(chi0 / chik - 1.0) / (2.0 * sin(SGO_PI / (double)L));
 }

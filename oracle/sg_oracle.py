@@ -63,6 +63,9 @@ def lib():
         L.sgo_num_threads.restype = i
         L.sgo_pt_sweep.argtypes = [i, dp, dp, ip, ip, u64, u32, u32, u64p, u64p]
         L.sgo_overlap.argtypes = [i, dp, dp, dp]
+        L.sgo_chirality.argtypes = [i, dp, i, i]; L.sgo_chirality.restype = d
+        L.sgo_chiral_overlap.argtypes = [i, dp, dp, dp]
+        L.sgo_xi.argtypes = [i, d, d]; L.sgo_xi.restype = d
         _lib = L
     return _lib
 
@@ -189,6 +192,23 @@ def overlap(L, sa, sb):
     return out
 
 
+def chirality(L, s, i, mu):
+    """zeta_{x,mu} of Eq. (2) at site i of one copy s [3][N]."""
+    return float(lib().sgo_chirality(L, _dp(s), int(i), int(mu)))
+
+
+def chiral_overlap(L, sa, sb):
+    """(qc0[3], qck[3][3][2]): q^_CG^mu(0) and q^_CG^mu(k_nu) (Re, Im) of two copies."""
+    out = np.zeros(21)
+    lib().sgo_chiral_overlap(L, _dp(sa), _dp(sb), _dp(out))
+    return out[:3].copy(), out[3:].reshape(3, 3, 2).copy()
+
+
+def xi(L, chi0, chik):
+    """Second-moment correlation length, Eq. (4)."""
+    return float(lib().sgo_xi(int(L), float(chi0), float(chik)))
+
+
 def replica_pairs(R):
     """Pairs a<b in the order (0,1),(0,2),...,(R-2,R-1) (reading R15)."""
     return [(a, b) for a in range(R) for b in range(a + 1, R)]
@@ -301,6 +321,20 @@ class OracleSim:
                     q0[s, p, t] = o[0]
                     qk[s, p, t] = o[1:].reshape(3, 2)
         return e, q0, qk
+
+    def measure_chiral(self):
+        """qc0[S][P][T][3], qck[S][P][T][3][3][2]: chiral-glass overlaps of the replica pairs a<b with both
+        copies at temperature t (Eq. (2))."""
+        pairs = replica_pairs(self.R)
+        qc0 = np.zeros((self.S, len(pairs), self.T, 3))
+        qck = np.zeros((self.S, len(pairs), self.T, 3, 3, 2))
+        for s in range(self.S):
+            for p, (a, b) in enumerate(pairs):
+                for t in range(self.T):
+                    sa = self.spins[s][a * self.T + self.slot_of_temp[s, a, t]]
+                    sb = self.spins[s][b * self.T + self.slot_of_temp[s, b, t]]
+                    qc0[s, p, t], qck[s, p, t] = chiral_overlap(self.L, sa, sb)
+        return qc0, qck
 
     def unit(self, n_or):
         """One MCS: 1 HB sweep, n_or OR sweeps, 1 PT sweep."""
