@@ -108,6 +108,21 @@ int sg_pt_swap(sg_ctx* ctx);
  * Synchronises the stream. */
 int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk);
 
+/* Chiral-glass overlaps (Sect. II.B, Eq. (2)):
+ *   zeta_{x,mu}  = s_{x+e_mu} . (s_x x s_{x-e_mu}),  kappa_{x,mu} = zeta^a_{x,mu} zeta^b_{x,mu}
+ *   qc0 double [S][P][T][3]        q^_CG^mu(0)    = sum_x kappa_{x,mu} / N
+ *   qck double [S][P][T][3][3][2]  q^_CG^mu(k_nu) = sum_x kappa_{x,mu} exp(+i 2 pi x_nu / L) / N, (Re, Im)
+ * for the replica pairs a < b in the order of sg_measure, both copies at temperature t (found through the
+ * temperature permutation), mu = chirality direction, nu = direction of k_min.  Host outputs, either may
+ * be NULL.  fp32 triple products, fp64 sums in a fixed order.  For L = 2 every zeta vanishes up to rounding (x+e = x-e).
+ * Synchronises the stream.  Errors: SG_EINVAL (ctx NULL), SG_ESTATE (a sample not initialised), SG_ECUDA. */
+int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck);
+
+/* Second-moment correlation length, Eq. (4) PAPER.md:93-97 (host arithmetic, no device work):
+ *   xi = sqrt(chi(0)/chi(k_min) - 1) / (2 sin(pi/L)),   chi(k) = N <|q^(k)|^2>  (Eq. (3))
+ * for either overlap field.  NaN when chi0 < chik. */
+double sg_correlation_length(int L, double chi0, double chik);
+
 /* ---- state access: tests, checkpoint / resume (all synchronise) ---- */
 int sg_get_spins(sg_ctx* ctx, int sample, float* out /* [C][3][N] */);
 int sg_set_spins(sg_ctx* ctx, int sample, const float* in /* [C][3][N] */);

@@ -18,7 +18,7 @@ SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH = 0, 1, 2
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_sweep_or", "sg_sweep_hb",
-    "sg_pt_swap", "sg_measure", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
+    "sg_pt_swap", "sg_measure", "sg_measure_chiral", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
     "sg_halfsweep", "sg_pt_stats", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
@@ -60,6 +60,8 @@ def load_library():
     L.sg_sweep_hb.argtypes = [vp, i]; L.sg_sweep_hb.restype = i
     L.sg_pt_swap.argtypes = [vp]; L.sg_pt_swap.restype = i
     L.sg_measure.argtypes = [vp, vp, vp, vp]; L.sg_measure.restype = i
+    L.sg_measure_chiral.argtypes = [vp, vp, vp]; L.sg_measure_chiral.restype = i
+    L.sg_correlation_length.argtypes = [i, ctypes.c_double, ctypes.c_double]; L.sg_correlation_length.restype = ctypes.c_double
     L.sg_get_spins.argtypes = [vp, i, vp]; L.sg_get_spins.restype = i
     L.sg_set_spins.argtypes = [vp, i, vp]; L.sg_set_spins.restype = i
     L.sg_get_couplings.argtypes = [vp, i, vp]; L.sg_get_couplings.restype = i
@@ -92,6 +94,11 @@ def _ptr(a):
 def workspace_bytes(L, n_samples, n_replicas, n_temps, seed=0, first_sample=0):
     shape = SgShape(L, n_samples, n_replicas, n_temps, first_sample, 0, seed)
     return int(load_library().sg_workspace_bytes(ctypes.byref(shape)))
+
+
+def correlation_length(L, chi0, chik):
+    """Eq. (4): second-moment correlation length from chi(0), chi(k_min)."""
+    return float(load_library().sg_correlation_length(int(L), float(chi0), float(chik)))
 
 
 def philox4x32_10(ctr, key):
@@ -171,6 +178,12 @@ class SpinGlass:
         qk = np.empty((self.S, self.P, self.T, 3, 2))
         self._check(self._lib.sg_measure(self._ctx, _ptr(e), _ptr(q0), _ptr(qk)), "sg_measure")
         return e, q0, qk
+
+    def measure_chiral(self):
+        """(qc0 [S][P][T][3], qck [S][P][T][3][3][2]): chiral-glass overlaps, Eq. (2) PAPER.md:81-85."""
+        qc0 = np.empty((self.S, self.P, self.T, 3)); qck = np.empty((self.S, self.P, self.T, 3, 3, 2))
+        self._check(self._lib.sg_measure_chiral(self._ctx, _ptr(qc0), _ptr(qck)), "sg_measure_chiral")
+        return qc0, qck
 
     def unit(self, n_or):
         """One MCS: 1 HB sweep, n_or OR sweeps, 1 PT sweep."""

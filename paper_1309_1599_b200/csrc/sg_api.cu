@@ -99,8 +99,8 @@ Offsets offsets(const Geometry& g)
     o.E = c.take((size_t)g.S * g.Cp * sizeof(double));
     o.Epart = c.take((size_t)g.S * g.NG * g.ntiles * G * sizeof(double));
     o.phase = c.take((size_t)g.L * 2 * sizeof(double));
-    o.Mpart = c.take((size_t)g.S * g.nchunk * (g.P * g.T > 0 ? g.P * g.T : 1) * 7 * sizeof(double));
-    o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 7 + 1) * sizeof(double));
+    o.Mpart = c.take((size_t)g.S * g.nchunk * (g.P * g.T > 0 ? g.P * g.T : 1) * 21 * sizeof(double));   // 7 per item (overlap), 21 (chirality)
+    o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + 1) * sizeof(double));
     o.sot = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     o.tos = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     size_t st = (size_t)g.S * g.R * (g.T > 1 ? g.T - 1 : 1) * sizeof(unsigned long long);
@@ -556,6 +556,38 @@ int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
     if (qk && nQ) SG_CUDA(ctx, cudaMemcpyAsync(qk, ctx->result + nE + nQ, (size_t)nQ * 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
+}
+
+int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck)
+{
+    if (!ctx) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    const int PT = ctx->P * ctx->T;
+    const int nQ = ctx->S * PT;
+    if (PT == 0) return SG_OK;
+    ChiralParams p;
+    p.spins = ctx->spins; p.slot_of_temp = ctx->slot_of_temp; p.phase = ctx->phase; p.Mpart = ctx->Mpart;
+    p.L = ctx->L; p.N = ctx->N; p.NG = ctx->NG; p.Cp = ctx->Cp; p.R = ctx->R; p.T = ctx->T; p.P = ctx->P;
+    p.nchunk = ctx->nchunk; p.chunk_sites = ctx->chunk_sites; p.MS = ctx->MS;
+    int threads = ((PT + 31) / 32) * 32;
+    if (threads > 512) threads = 512;
+    if (threads < 128) threads = 128;        // the zeta stage wants a few warps even when there are few items
+    const int nbatch = (PT + threads - 1) / threads;
+    const size_t smem = (size_t)ctx->MS * 3 * ctx->Cp * sizeof(float);
+    if (smem > 48 * 1024) return SG_EINVAL;
+    k_measure_chiral<<<dim3(ctx->nchunk, ctx->S, nbatch), threads, smem, ctx->stream>>>(p);
+    SG_LAUNCHED(ctx);
+    k_reduce_chiral<<<(nQ * 21 + 127) / 128, 128, 0, ctx->stream>>>(ctx->Mpart, ctx->result, ctx->S, PT, ctx->nchunk, ctx->N);
+    SG_LAUNCHED(ctx);
+    if (qc0) SG_CUDA(ctx, cudaMemcpyAsync(qc0, ctx->result, (size_t)nQ * 3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    if (qck) SG_CUDA(ctx, cudaMemcpyAsync(qck, ctx->result + (size_t)nQ * 3, (size_t)nQ * 18 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+double sg_correlation_length(int L, double chi0, double chik)
+{
+    return std::sqrt(chi0 / chik - 1.0) / (2.0 * std::sin(3.14159265358979323846 / (double)L));
 }
 
 int sg_get_couplings(sg_ctx* ctx, int sample, float* out)

@@ -398,4 +398,109 @@ __global__ void k_reduce_measure(const double* __restrict__ Mpart, const double*
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Chirality observables (Eq. (2)): zeta_{x,mu} = s_{x+e_mu} . (s_x x s_{x-e_mu}),
+// kappa_{x,mu} = zeta^a zeta^b, q^_CG^mu(k) = sum_x kappa_{x,mu} e^{ik.x}/N at k = 0 and k_nu = 2 pi e_nu/L.
+// Same structure as k_measure: a CTA owns a chunk of sites; per batch of MS sites the threads first
+// compute zeta_{x,mu} of EVERY copy (thread = copy lane: coalesced 128-byte lines, the stencil's re-reads
+// hit L1/L2) into shared memory, then thread = (replica pair, temperature) looks its two copies up
+// through the temperature permutation and accumulates the 21 sums in fp64.
+// ------------------------------------------------------------------------------------------------
+struct ChiralParams {
+    const float* spins;        // [S][NG][2][Nh][3][G]
+    const int* slot_of_temp;   // [S][R][T]
+    const double* phase;       // [L][2]
+    double* Mpart;             // [S][nchunk][PT][21]
+    int L, N, NG, Cp, R, T, P, nchunk, chunk_sites, MS;
+};
+
+__global__ void k_measure_chiral(const ChiralParams p)
+{
+    extern __shared__ float sm[];   // [MS][3][Cp]: zeta_{x,mu} of every copy
+    const int chunk = blockIdx.x, sample = blockIdx.y;
+    const int PT = p.P * p.T;
+    const int item = blockIdx.z * blockDim.x + threadIdx.x;
+    int ca = 0, cb = 0;
+    const bool live = item < PT;
+    if (live) {
+        const int pr = item / p.T, t = item % p.T;
+        int a = 0, rem = pr;
+        while (rem >= p.R - 1 - a) { rem -= p.R - 1 - a; ++a; }
+        const int b = a + 1 + rem;
+        ca = a * p.T + p.slot_of_temp[((size_t)sample * p.R + a) * p.T + t];
+        cb = b * p.T + p.slot_of_temp[((size_t)sample * p.R + b) * p.T + t];
+    }
+    double acc[21];
+#pragma unroll
+    for (int k = 0; k < 21; ++k) acc[k] = 0.0;
+    const int i_begin = chunk * p.chunk_sites, i_end = min(p.N, i_begin + p.chunk_sites);
+    const float* base = p.spins + (size_t)sample * p.NG * p.N * SITE_FLOATS;
+    const int row = 3 * p.Cp, L = p.L, Nh = p.N >> 1;
+    for (int i0 = i_begin; i0 < i_end; i0 += p.MS) {
+        const int ms = min(p.MS, i_end - i0);
+        __syncthreads();
+        for (int e = threadIdx.x; e < ms * p.Cp; e += blockDim.x) {
+            const int lane = e % G, grp = (e / G) % p.NG, m = e / p.Cp;
+            const int i = i0 + m;
+            const int x[3] = { i % L, (i / L) % L, i / (L * L) };
+            const int stride[3] = { 1, L, L * L };
+            const float* gb = base + (size_t)grp * p.N * SITE_FLOATS + lane;
+            const float* c0 = gb + site_slot(i, L, Nh) * SITE_FLOATS;
+            const float bx = c0[0], by = c0[G], bz = c0[2 * G];
+#pragma unroll
+            for (int mu = 0; mu < 3; ++mu) {
+                const int ip = (x[mu] + 1 == L) ? i - (L - 1) * stride[mu] : i + stride[mu];
+                const int im = (x[mu] == 0) ? i + (L - 1) * stride[mu] : i - stride[mu];
+                const float* pa = gb + site_slot(ip, L, Nh) * SITE_FLOATS;
+                const float* pc = gb + site_slot(im, L, Nh) * SITE_FLOATS;
+                const float ax = pa[0], ay = pa[G], az = pa[2 * G];
+                const float cx = pc[0], cy = pc[G], cz = pc[2 * G];
+                // a . (b x c)
+                const float z = fmaf(ax, fmaf(by, cz, -bz * cy), fmaf(ay, fmaf(bz, cx, -bx * cz), az * fmaf(bx, cy, -by * cx)));
+                sm[m * row + mu * p.Cp + grp * G + lane] = z;
+            }
+        }
+        __syncthreads();
+        if (live) {
+            for (int m = 0; m < ms; ++m) {
+                const float* z = sm + m * row;
+                const int i = i0 + m;
+                const int x[3] = { i % L, (i / L) % L, i / (L * L) };
+                double ph[3][2];
+#pragma unroll
+                for (int nu = 0; nu < 3; ++nu) { ph[nu][0] = p.phase[2 * x[nu]]; ph[nu][1] = p.phase[2 * x[nu] + 1]; }
+#pragma unroll
+                for (int mu = 0; mu < 3; ++mu) {
+                    const double kap = (double)(z[mu * p.Cp + ca] * z[mu * p.Cp + cb]);
+                    acc[mu] += kap;
+#pragma unroll
+                    for (int nu = 0; nu < 3; ++nu) {
+                        acc[3 + 2 * (3 * mu + nu)] = fma(kap, ph[nu][0], acc[3 + 2 * (3 * mu + nu)]);
+                        acc[4 + 2 * (3 * mu + nu)] = fma(kap, ph[nu][1], acc[4 + 2 * (3 * mu + nu)]);
+                    }
+                }
+            }
+        }
+    }
+    if (live) {
+        double* dst = p.Mpart + (((size_t)sample * p.nchunk + chunk) * PT + item) * 21;
+#pragma unroll
+        for (int k = 0; k < 21; ++k) dst[k] = acc[k];
+    }
+}
+
+// result = [ qc0[S][P][T][3] | qck[S][P][T][3][3][2] ]: fixed-order sum over the chunks, times 1/N
+__global__ void k_reduce_chiral(const double* __restrict__ Mpart, double* __restrict__ result, int S, int PT, int nchunk, int N)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int nQ = S * PT;
+    if (t >= nQ * 21) return;
+    const int k = t % 21, item = (t / 21) % PT, sample = t / (21 * PT);
+    double acc = 0.0;
+    for (int c = 0; c < nchunk; ++c) acc += Mpart[(((size_t)sample * nchunk + c) * PT + item) * 21 + k];
+    acc /= (double)N;
+    if (k < 3) result[((size_t)sample * PT + item) * 3 + k] = acc;
+    else result[(size_t)nQ * 3 + ((size_t)sample * PT + item) * 18 + (k - 3)] = acc;
+}
+
 }  // namespace sg
