@@ -470,3 +470,23 @@ double sgo_xi(int L, double chi0, double chik)
 {
     return sqrt(chi0 / chik - 1.0) / (2.0 * sin(SGO_PI / (double)L));
 }
+
+/* ------------------------------------------------------------------------------------------ */
+/* Schwinger-Dyson monitor (App. A.4, Eq. (A6)): the two site averages of     */
+/*   2 T <s_x.h_x> - <(h_x)^2 - (s_x.h_x)^2> = 0,   "averaged over all the sites in the lattice" */
+/* ------------------------------------------------------------------------------------------ */
+/* out[0] = sum_x s_x.h_x / N,  out[1] = sum_x [ h_x.h_x - (s_x.h_x)^2 ] / N  of one configuration. */
+void sgo_sd_terms(int L, const double* M, const double* s, double out[2])
+{
+    int N = L * L * L;
+    out[0] = out[1] = 0.0;
+    for (int i = 0; i < N; ++i) {
+        double h[3];
+        sgo_local_field(L, M, s, i, h);
+        double sh = s[0 * N + i] * h[0] + s[1 * N + i] * h[1] + s[2 * N + i] * h[2];
+        out[0] += sh;
+        out[1] += h[0] * h[0] + h[1] * h[1] + h[2] * h[2] - sh * sh;
+    }
+    out[0] /= (double)N;
+    out[1] /= (double)N;
+}

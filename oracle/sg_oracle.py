@@ -66,6 +66,7 @@ def lib():
         L.sgo_chirality.argtypes = [i, dp, i, i]; L.sgo_chirality.restype = d
         L.sgo_chiral_overlap.argtypes = [i, dp, dp, dp]
         L.sgo_xi.argtypes = [i, d, d]; L.sgo_xi.restype = d
+        L.sgo_sd_terms.argtypes = [i, dp, dp, dp]
         _lib = L
     return _lib
 
@@ -209,6 +210,13 @@ def xi(L, chi0, chik):
     return float(lib().sgo_xi(int(L), float(chi0), float(chik)))
 
 
+def sd_terms(L, M, s):
+    """(sum_x s.h / N, sum_x [h.h - (s.h)^2] / N) of one copy: the two site averages of Eq. (A6)."""
+    out = np.zeros(2)
+    lib().sgo_sd_terms(L, _dp(M), _dp(s), _dp(out))
+    return out
+
+
 def replica_pairs(R):
     """Pairs a<b in the order (0,1),(0,2),...,(R-2,R-1) (reading R15)."""
     return [(a, b) for a in range(R) for b in range(a + 1, R)]
@@ -335,6 +343,15 @@ class OracleSim:
                     sb = self.spins[s][b * self.T + self.slot_of_temp[s, b, t]]
                     qc0[s, p, t], qck[s, p, t] = chiral_overlap(self.L, sa, sb)
         return qc0, qck
+
+    def schwinger_dyson(self):
+        """sd[S][R][T][2]: the two site averages of Eq. (A6) for the copy of replica r at temperature t."""
+        out = np.zeros((self.S, self.R, self.T, 2))
+        for s in range(self.S):
+            for r in range(self.R):
+                for t in range(self.T):
+                    out[s, r, t] = sd_terms(self.L, self.M[s], self.spins[s][r * self.T + self.slot_of_temp[s, r, t]])
+        return out
 
     def unit(self, n_or):
         """One MCS: 1 HB sweep, n_or OR sweeps, 1 PT sweep."""

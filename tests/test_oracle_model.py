@@ -383,3 +383,32 @@ def test_box_muller_normality(oracle):
     from scipy import stats
     M = oracle.gen_couplings(8, 9, 0, 2, 1.0)          # GENERAL9: nine normals per link
     assert stats.kstest(M.ravel(), "norm").pvalue > 1e-3
+
+
+# ---------------------------------------------------------------------------------------------
+# Schwinger-Dyson terms (Eq. (A6)): pins of oracle.sd_terms
+# ---------------------------------------------------------------------------------------------
+def test_sd_terms_closed_forms_and_energy_relation(oracle):
+    """Ferromagnet, all spins equal: h = 6 s, so <s.h> = 6 and <h^2 - (s.h)^2> = 0; staggered: s.h = -6.
+    Any couplings: sum_x s.h = -2 H (each link enters the fields of both its ends).  A spin orthogonal to its
+    field contributes h^2 to the second term: checked on the dense numpy route (h = A s)."""
+    L = 4
+    N = L ** 3
+    M = oracle.gen_couplings(L, 1, 0, oracle.FERRO, 0.0)
+    s = np.zeros((3, N)); s[2] = 1.0
+    assert np.allclose(oracle.sd_terms(L, M, s), [6.0, 0.0], atol=1e-14)
+    idx = np.arange(N)
+    stag = np.where((idx % L + (idx // L) % L + idx // (L * L)) % 2 == 0, 1.0, -1.0)
+    s2 = np.zeros((3, N)); s2[2] = stag
+    assert np.allclose(oracle.sd_terms(L, M, s2), [-6.0, 0.0], atol=1e-14)
+    rng = np.random.default_rng(12)
+    for L in (2, 4):
+        N = L ** 3
+        M = W.random_couplings(rng, N, "general")
+        s = W.random_spins(rng, 1, N, fp32=False)[0]
+        a, b = oracle.sd_terms(L, M, s)
+        assert abs(a * N + 2.0 * oracle.energy(L, M, s)) < 1e-11 * N
+        h = np.stack([oracle.local_field(L, M, s, i) for i in range(N)], axis=1)      # [3][N]
+        sh = (s * h).sum(axis=0)
+        assert abs(b - ((h * h).sum(axis=0) - sh ** 2).mean()) < 1e-12
+        assert b >= 0.0                                                                 # |h|^2 >= (s.h)^2 for unit s
