@@ -118,6 +118,13 @@ int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk);
  * Synchronises the stream.  Errors: SG_EINVAL (ctx NULL), SG_ESTATE (a sample not initialised), SG_ECUDA. */
 int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck);
 
+/* Schwinger-Dyson monitor (App. A.4, Eq. (A6)):
+ *   2 T <s_x.h_x> - <(h_x)^2 - (s_x.h_x)^2> = 0 in equilibrium, "averaged over all the sites in the lattice".
+ *   sd double [S][R][T][2]   sd[..][0] = sum_x s_x.h_x / N,  sd[..][1] = sum_x [h_x.h_x - (s_x.h_x)^2] / N
+ * of the copy of replica r at temperature t (current configuration; the caller averages over time and forms
+ * 2 sd[0]/beta_t - sd[1]).  Host output, required.  fp32 fields, fp64 sums in a fixed order.  Synchronises. */
+int sg_schwinger_dyson(sg_ctx* ctx, double* sd);
+
 /* Second-moment correlation length, Eq. (4) PAPER.md:93-97 (host arithmetic, no device work):
  *   xi = sqrt(chi(0)/chi(k_min) - 1) / (2 sin(pi/L)),   chi(k) = N <|q^(k)|^2>  (Eq. (3))
  * for either overlap field.  NaN when chi0 < chik. */

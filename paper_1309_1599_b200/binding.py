@@ -18,7 +18,7 @@ SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH = 0, 1, 2
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_sweep_or", "sg_sweep_hb",
-    "sg_pt_swap", "sg_measure", "sg_measure_chiral", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
+    "sg_pt_swap", "sg_measure", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
     "sg_halfsweep", "sg_pt_stats", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
@@ -61,6 +61,7 @@ def load_library():
     L.sg_pt_swap.argtypes = [vp]; L.sg_pt_swap.restype = i
     L.sg_measure.argtypes = [vp, vp, vp, vp]; L.sg_measure.restype = i
     L.sg_measure_chiral.argtypes = [vp, vp, vp]; L.sg_measure_chiral.restype = i
+    L.sg_schwinger_dyson.argtypes = [vp, vp]; L.sg_schwinger_dyson.restype = i
     L.sg_correlation_length.argtypes = [i, ctypes.c_double, ctypes.c_double]; L.sg_correlation_length.restype = ctypes.c_double
     L.sg_get_spins.argtypes = [vp, i, vp]; L.sg_get_spins.restype = i
     L.sg_set_spins.argtypes = [vp, i, vp]; L.sg_set_spins.restype = i
@@ -184,6 +185,12 @@ class SpinGlass:
         qc0 = np.empty((self.S, self.P, self.T, 3)); qck = np.empty((self.S, self.P, self.T, 3, 3, 2))
         self._check(self._lib.sg_measure_chiral(self._ctx, _ptr(qc0), _ptr(qck)), "sg_measure_chiral")
         return qc0, qck
+
+    def schwinger_dyson(self):
+        """sd [S][R][T][2]: site averages of s.h and of h.h - (s.h)^2 per (replica, temperature), Eq. (A6)."""
+        sd = np.empty((self.S, self.R, self.T, 2))
+        self._check(self._lib.sg_schwinger_dyson(self._ctx, _ptr(sd)), "sg_schwinger_dyson")
+        return sd
 
     def unit(self, n_or):
         """One MCS: 1 HB sweep, n_or OR sweeps, 1 PT sweep."""

@@ -19,7 +19,7 @@ struct sg_ctx {
     cudaStream_t stream;
     // device arrays (carved from the caller's workspace)
     float* spins; float* Jg; float* Jt; float* Mraw; float* staging; float* beta_slot;
-    double* betas; double* E; double* Epart; double* phase; double* Mpart; double* result;
+    double* betas; double* E; double* Epart; double* SDpart; double* phase; double* Mpart; double* result;
     int* slot_of_temp; int* temp_of_slot;
     unsigned long long* attempts; unsigned long long* accepts;
     // sweep geometry
@@ -82,7 +82,7 @@ struct Carve {
 };
 
 struct Offsets {
-    size_t spins, Jg, Jt, Mraw, staging, beta_slot, betas, E, Epart, phase, Mpart, result, sot, tos, att, acc, total;
+    size_t spins, Jg, Jt, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, total;
 };
 
 Offsets offsets(const Geometry& g)
@@ -98,6 +98,7 @@ Offsets offsets(const Geometry& g)
     o.betas = c.take((size_t)g.T * sizeof(double));
     o.E = c.take((size_t)g.S * g.Cp * sizeof(double));
     o.Epart = c.take((size_t)g.S * g.NG * g.ntiles * G * sizeof(double));
+    o.SDpart = c.take((size_t)g.S * g.NG * 2 * g.ntiles * G * 2 * sizeof(double));
     o.phase = c.take((size_t)g.L * 2 * sizeof(double));
     o.Mpart = c.take((size_t)g.S * g.nchunk * (g.P * g.T > 0 ? g.P * g.T : 1) * 21 * sizeof(double));   // 7 per item (overlap), 21 (chirality)
     o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + 1) * sizeof(double));
@@ -377,6 +378,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->spins = (float*)(base + o.spins); ctx->Jg = (float*)(base + o.Jg); ctx->Jt = (g.L % 8 == 0) ? (float*)(base + o.Jt) : nullptr; ctx->Mraw = (float*)(base + o.Mraw);
     ctx->staging = (float*)(base + o.staging); ctx->beta_slot = (float*)(base + o.beta_slot);
     ctx->betas = (double*)(base + o.betas); ctx->E = (double*)(base + o.E); ctx->Epart = (double*)(base + o.Epart);
+    ctx->SDpart = (double*)(base + o.SDpart);
     ctx->phase = (double*)(base + o.phase); ctx->Mpart = (double*)(base + o.Mpart);
     ctx->result = (double*)(base + o.result);
     ctx->slot_of_temp = (int*)(base + o.sot); ctx->temp_of_slot = (int*)(base + o.tos);
@@ -581,6 +583,24 @@ int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck)
     SG_LAUNCHED(ctx);
     if (qc0) SG_CUDA(ctx, cudaMemcpyAsync(qc0, ctx->result, (size_t)nQ * 3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (qck) SG_CUDA(ctx, cudaMemcpyAsync(qck, ctx->result + (size_t)nQ * 3, (size_t)nQ * 18 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_schwinger_dyson(sg_ctx* ctx, double* sd)
+{
+    if (!ctx || !sd) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    SdParams p;
+    p.spins = ctx->spins; p.Jg = ctx->Jg; p.SDpart = ctx->SDpart;
+    p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.ntiles = ctx->ntiles; p.tile_sites = ctx->tile_sites;
+    k_sd<<<dim3(ctx->NG * ctx->ntiles, ctx->S, 2), SWEEP_THREADS, 0, ctx->stream>>>(p);
+    SG_LAUNCHED(ctx);
+    const int total = ctx->S * ctx->R * ctx->T * 2;
+    k_reduce_sd<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->SDpart, ctx->slot_of_temp, ctx->result, ctx->S, ctx->R, ctx->T,
+                                                              ctx->NG, ctx->ntiles, ctx->N);
+    SG_LAUNCHED(ctx);
+    SG_CUDA(ctx, cudaMemcpyAsync(sd, ctx->result, (size_t)total * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
 }

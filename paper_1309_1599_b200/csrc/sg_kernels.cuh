@@ -503,4 +503,101 @@ __global__ void k_reduce_chiral(const double* __restrict__ Mpart, double* __rest
     else result[(size_t)nQ * 3 + ((size_t)sample * PT + item) * 18 + (k - 3)] = acc;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Schwinger-Dyson monitor (Eq. (A6)): per copy, the site sums of s.h and of
+// h.h - (s.h)^2 over BOTH colours (blockIdx.z = colour).  Same decomposition as k_sweep (a CTA = a tile of
+// same-colour sites of one copy group; neighbours through L1/L2); a read-only pass, off the timed path.
+// ------------------------------------------------------------------------------------------------
+struct SdParams {
+    const float* spins;      // [S][NG][2][Nh][3][G]
+    const float* Jg;         // [S][2][Nh][JG]
+    double* SDpart;          // [S][NG][2*ntiles][G][2]
+    int L, N, Nh, NG, ntiles, tile_sites;
+};
+
+__global__ void __launch_bounds__(SWEEP_THREADS) k_sd(const SdParams p)
+{
+    const int tid = threadIdx.x, q = tid & 7, slot = tid >> 3;
+    const int grp = blockIdx.x % p.NG, tile = blockIdx.x / p.NG, sample = blockIdx.y, colour = blockIdx.z;
+    const int L = p.L;
+    const float* const sp = p.spins + ((size_t)(sample * p.NG + grp) * p.N) * SITE_FLOATS + q * 4;
+    const float* const Jc = p.Jg + ((size_t)(sample * 2 + colour) * p.Nh) * JG;
+    float acc_a[4] = { 0.f, 0.f, 0.f, 0.f }, acc_b[4] = { 0.f, 0.f, 0.f, 0.f };
+    const int h_end = min(p.Nh, (tile + 1) * p.tile_sites);
+    for (int h = tile * p.tile_sites + slot; h < h_end; h += SLOTS) {
+        int x, y, z;
+        site_of<0>(h, colour, L, x, y, z);
+        const int xp = (x + 1 == L) ? 0 : x + 1, xm = (x == 0) ? L - 1 : x - 1;
+        const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+        const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+        const int row = L * (y + L * z);
+        const int nb[6] = { xp + row, xm + row, x + L * (yp + L * z), x + L * (ym + L * z), x + L * (y + L * zp), x + L * (y + L * zm) };
+        float J[JG];
+        const float* jp = Jc + (size_t)h * JG;
+#pragma unroll
+        for (int v = 0; v < JG / 4; ++v) {
+            const float4 t4 = ldg4(jp + 4 * v);
+            J[4 * v] = t4.x; J[4 * v + 1] = t4.y; J[4 * v + 2] = t4.z; J[4 * v + 3] = t4.w;
+        }
+        const float* const own = sp + ((size_t)colour * p.Nh + h) * SITE_FLOATS;
+        float s[3][4], hf[3][4];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const float4 t4 = ld4(own + a * G);
+            s[a][0] = t4.x; s[a][1] = t4.y; s[a][2] = t4.z; s[a][3] = t4.w;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) hf[a][j] = 0.f;
+        }
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const float* np_ = sp + ((size_t)(1 - colour) * p.Nh + (nb[k] >> 1)) * SITE_FLOATS;
+            float n[3][4];
+#pragma unroll
+            for (int b = 0; b < 3; ++b) {
+                const float4 t4 = ld4(np_ + b * G);
+                n[b][0] = t4.x; n[b][1] = t4.y; n[b][2] = t4.z; n[b][3] = t4.w;
+            }
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * k + 3 * a + b], n[b][j], hf[a][j]);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const float sh = fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
+            const float hh = fmaf(hf[0][j], hf[0][j], fmaf(hf[1][j], hf[1][j], hf[2][j] * hf[2][j]));
+            acc_a[j] += sh;
+            acc_b[j] += fmaf(-sh, sh, hh);
+        }
+    }
+    __shared__ double red[SLOTS][G + 1];
+    for (int k = 0; k < 2; ++k) {
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) red[slot][q * 4 + j] = (double)(k ? acc_b[j] : acc_a[j]);
+        __syncthreads();
+        if (tid < G) {
+            double acc = 0.0;
+            for (int r = 0; r < SLOTS; ++r) acc += red[r][tid];
+            p.SDpart[((((size_t)(sample * p.NG + grp) * 2 + colour) * p.ntiles + tile) * G + tid) * 2 + k] = acc;
+        }
+    }
+}
+
+// sd[S][R][T][2] = (sum_x s.h / N, sum_x [h.h - (s.h)^2] / N) of the copy of replica r at temperature t
+__global__ void k_reduce_sd(const double* __restrict__ SDpart, const int* __restrict__ slot_of_temp, double* __restrict__ result,
+                            int S, int R, int T, int NG, int ntiles, int N)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= S * R * T * 2) return;
+    const int k = u & 1, t = (u >> 1) % T, r = (u / (2 * T)) % R, sample = u / (2 * T * R);
+    const int c = r * T + slot_of_temp[((size_t)sample * R + r) * T + t];
+    const int grp = c / G, lane = c % G;
+    double acc = 0.0;
+    for (int b = 0; b < 2 * ntiles; ++b) acc += SDpart[((((size_t)(sample * NG + grp)) * 2 * ntiles + b) * G + lane) * 2 + k];
+    result[u] = acc / (double)N;
+}
+
 }  // namespace sg

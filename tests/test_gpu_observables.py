@@ -1,4 +1,4 @@
-"""GPU parity of sg_measure_chiral (Eq. (2)) against the oracle on the same seeded inputs,
+"""GPU parity of the widened observables: sg_schwinger_dyson (Eq. (A6); end of file) and sg_measure_chiral (Eq. (2)) against the oracle on the same seeded inputs,
 element by element; tolerance 1e-6 absolute on every q^_CG (fp32 triple products of unit vectors, fp64 sums:
 the same bar as the overlap q^ of sg_measure)."""
 import numpy as np
@@ -90,3 +90,65 @@ def test_measure_chiral_at_full_size(sg, oracle):
 def test_correlation_length_matches_eq4(sg, oracle):
     for L, c0, ck in [(8, 2.0, 1.0), (64, 10.0, 0.3), (16, 1.5, 1.4)]:
         assert abs(sg.correlation_length(L, c0, ck) - oracle.xi(L, c0, ck)) <= 1e-12 * oracle.xi(L, c0, ck)
+
+
+# ---------------------------------------------------------------------------------------------
+# Schwinger-Dyson monitor (Eq. (A6))
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("sh", SHAPES)
+def test_schwinger_dyson_terms_match_oracle(sg, oracle, sh):
+    """Element by element on the same seeded configuration, through a non-trivial permutation.  Tolerance: the
+    north star's energy bar, 1e-6 relative to max(1, |value|) (fp32 fields, fp64 sums)."""
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, np.linspace(0.5, 2.0, T), seed=23, gen_mode=2)
+    rng = np.random.default_rng(4)
+    for s in range(S):
+        tos = np.stack([rng.permutation(T) for _ in range(R)]).astype(np.int32)
+        gpu.set_perm(s, tos)
+        sim.temp_of_slot[s] = tos
+        for r in range(R):
+            sim.slot_of_temp[s, r, tos[r]] = np.arange(T)
+    got, want = gpu.schwinger_dyson(), sim.schwinger_dyson()
+    assert np.all(np.abs(got - want) <= 1e-6 * np.maximum(1.0, np.abs(want))), np.abs(got - want).max()
+
+
+def test_schwinger_dyson_identity_holds_in_equilibrium_on_gpu(sg, oracle):
+    """cfg 0 chain on the GPU (HB + OR + PT): the time average of 2 T s.h - (h^2 - (s.h)^2) vanishes within errors at
+    every temperature, and does not when the temperature is misassigned by 10 % (power check)."""
+    cfg = W.CONFIGS[0]
+    K, n_units = 4, 3000
+    L, R, T = cfg.L, cfg.n_replicas, cfg.n_temps
+    gpu = sg.SpinGlass(L, K, R, T, cfg.betas, seed=5)
+    M = oracle.gen_couplings(L, cfg.seed, 0, oracle.OFFDIAG_SYM, cfg.sigma_D).astype(np.float32)
+    for k in range(K):
+        gpu.init_sample(k, couplings=M)
+    rows = []
+    for u in range(n_units):
+        gpu.unit(cfg.n_or)
+        if u >= n_units // 3:
+            rows.append(gpu.schwinger_dyson())
+    sd = np.array(rows)                                              # [n][K][R][T][2]
+    Tt = 1.0 / cfg.betas
+    for scale, must_hold in ((1.0, True), (1.1, False)):
+        v = 2 * scale * Tt * sd[..., 0] - sd[..., 1]                 # [n][K][R][T]
+        nb = 10
+        n = (v.shape[0] // nb) * nb
+        b = v[:n].reshape(nb, n // nb, K, R, T).mean(axis=1).reshape(nb * K * R, T)
+        z = b.mean(axis=0) / (b.std(axis=0, ddof=1) / np.sqrt(b.shape[0]))
+        assert (np.abs(z).max() < 4.5) == must_hold, (scale, z)
+
+
+def test_schwinger_dyson_at_full_size(sg, oracle):
+    cfg = W.CONFIGS[4]
+    L, R, T = cfg.L, cfg.n_replicas, cfg.n_temps
+    C = R * T
+    M = oracle.gen_couplings(L, cfg.seed, 0, oracle.OFFDIAG_SYM, cfg.sigma_D)
+    X = np.empty((C, 3, L ** 3), dtype=np.float32)
+    for c in range(C):
+        X[c] = oracle.gen_spins(L, cfg.seed, c)
+    gpu = sg.SpinGlass(L, 1, R, T, cfg.betas, seed=cfg.seed)
+    gpu.init_sample(0, couplings=M.astype(np.float32), spins=X)
+    got = gpu.schwinger_dyson()
+    for r, t in [(0, 0), (3, 47), (1, 16), (2, 31)]:
+        want = oracle.sd_terms(L, M, X[r * T + t].astype(np.float64))
+        assert np.all(np.abs(got[0, r, t] - want) <= 1e-6 * np.maximum(1.0, np.abs(want)))
