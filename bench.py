@@ -7,7 +7,8 @@ A step is one unit (MCS): sg_sweep_hb(1); sg_sweep_or(n_or); sg_pt
 after every `measure_every`-th unit.  `value` = HB + OR single-spin updates per second over the whole job
 (all ranks), state resident in HBM, timed with CUDA events on the launching stream, max over ranks.
 `e2e` = the same unit through the C ABI with host buffers: every step uploads the spin state of every
-sample from pinned host memory (sg_set_spins), runs the unit and reads the measurement back (sg_measure).
+sample from pinned host memory (sg_set_spins), runs the unit and reads the measurement back (sg_measure);
+the samples are independent chains, each driven through its own context / stream / host thread.
 `roofline` = the OR half-sweep kernel against the measured HBM copy bandwidth.
 `cpu_baseline` / `--impl reference` = the fp64 oracle (oracle/), as it stands, on the host cores.
 Prints ONE JSON line on rank 0.
@@ -233,22 +234,38 @@ def run_ours(args, cfg):
     for s in range(S):
         host[s].numpy()[...] = gpu.get_spins(s)
     e2e_steps = max(1, min(args.steps, 5))
-    d2h = 0
 
-    def e2e_step(k):
-        for s in range(S):
-            gpu.set_spins(s, host[s].numpy())
-        gpu.sweep_hb(1); gpu.sweep_or(cfg.n_or); gpu.pt_swap()
-        res = gpu.measure()
-        return sum(a.nbytes for a in res)
+    # One single-sample context per sample, each on its own stream and host thread (ctypes releases the GIL):
+    # the samples are independent chains, and `first_sample` gives every context the Philox
+    # streams it has inside the S-sample context, so the upload of one sample overlaps the sweeps of the others.
+    first = multi.first_sample_of_rank(rank, S)
+    gpu.close(); del gpu
+    import concurrent.futures as cf
+    ctxs = []
+    for s in range(S):
+        c = sg.SpinGlass(L, 1, R, T, cfg.betas, seed=cfg.seed, first_sample=first + s, stream=torch.cuda.Stream(device))
+        c.init_sample(0, sg.GEN_OFFDIAG_SYM, cfg.sigma_D)
+        ctxs.append(c)
 
-    e2e_step(0)
-    multi.barrier(); torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    for k in range(e2e_steps):
-        d2h = e2e_step(k)
-    torch.cuda.synchronize()
-    e2e_seconds = time.perf_counter() - t0
+    upload = threading.Lock()       # one upload at a time: the samples take turns on the PCIe link instead of sharing it
+
+    def e2e_chain(s, n_steps):
+        torch.cuda.set_device(local_rank)
+        c, nbytes = ctxs[s], 0
+        for k in range(n_steps):
+            with upload:
+                c.set_spins(0, host[s].numpy())
+            c.sweep_hb(1); c.sweep_or(cfg.n_or); c.pt_swap()
+            nbytes = sum(a.nbytes for a in c.measure())
+        return nbytes
+
+    with cf.ThreadPoolExecutor(max_workers=S) as pool:
+        list(pool.map(lambda s: e2e_chain(s, 1), range(S)))          # warm-up step
+        multi.barrier(); torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        d2h = sum(pool.map(lambda s: e2e_chain(s, e2e_steps), range(S)))
+        torch.cuda.synchronize()
+        e2e_seconds = time.perf_counter() - t0
     multi.barrier()
     e2e_value, _, _ = multi.whole_job_rate(e2e_steps * cfg.updates_per_unit, e2e_seconds, device)
 
@@ -262,8 +279,9 @@ def run_ours(args, cfg):
                                   % (state_bytes / 1e9)),
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": int(d2h),
-                "steps": e2e_steps, "what": "per step: sg_set_spins of every sample from pinned host memory, "
-                                            "one unit, sg_measure to host"},
+                "steps": e2e_steps, "what": "per step and sample: sg_set_spins from pinned host memory, one unit, sg_measure to "
+                                            "host; one single-sample context, stream and host thread per sample (independent "
+                                            "chains), so uploads overlap sweeps; wall clock over all samples and steps"},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": "OR half-sweep (k_sweep_zm<OR> for L %% 8 == 0, else k_sweep<OR>), sweep_impl=%s zchunk=%d"
                                                   % (args.sweep_impl, args.zchunk),
