@@ -72,7 +72,7 @@ Geometry geometry(const sg_shape* s)
     // measure chunks
     g.nchunk = g.N / 512; if (g.nchunk < 1) g.nchunk = 1; if (g.nchunk > 256) g.nchunk = 256;
     g.chunk_sites = (g.N + g.nchunk - 1) / g.nchunk;
-    g.MS = 10240 / (3 * g.Cp); if (g.MS < 1) g.MS = 1; if (g.MS > 8) g.MS = 8;
+    g.MS = 11500 / (3 * g.Cp); if (g.MS < 1) g.MS = 1; if (g.MS > 16) g.MS = 16;
     return g;
 }
 
@@ -543,7 +543,7 @@ int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
         int threads = ((PT + 31) / 32) * 32;
         if (threads > 512) threads = 512;
         const int nbatch = (PT + threads - 1) / threads;
-        const size_t smem = (size_t)ctx->MS * 3 * ctx->Cp * sizeof(float);
+        const size_t smem = (size_t)ctx->MS * 3 * ctx->Cp * sizeof(float) + (size_t)ctx->MS * 6 * sizeof(double);
         if (smem > 48 * 1024) return SG_EINVAL;
         k_measure<<<dim3(ctx->nchunk, ctx->S, nbatch), threads, smem, ctx->stream>>>(p);
         SG_LAUNCHED(ctx);
@@ -575,7 +575,7 @@ int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck)
     if (threads > 512) threads = 512;
     if (threads < 128) threads = 128;        // the zeta stage wants a few warps even when there are few items
     const int nbatch = (PT + threads - 1) / threads;
-    const size_t smem = (size_t)ctx->MS * 3 * ctx->Cp * sizeof(float);
+    const size_t smem = (size_t)ctx->MS * 3 * ctx->Cp * sizeof(float) + (size_t)ctx->MS * 6 * sizeof(double) + (size_t)ctx->MS * 8 * sizeof(int);
     if (smem > 48 * 1024) return SG_EINVAL;
     k_measure_chiral<<<dim3(ctx->nchunk, ctx->S, nbatch), threads, smem, ctx->stream>>>(p);
     SG_LAUNCHED(ctx);

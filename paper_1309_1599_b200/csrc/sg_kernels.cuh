@@ -326,7 +326,8 @@ struct MeasureParams {
 
 __global__ void k_measure(const MeasureParams p)
 {
-    extern __shared__ float sm[];   // [MS][3][Cp]
+    extern __shared__ float sm[];   // [MS][3][Cp] spins, then [MS][3][2] doubles: phases of the batch's sites
+    double* const ph = reinterpret_cast<double*>(sm + (size_t)p.MS * 3 * p.Cp);
     const int chunk = blockIdx.x, sample = blockIdx.y;
     const int PT = p.P * p.T;
     const int item = blockIdx.z * blockDim.x + threadIdx.x;
@@ -347,10 +348,18 @@ __global__ void k_measure(const MeasureParams p)
     for (int i0 = i_begin; i0 < i_end; i0 += p.MS) {
         const int ms = min(p.MS, i_end - i0);
         __syncthreads();
-        for (int e = threadIdx.x; e < ms * p.NG * SITE_FLOATS; e += blockDim.x) {
-            const int lane = e % G, comp = (e / G) % 3, grp = (e / SITE_FLOATS) % p.NG, m = e / (SITE_FLOATS * p.NG);
-            sm[m * row + comp * p.Cp + grp * G + lane] =
-                base[((size_t)grp * p.N + site_slot(i0 + m, p.L, p.N >> 1)) * SITE_FLOATS + comp * G + lane];
+        // a warp copies the three 128-byte lines of one (site, copy group) per pass
+        for (int r = threadIdx.x >> 5; r < ms * p.NG; r += blockDim.x >> 5) {
+            const int m = r / p.NG, grp = r - m * p.NG, lane = threadIdx.x & 31;
+            const float* src = base + ((size_t)grp * p.N + site_slot(i0 + m, p.L, p.N >> 1)) * SITE_FLOATS + lane;
+            float* dst = sm + m * row + grp * G + lane;
+            dst[0] = src[0]; dst[p.Cp] = src[G]; dst[2 * p.Cp] = src[2 * G];
+        }
+        if (threadIdx.x < ms * 3) {                 // e^{i 2 pi x_mu / L} of the batch's sites, once per batch
+            const int m = threadIdx.x / 3, mu = threadIdx.x % 3, i = i0 + m;
+            const int xm = (mu == 0) ? i % p.L : ((mu == 1) ? (i / p.L) % p.L : i / (p.L * p.L));
+            ph[m * 6 + 2 * mu] = p.phase[2 * xm];
+            ph[m * 6 + 2 * mu + 1] = p.phase[2 * xm + 1];
         }
         __syncthreads();
         if (live) {
@@ -358,14 +367,9 @@ __global__ void k_measure(const MeasureParams p)
                 const float* s = sm + m * row;
                 const float qf = fmaf(s[ca], s[cb], fmaf(s[p.Cp + ca], s[p.Cp + cb], s[2 * p.Cp + ca] * s[2 * p.Cp + cb]));
                 const double qx = (double)qf;
-                const int i = i0 + m;
-                const int x[3] = { i % p.L, (i / p.L) % p.L, i / (p.L * p.L) };
                 acc[0] += qx;
 #pragma unroll
-                for (int mu = 0; mu < 3; ++mu) {
-                    acc[1 + 2 * mu] = fma(qx, p.phase[2 * x[mu]], acc[1 + 2 * mu]);
-                    acc[2 + 2 * mu] = fma(qx, p.phase[2 * x[mu] + 1], acc[2 + 2 * mu]);
-                }
+                for (int k = 0; k < 6; ++k) acc[1 + k] = fma(qx, ph[m * 6 + k], acc[1 + k]);
             }
         }
     }
@@ -416,7 +420,9 @@ struct ChiralParams {
 
 __global__ void k_measure_chiral(const ChiralParams p)
 {
-    extern __shared__ float sm[];   // [MS][3][Cp]: zeta_{x,mu} of every copy
+    extern __shared__ float sm[];   // [MS][3][Cp]: zeta_{x,mu} of every copy; then [MS][3][2] doubles: phases
+    double* const phs = reinterpret_cast<double*>(sm + (size_t)p.MS * 3 * p.Cp);
+    int* const nbs = reinterpret_cast<int*>(phs + (size_t)p.MS * 6);   // [MS][8]: site positions of the stencil
     const int chunk = blockIdx.x, sample = blockIdx.y;
     const int PT = p.P * p.T;
     const int item = blockIdx.z * blockDim.x + threadIdx.x;
@@ -439,20 +445,30 @@ __global__ void k_measure_chiral(const ChiralParams p)
     for (int i0 = i_begin; i0 < i_end; i0 += p.MS) {
         const int ms = min(p.MS, i_end - i0);
         __syncthreads();
-        for (int e = threadIdx.x; e < ms * p.Cp; e += blockDim.x) {
-            const int lane = e % G, grp = (e / G) % p.NG, m = e / p.Cp;
-            const int i = i0 + m;
-            const int x[3] = { i % L, (i / L) % L, i / (L * L) };
-            const int stride[3] = { 1, L, L * L };
+        // positions (own, x1+-1, x2+-1, x3+-1) of the batch's sites in the colour-split order, once per batch
+        if (threadIdx.x < ms * 7) {
+            const int m = threadIdx.x / 7, k = threadIdx.x % 7, i = i0 + m;
+            int j = i;
+            if (k > 0) {
+                const int mu = (k - 1) >> 1, up = (k - 1) & 1 ? 0 : 1;
+                const int st = (mu == 0) ? 1 : ((mu == 1) ? L : L * L);
+                const int xm = (mu == 0) ? i % L : ((mu == 1) ? (i / L) % L : i / (L * L));
+                j = up ? ((xm + 1 == L) ? i - (L - 1) * st : i + st) : ((xm == 0) ? i + (L - 1) * st : i - st);
+            }
+            nbs[m * 8 + k] = (int)site_slot(j, L, Nh);
+        }
+        __syncthreads();
+        // a warp computes zeta_{x,mu} of the 32 copies of one (site, copy group) per pass
+        for (int r = threadIdx.x >> 5; r < ms * p.NG; r += blockDim.x >> 5) {
+            const int m = r / p.NG, grp = r - m * p.NG, lane = threadIdx.x & 31;
             const float* gb = base + (size_t)grp * p.N * SITE_FLOATS + lane;
-            const float* c0 = gb + site_slot(i, L, Nh) * SITE_FLOATS;
+            const int* nb = nbs + m * 8;
+            const float* c0 = gb + (size_t)nb[0] * SITE_FLOATS;
             const float bx = c0[0], by = c0[G], bz = c0[2 * G];
 #pragma unroll
             for (int mu = 0; mu < 3; ++mu) {
-                const int ip = (x[mu] + 1 == L) ? i - (L - 1) * stride[mu] : i + stride[mu];
-                const int im = (x[mu] == 0) ? i + (L - 1) * stride[mu] : i - stride[mu];
-                const float* pa = gb + site_slot(ip, L, Nh) * SITE_FLOATS;
-                const float* pc = gb + site_slot(im, L, Nh) * SITE_FLOATS;
+                const float* pa = gb + (size_t)nb[1 + 2 * mu] * SITE_FLOATS;   // s_{x+e_mu}
+                const float* pc = gb + (size_t)nb[2 + 2 * mu] * SITE_FLOATS;   // s_{x-e_mu}
                 const float ax = pa[0], ay = pa[G], az = pa[2 * G];
                 const float cx = pc[0], cy = pc[G], cz = pc[2 * G];
                 // a . (b x c)
@@ -460,15 +476,19 @@ __global__ void k_measure_chiral(const ChiralParams p)
                 sm[m * row + mu * p.Cp + grp * G + lane] = z;
             }
         }
+        if (threadIdx.x < ms * 3) {
+            const int m = threadIdx.x / 3, nu = threadIdx.x % 3, i = i0 + m;
+            const int xn = (nu == 0) ? i % L : ((nu == 1) ? (i / L) % L : i / (L * L));
+            phs[m * 6 + 2 * nu] = p.phase[2 * xn];
+            phs[m * 6 + 2 * nu + 1] = p.phase[2 * xn + 1];
+        }
         __syncthreads();
         if (live) {
             for (int m = 0; m < ms; ++m) {
                 const float* z = sm + m * row;
-                const int i = i0 + m;
-                const int x[3] = { i % L, (i / L) % L, i / (L * L) };
                 double ph[3][2];
 #pragma unroll
-                for (int nu = 0; nu < 3; ++nu) { ph[nu][0] = p.phase[2 * x[nu]]; ph[nu][1] = p.phase[2 * x[nu] + 1]; }
+                for (int nu = 0; nu < 3; ++nu) { ph[nu][0] = phs[m * 6 + 2 * nu]; ph[nu][1] = phs[m * 6 + 2 * nu + 1]; }
 #pragma unroll
                 for (int mu = 0; mu < 3; ++mu) {
                     const double kap = (double)(z[mu * p.Cp + ca] * z[mu * p.Cp + cb]);
