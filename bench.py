@@ -177,7 +177,7 @@ def run_ours(args, cfg):
 
     S, R, T, L, N, C = cfg.n_samples, cfg.n_replicas, cfg.n_temps, cfg.L, cfg.n_sites, cfg.n_copies
     gpu = sg.SpinGlass(L, S, R, T, cfg.betas, seed=cfg.seed, first_sample=multi.first_sample_of_rank(rank, S))
-    gpu.tune(sg.TUNE_SWEEP_IMPL, {"auto": sg.SWEEP_AUTO, "tiled": sg.SWEEP_TILED, "zmarch": sg.SWEEP_ZMARCH}[args.sweep_impl])
+    gpu.tune(sg.TUNE_SWEEP_IMPL, {"auto": sg.SWEEP_AUTO, "tiled": sg.SWEEP_TILED, "zmarch": sg.SWEEP_ZMARCH, "resident": sg.SWEEP_RESIDENT}[args.sweep_impl])
     if args.zchunk:
         gpu.tune(sg.TUNE_ZCHUNK, args.zchunk)
     for s in range(S):
@@ -313,7 +313,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (default: the headline cfg 4)")
-    ap.add_argument("--sweep-impl", default="auto", choices=["auto", "tiled", "zmarch"],
+    ap.add_argument("--sweep-impl", default="auto", choices=["auto", "tiled", "zmarch", "resident"],
                     help="sg_tune(SG_TUNE_SWEEP_IMPL): which half-sweep kernel serves the sweeps (default: the library's choice)")
     ap.add_argument("--zchunk", type=int, default=0, help="sg_tune(SG_TUNE_ZCHUNK): planes per CTA of the z-marching kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (profiling runs)")

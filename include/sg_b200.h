@@ -150,12 +150,19 @@ int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts);
 
 /* ---- tuning (results do not depend on it beyond floating-point summation order) ----
  * SG_TUNE_SWEEP_IMPL: which half-sweep kernel serves sg_sweep_or / sg_sweep_hb / the energy pass.
- *   SG_SWEEP_AUTO   z-marching kernel when L is a multiple of 8, else the tiled kernel (default)
- *   SG_SWEEP_TILED  the tiled kernel (any even L)
- *   SG_SWEEP_ZMARCH the z-marching kernel; SG_EINVAL unless L is a multiple of 8
- * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else even, >= 4 and a divisor of L. */
-enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1 };
-enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2 };
+ *   SG_SWEEP_AUTO     the resident kernel when the lattice of 8 copies fits in shared memory (N * 96 B <= 200 KB: L <= 12), else the
+ *                     z-marching kernel when L is a multiple of 8, else the tiled kernel (default)
+ *   SG_SWEEP_TILED    the tiled kernel (any even L)
+ *   SG_SWEEP_ZMARCH   the z-marching kernel; SG_EINVAL unless L is a multiple of 8
+ *   SG_SWEEP_RESIDENT all n sweeps of an sg_sweep_or / sg_sweep_hb call in ONE launch, the lattice of a (sample, group of
+ *                     32 copies) held in shared memory; SG_EINVAL unless the lattice of 4 copies fits (N * 48 B <= 200 KB).
+ *                     sg_halfsweep and the stand-alone energy pass keep using the z-marching / tiled kernel.
+ * All kernels perform the same arithmetic in the same order: the spins do not depend on the choice.
+ * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else even, >= 4 and a divisor of L.
+ * SG_TUNE_RES_COPIES: copies per CTA of the resident kernel: 0 = automatic, else 4, 8, 16 or 32 (SG_EINVAL if the lattice
+ *   of that many copies does not fit in shared memory). */
+enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2 };
+enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2, SG_SWEEP_RESIDENT = 3 };
 int sg_tune(sg_ctx* ctx, int knob, int value);
 
 /* ---- utilities ---- */

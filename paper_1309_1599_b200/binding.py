@@ -12,8 +12,8 @@ _LIB_PATH = os.path.join(_HERE, "libsg_b200.so")
 GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2, 3, 4
 KIND_OR, KIND_HB = 0, 1
 SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
-TUNE_SWEEP_IMPL, TUNE_ZCHUNK = 0, 1
-SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH = 0, 1, 2
+TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES = 0, 1, 2
+SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT = 0, 1, 2, 3
 
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "sg_kernels.cuh"
+#include "sg_sweep_res.cuh"
 
 using namespace sg;
 
@@ -25,7 +26,9 @@ struct sg_ctx {
     // sweep geometry
     int tile_sites, ntiles, log2L;
     // z-marching sweep (L a multiple of 8): tuning knobs and the derived chunking
-    int sweep_impl;   // SG_SWEEP_AUTO / SG_SWEEP_TILED / SG_SWEEP_ZMARCH
+    int sweep_impl;   // SG_SWEEP_AUTO / SG_SWEEP_TILED / SG_SWEEP_ZMARCH / SG_SWEEP_RESIDENT
+    int res_ok, res_auto;   // the lattice of 4 (explicit request) / 8 (automatic choice) copies fits in shared memory
+    int res_cpc, res_cpc_req;   // copies per CTA of the resident kernel (4, 8, 16, 32); requested, 0 = automatic
     int zm_zc_req;    // requested planes per chunk, 0 = automatic
     int zm_ok, zm_ZC, zm_nzc;
     // measure geometry
@@ -326,10 +329,79 @@ int fill_beta_slot(sg_ctx* ctx)
     return SG_OK;
 }
 
+// ---- shared-memory-resident multi-sweep kernel (sg_sweep_res.cuh): n sweeps of one kind in ONE launch ----
+constexpr size_t RES_SMEM_MAX = 200 * 1024;   // + 8.4 KB static reduction scratch <= 227 KB per CTA
+
+template <int KIND, int CPC>
+int launch_res_c(sg_ctx* ctx, const ResParams& p)
+{
+    const size_t smem = res_smem_bytes(ctx->N, CPC);
+    const dim3 grid(ctx->NG * (G / CPC), ctx->S);
+#define SG_RES_CASE(LG)                                                                                              \
+    {                                                                                                                \
+        auto kern = k_sweep_res<KIND, LG, CPC>;                                                                      \
+        SG_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES_SMEM_MAX));    \
+        kern<<<grid, RES_THREADS, smem, ctx->stream>>>(p);                                                           \
+    }
+    switch (ctx->log2L) {
+    case 1: SG_RES_CASE(1) break;
+    case 2: SG_RES_CASE(2) break;
+    case 3: SG_RES_CASE(3) break;
+    default: SG_RES_CASE(0) break;
+    }
+#undef SG_RES_CASE
+    return SG_OK;
+}
+
+template <int KIND>
+int launch_res(sg_ctx* ctx, const ResParams& p)
+{
+    switch (ctx->res_cpc) {
+    case 4: return launch_res_c<KIND, 4>(ctx, p);
+    case 8: return launch_res_c<KIND, 8>(ctx, p);
+    case 16: return launch_res_c<KIND, 16>(ctx, p);
+    default: return launch_res_c<KIND, 32>(ctx, p);
+    }
+}
+
+// copies per CTA of the resident kernel: 8 (full 32-byte sectors, several CTAs per SM), 4 when even that leaves most
+// SMs idle; a request through sg_tune(SG_TUNE_RES_COPIES) wins if its lattice fits
+void res_plan(sg_ctx* ctx)
+{
+    ctx->res_ok = (res_smem_bytes(ctx->N, 4) <= RES_SMEM_MAX) ? 1 : 0;     // an explicit request is honoured down to 4 copies
+    ctx->res_auto = (res_smem_bytes(ctx->N, 8) <= RES_SMEM_MAX) ? 1 : 0;   // automatic choice: full 32-byte sectors only
+    int cpc = ctx->res_cpc_req;
+    if (cpc == 0) cpc = ((long)ctx->S * ctx->NG * (G / 8) < 148) ? 4 : 8;
+    while (cpc > 4 && res_smem_bytes(ctx->N, cpc) > RES_SMEM_MAX) cpc /= 2;
+    ctx->res_cpc = cpc;
+}
+
+bool use_resident(const sg_ctx* ctx)
+{
+    return (ctx->res_auto && ctx->sweep_impl == SG_SWEEP_AUTO) || (ctx->res_ok && ctx->sweep_impl == SG_SWEEP_RESIDENT);
+}
+
+int sweeps_resident(sg_ctx* ctx, int kind, int n_sweeps)
+{
+    ResParams p;
+    p.spins = ctx->spins; p.Jg = ctx->Jg; p.beta_slot = ctx->beta_slot; p.E = ctx->E;
+    p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.C = ctx->C; p.Cp = ctx->Cp;
+    p.n_sweeps = n_sweeps;
+    p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
+    p.hb_counter = (uint32_t)ctx->hb_counter;
+    p.g_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->C;
+    if (int rc = (kind == KIND_HB) ? launch_res<1>(ctx, p) : launch_res<0>(ctx, p)) return rc;
+    SG_LAUNCHED(ctx);
+    if (kind == KIND_HB) ctx->hb_counter += (uint64_t)n_sweeps;
+    ctx->energies_fresh = true;
+    return SG_OK;
+}
+
 int sweeps(sg_ctx* ctx, int kind, int n_sweeps)
 {
     if (!ctx || n_sweeps < 0) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
+    if (n_sweeps > 0 && use_resident(ctx)) return sweeps_resident(ctx, kind, n_sweeps);
     for (int k = 0; k < n_sweeps; ++k) {
         if (int rc = half_sweep(ctx, kind, 0, false)) return rc;
         if (int rc = half_sweep(ctx, kind, 1, k == n_sweeps - 1)) return rc;
@@ -387,6 +459,8 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->inited.assign(g.S, 0);
     ctx->hb_counter = ctx->pt_counter = ctx->launches = 0;
     ctx->sweep_impl = SG_SWEEP_AUTO; ctx->zm_zc_req = 0;
+    ctx->res_cpc_req = 0;
+    res_plan(ctx);
     zm_plan(ctx);
     ctx->energies_fresh = false;
     ctx->last_cuda = 0;
@@ -701,9 +775,16 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
     if (!ctx) return SG_EINVAL;
     switch (knob) {
     case SG_TUNE_SWEEP_IMPL:
-        if (value != SG_SWEEP_AUTO && value != SG_SWEEP_TILED && value != SG_SWEEP_ZMARCH) return SG_EINVAL;
+        if (value != SG_SWEEP_AUTO && value != SG_SWEEP_TILED && value != SG_SWEEP_ZMARCH && value != SG_SWEEP_RESIDENT) return SG_EINVAL;
         if (value == SG_SWEEP_ZMARCH && ctx->L % 8 != 0) return SG_EINVAL;
+        if (value == SG_SWEEP_RESIDENT && !ctx->res_ok) return SG_EINVAL;
         ctx->sweep_impl = value;
+        return SG_OK;
+    case SG_TUNE_RES_COPIES:
+        if (value != 0 && value != 4 && value != 8 && value != 16 && value != 32) return SG_EINVAL;
+        if (value > 0 && res_smem_bytes(ctx->N, value) > RES_SMEM_MAX) return SG_EINVAL;
+        ctx->res_cpc_req = value;
+        res_plan(ctx);
         return SG_OK;
     case SG_TUNE_ZCHUNK:
         if (value < 0) return SG_EINVAL;

@@ -355,8 +355,8 @@ __global__ void k_measure(const MeasureParams p)
             float* dst = sm + m * row + grp * G + lane;
             dst[0] = src[0]; dst[p.Cp] = src[G]; dst[2 * p.Cp] = src[2 * G];
         }
-        if (threadIdx.x < ms * 3) {                 // e^{i 2 pi x_mu / L} of the batch's sites, once per batch
-            const int m = threadIdx.x / 3, mu = threadIdx.x % 3, i = i0 + m;
+        for (int u = threadIdx.x; u < ms * 3; u += blockDim.x) {   // e^{i 2 pi x_mu / L} of the batch's sites, once per batch
+            const int m = u / 3, mu = u % 3, i = i0 + m;
             const int xm = (mu == 0) ? i % p.L : ((mu == 1) ? (i / p.L) % p.L : i / (p.L * p.L));
             ph[m * 6 + 2 * mu] = p.phase[2 * xm];
             ph[m * 6 + 2 * mu + 1] = p.phase[2 * xm + 1];
@@ -446,8 +446,8 @@ __global__ void k_measure_chiral(const ChiralParams p)
         const int ms = min(p.MS, i_end - i0);
         __syncthreads();
         // positions (own, x1+-1, x2+-1, x3+-1) of the batch's sites in the colour-split order, once per batch
-        if (threadIdx.x < ms * 7) {
-            const int m = threadIdx.x / 7, k = threadIdx.x % 7, i = i0 + m;
+        for (int u = threadIdx.x; u < ms * 7; u += blockDim.x) {
+            const int m = u / 7, k = u % 7, i = i0 + m;
             int j = i;
             if (k > 0) {
                 const int mu = (k - 1) >> 1, up = (k - 1) & 1 ? 0 : 1;
@@ -476,8 +476,8 @@ __global__ void k_measure_chiral(const ChiralParams p)
                 sm[m * row + mu * p.Cp + grp * G + lane] = z;
             }
         }
-        if (threadIdx.x < ms * 3) {
-            const int m = threadIdx.x / 3, nu = threadIdx.x % 3, i = i0 + m;
+        for (int u = threadIdx.x; u < ms * 3; u += blockDim.x) {
+            const int m = u / 3, nu = u % 3, i = i0 + m;
             const int xn = (nu == 0) ? i % L : ((nu == 1) ? (i / L) % L : i / (L * L));
             phs[m * 6 + 2 * nu] = p.phase[2 * xn];
             phs[m * 6 + 2 * nu + 1] = p.phase[2 * xn + 1];

@@ -1,0 +1,144 @@
+// sg_sweep_res.cuh -- the shared-memory-resident multi-sweep kernel of libsg_b200 for small lattices
+// (multi-sweep fusion where the state fits on chip).
+//
+// Why.  For L <= 8 a half-sweep is a few thousand site updates per copy group: one launch per half-sweep is
+// pure launch and pipeline latency (cfg 1: 16 CTAs per launch, 15 us each, 0.05 of the HBM roofline).  Copies
+// are independent between parallel-tempering swaps, so a CTA can keep the WHOLE lattice of one
+// (sample, group of 32 copies) in shared memory -- N sites x 384 bytes: 24 KB at L = 4, 192 KB at L = 8 -- and
+// run all n sweeps of an sg_sweep_or / sg_sweep_hb call in one launch: spins cross HBM once per call instead of
+// once per half-sweep, and the per-copy energies come out of the last half-sweep with no second kernel.
+// The couplings (224 bytes per site, shared by the 32 copies) are read through L1/L2 every half-sweep.
+//
+// Same arithmetic, in the same order, as k_sweep / k_sweep_zm (field: neighbours +x1,-x1,+x2,-x2,+x3,-x3, rows,
+// columns), so the spins after a call are bit-identical to the other two kernels'; only the energy summation
+// order differs.  Thread = (site slot, quad of copies).  A CTA takes CPC = 32, 16, 8 or 4 consecutive copies of a
+// group (CPC/4 quads x 1024/CPC site slots): small problems are spread over more SMs by giving each CTA fewer
+// copies (cfg 1 has only 16 (sample, group) pairs for 148 SMs); CPC >= 8 keeps every global access a full 32-byte sector.
+#pragma once
+#include "sg_device.cuh"
+
+namespace sg {
+
+struct ResParams {
+    float* spins;            // [S][NG][2][Nh][3][G]
+    const float* Jg;         // [S][2][Nh][JG]
+    const float* beta_slot;  // [S][Cp]
+    double* E;               // [S][Cp]: total H of every slot, written by the last half-sweep
+    int L, N, Nh, NG, C, Cp;
+    int n_sweeps;
+    uint32_t key0, key1, hb_counter, g_first;
+};
+
+constexpr int RES_THREADS = 256;
+
+inline size_t res_smem_bytes(int N, int cpc) { return (size_t)N * 3 * cpc * sizeof(float); }
+
+template <int KIND_, int LOG2L, int CPC>
+__global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
+{
+    constexpr int QUADS = CPC / 4, RES_SLOTS = RES_THREADS / QUADS, SUBS = G / CPC, SITE = 3 * CPC;
+    extern __shared__ __align__(16) float lat[];      // [2][Nh][3][CPC]: the lattice of this CTA's copies
+    __shared__ double red[RES_SLOTS * (CPC + 1)];
+    const int tid = threadIdx.x, q = tid % QUADS, slot = tid / QUADS;
+    const int grp = blockIdx.x / SUBS, sub = blockIdx.x % SUBS, sample = blockIdx.y;
+    const int c_first = grp * G + sub * CPC;          // first copy of this CTA inside the sample
+    if (c_first >= p.C) return;                       // padding copies only
+    const int L = p.L;
+    float* const gl = p.spins + ((size_t)(sample * p.NG + grp) * p.N) * SITE_FLOATS + sub * CPC;
+    for (int e = tid; e < p.N * 3 * QUADS; e += RES_THREADS) {
+        const int qq = e % QUADS, line = e / QUADS;   // line = site * 3 + component
+        st4(lat + line * CPC + qq * 4, ld4(gl + (size_t)line * G + qq * 4));
+    }
+    __syncthreads();
+
+    float* const sp = lat + q * 4;
+    float4 beta4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (KIND_ == 1) beta4 = ldg4(p.beta_slot + (size_t)sample * p.Cp + c_first + q * 4);
+    const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.C + (uint32_t)(c_first + q * 4);
+    float eacc[4] = { 0.f, 0.f, 0.f, 0.f };
+
+    for (int sw = 0; sw < p.n_sweeps; ++sw) {
+        for (int colour = 0; colour < 2; ++colour) {
+            const bool last = (sw == p.n_sweeps - 1) && (colour == 1);
+            const float* const Jc = p.Jg + ((size_t)(sample * 2 + colour) * p.Nh) * JG;
+            for (int h = slot; h < p.Nh; h += RES_SLOTS) {
+                int x, y, z;
+                site_of<LOG2L>(h, colour, L, x, y, z);
+                const int xp = (x + 1 == L) ? 0 : x + 1, xm = (x == 0) ? L - 1 : x - 1;
+                const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+                const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+                const int row = L * (y + L * z);
+                const int i = x + row;
+                const int nb[6] = { xp + row, xm + row, x + L * (yp + L * z), x + L * (ym + L * z),
+                                    x + L * (y + L * zp), x + L * (y + L * zm) };
+                float J[JG];
+                const float* jp = Jc + (size_t)h * JG;
+#pragma unroll
+                for (int v = 0; v < JG / 4; ++v) {
+                    const float4 t4 = ldg4(jp + 4 * v);
+                    J[4 * v] = t4.x; J[4 * v + 1] = t4.y; J[4 * v + 2] = t4.z; J[4 * v + 3] = t4.w;
+                }
+                float* const own = sp + (colour * p.Nh + h) * SITE;
+                float s[3][4], hf[3][4];
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const float4 t4 = ld4(own + a * CPC);
+                    s[a][0] = t4.x; s[a][1] = t4.y; s[a][2] = t4.z; s[a][3] = t4.w;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) hf[a][j] = 0.f;
+                }
+#pragma unroll
+                for (int k = 0; k < 6; ++k) {
+                    const float* np_ = sp + ((1 - colour) * p.Nh + (nb[k] >> 1)) * SITE;
+                    float n[3][4];
+#pragma unroll
+                    for (int b = 0; b < 3; ++b) {
+                        const float4 t4 = ld4(np_ + b * CPC);
+                        n[b][0] = t4.x; n[b][1] = t4.y; n[b][2] = t4.z; n[b][3] = t4.w;
+                    }
+#pragma unroll
+                    for (int a = 0; a < 3; ++a)
+#pragma unroll
+                        for (int b = 0; b < 3; ++b)
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * k + 3 * a + b], n[b][j], hf[a][j]);
+                }
+                if (KIND_ == 0) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        if (last) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
+                        or_update(hf[0][j], hf[1][j], hf[2][j], s[0][j], s[1][j], s[2][j]);
+                    }
+                } else {
+                    const float bt[4] = { beta4.x, beta4.y, beta4.z, beta4.w };
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        uint32_t w[4];
+                        philox4x32_10((uint32_t)i, g0 + j, p.hb_counter + (uint32_t)sw, STREAM_HB, p.key0, p.key1, w);
+                        hb_update(hf[0][j], hf[1][j], hf[2][j], bt[j], uniform23(w[0]), uniform23(w[1]), s[0][j], s[1][j], s[2][j]);
+                        if (last) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
+                    }
+                }
+#pragma unroll
+                for (int a = 0; a < 3; ++a) st4(own + a * CPC, make_float4(s[a][0], s[a][1], s[a][2], s[a][3]));
+            }
+            __syncthreads();      // the other colour reads what this colour wrote
+        }
+    }
+
+    for (int e = tid; e < p.N * 3 * QUADS; e += RES_THREADS) {
+        const int qq = e % QUADS, line = e / QUADS;
+        st4(gl + (size_t)line * G + qq * 4, ld4(lat + line * CPC + qq * 4));
+    }
+    // E = - sum over the colour-1 sites of s.h (every link joins the two colours): fixed order, fp64 across threads
+#pragma unroll
+    for (int j = 0; j < 4; ++j) red[slot * (CPC + 1) + q * 4 + j] = (double)eacc[j];
+    __syncthreads();
+    if (tid < CPC) {
+        double acc = 0.0;
+        for (int r = 0; r < RES_SLOTS; ++r) acc += red[r * (CPC + 1) + tid];
+        p.E[(size_t)sample * p.Cp + c_first + tid] = -acc;
+    }
+}
+
+}  // namespace sg

@@ -40,6 +40,12 @@ SHAPES = [
     dict(L=16, S=2, R=2, T=17, b=(0.5, 2.2), tune=((0, 2), (1, 4))),
     dict(L=16, S=1, R=2, T=17, b=(0.5, 2.2), tune=((0, 2), (1, 16))),
     dict(L=24, S=1, R=2, T=5, b=(0.5, 2.2), tune=((0, 2), (1, 6))),
+    # L <= 8 defaults to the shared-memory-resident multi-sweep kernel for the sweep calls: keep the tiled and the
+    # z-marching kernels covered there too, and name the resident kernel explicitly once
+    dict(L=4, S=1, R=2, T=4, b=(0.6, 1.6), tune=((0, 1),)),
+    dict(L=6, S=2, R=4, T=10, b=(0.5, 2.0), tune=((0, 1),)),
+    dict(L=8, S=3, R=4, T=16, b=(0.5, 2.0), tune=((0, 2),)),
+    dict(L=8, S=3, R=4, T=16, b=(0.5, 2.0), tune=((0, 3),)),
 ]
 
 
@@ -378,4 +384,55 @@ def test_errors_on_gpu(sg):
     gpu.init_sample(1)
     n0 = gpu.kernel_launches()
     gpu.sweep_or(2)
-    assert gpu.kernel_launches() == n0 + 5       # 4 half-sweeps + 1 energy reduction
+    assert gpu.kernel_launches() == n0 + 1       # L = 4: the resident kernel runs both sweeps and the energies in one launch
+    gpu.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_TILED)
+    gpu.sweep_or(2)
+    assert gpu.kernel_launches() == n0 + 6       # 4 half-sweeps + 1 energy reduction
+    with pytest.raises(sg.SgError):
+        sg.SpinGlass(32, 1, 2, 4, np.linspace(0.6, 1.6, 4)).tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_RESIDENT)   # 1.5 MB for 4 copies
+
+
+@pytest.mark.parametrize("L,S,R,T", [(2, 2, 2, 3), (4, 1, 2, 4), (6, 2, 4, 10), (8, 3, 4, 16), (8, 8, 4, 16), (10, 1, 3, 11), (16, 1, 2, 20)])
+def test_resident_kernel_is_bit_identical_to_the_per_half_sweep_kernels(sg, L, S, R, T):
+    """Same seeded start, one unit sequence (2 HB sweeps, 5 OR sweeps) through the resident multi-sweep kernel and
+    through the tiled kernel (and the z-marching kernel for L = 8): the spins must agree bit for bit (same arithmetic,
+    same order), the fused energies to summation-order rounding, the HB counter must advance alike."""
+    betas = np.linspace(0.5, 2.0, T)
+    # (kernel, copies per CTA of the resident kernel): every CTA shape of the resident kernel against the other two
+    impls = [(sg.SWEEP_TILED, 0), (sg.SWEEP_RESIDENT, 0)] + ([(sg.SWEEP_ZMARCH, 0)] if L % 8 == 0 else []) + \
+            [(sg.SWEEP_RESIDENT, c) for c in (4, 8, 16, 32) if L ** 3 * 12 * c <= 200 * 1024]
+    out = []
+    for impl, cpc in impls:
+        gpu = sg.SpinGlass(L, S, R, T, betas, seed=11)
+        gpu.tune(sg.TUNE_SWEEP_IMPL, impl)
+        if cpc:
+            gpu.tune(sg.TUNE_RES_COPIES, cpc)
+        for s in range(S):
+            gpu.init_sample(s, sg.GEN_GENERAL9, 1.0)
+        gpu.sweep_hb(2); gpu.sweep_or(5)
+        E = gpu.get_energies()
+        gpu.pt_swap(); gpu.sweep_hb(1); gpu.sweep_or(1)          # beta follows the permutation in the next call
+        out.append((np.stack([gpu.get_spins(s) for s in range(S)]), E, gpu.get_counters(), gpu.get_energies()))
+        gpu.close()
+    for spins, E, ctr, E2 in out[1:]:
+        assert ctr == out[0][2]
+        assert np.abs(E - out[0][1]).max() <= 1e-6 * max(1.0, np.abs(E).max())
+        # identical energies up to rounding may still flip a PT decision at a near-tie; compare the pre-PT part strictly
+        if np.array_equal(spins, out[0][0]):
+            assert np.abs(E2 - out[0][3]).max() <= 1e-6 * max(1.0, np.abs(E2).max())
+    # the strict part: state before the PT step
+    ref = None
+    for impl, cpc in impls:
+        gpu = sg.SpinGlass(L, S, R, T, betas, seed=11)
+        gpu.tune(sg.TUNE_SWEEP_IMPL, impl)
+        if cpc:
+            gpu.tune(sg.TUNE_RES_COPIES, cpc)
+        for s in range(S):
+            gpu.init_sample(s, sg.GEN_GENERAL9, 1.0)
+        gpu.sweep_hb(2); gpu.sweep_or(5)
+        spins = np.stack([gpu.get_spins(s) for s in range(S)])
+        gpu.close()
+        if ref is None:
+            ref = spins
+        else:
+            assert np.array_equal(spins, ref), (impl, cpc)
