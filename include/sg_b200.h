@@ -101,6 +101,11 @@ int sg_sweep_hb(sg_ctx* ctx, int n_sweeps);
  * are recomputed first if stale.  The PT counter advances by one. */
 int sg_pt_swap(sg_ctx* ctx);
 
+/* n_units Monte Carlo steps (MCS, Sect. III, App. A.1): each is sg_sweep_hb(ctx, 1);
+ * sg_sweep_or(ctx, n_or); sg_pt_swap(ctx), issued from native code so that small lattices are not bound by the
+ * caller's per-call overhead.  Asynchronous on the stream; identical results to the three calls made one by one. */
+int sg_run_units(sg_ctx* ctx, int n_units, int n_or);
+
 /* S3 + S5.  Host outputs (any may be NULL):
  *   e  double [S][R][T]        H/N of the copy of replica r at temperature t
  *   q0 double [S][P][T]        q^(0)   = sum_x s^a_x.s^b_x / N, both copies at temperature t

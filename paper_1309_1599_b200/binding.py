@@ -18,7 +18,7 @@ SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT = 0, 1, 2, 3
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_sweep_or", "sg_sweep_hb",
-    "sg_pt_swap", "sg_measure", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
+    "sg_pt_swap", "sg_run_units", "sg_measure", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
     "sg_halfsweep", "sg_pt_stats", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
@@ -60,6 +60,7 @@ def load_library():
     L.sg_sweep_hb.argtypes = [vp, i]; L.sg_sweep_hb.restype = i
     L.sg_pt_swap.argtypes = [vp]; L.sg_pt_swap.restype = i
     L.sg_measure.argtypes = [vp, vp, vp, vp]; L.sg_measure.restype = i
+    L.sg_run_units.argtypes = [vp, i, i]; L.sg_run_units.restype = i
     L.sg_measure_chiral.argtypes = [vp, vp, vp]; L.sg_measure_chiral.restype = i
     L.sg_schwinger_dyson.argtypes = [vp, vp]; L.sg_schwinger_dyson.restype = i
     L.sg_correlation_length.argtypes = [i, ctypes.c_double, ctypes.c_double]; L.sg_correlation_length.restype = ctypes.c_double
@@ -179,6 +180,10 @@ class SpinGlass:
         qk = np.empty((self.S, self.P, self.T, 3, 2))
         self._check(self._lib.sg_measure(self._ctx, _ptr(e), _ptr(q0), _ptr(qk)), "sg_measure")
         return e, q0, qk
+
+    def run_units(self, n_units, n_or):
+        """n_units MCS (1 HB + n_or OR + PT each) issued from native code."""
+        self._check(self._lib.sg_run_units(self._ctx, int(n_units), int(n_or)), "sg_run_units")
 
     def measure_chiral(self):
         """(qc0 [S][P][T][3], qck [S][P][T][3][3][2]): chiral-glass overlaps, Eq. (2) PAPER.md:81-85."""

@@ -603,6 +603,17 @@ int sg_pt_swap(sg_ctx* ctx)
     return SG_OK;
 }
 
+int sg_run_units(sg_ctx* ctx, int n_units, int n_or)
+{
+    if (!ctx || n_units < 0 || n_or < 0) return SG_EINVAL;
+    for (int u = 0; u < n_units; ++u) {
+        if (int rc = sg_sweep_hb(ctx, 1)) return rc;
+        if (int rc = sg_sweep_or(ctx, n_or)) return rc;
+        if (int rc = sg_pt_swap(ctx)) return rc;
+    }
+    return SG_OK;
+}
+
 int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
 {
     if (!ctx) return SG_EINVAL;

@@ -436,3 +436,20 @@ def test_resident_kernel_is_bit_identical_to_the_per_half_sweep_kernels(sg, L, S
             ref = spins
         else:
             assert np.array_equal(spins, ref), (impl, cpc)
+
+
+def test_run_units_equals_the_three_calls(sg):
+    """sg_run_units(n, n_or) = n x (sg_sweep_hb(1); sg_sweep_or(n_or); sg_pt_swap()), bit for bit."""
+    L, S, R, T = 6, 2, 2, 6
+    betas = np.linspace(0.5, 1.8, T)
+    a = sg.SpinGlass(L, S, R, T, betas, seed=4); b = sg.SpinGlass(L, S, R, T, betas, seed=4)
+    for g in (a, b):
+        for s in range(S):
+            g.init_sample(s)
+    for _ in range(7):
+        a.unit(3)
+    b.run_units(7, 3)
+    for s in range(S):
+        assert np.array_equal(a.get_spins(s), b.get_spins(s))
+        assert np.array_equal(a.get_perm(s)[0], b.get_perm(s)[0])
+    assert np.array_equal(a.get_energies(), b.get_energies()) and a.get_counters() == b.get_counters() == (7, 7)
