@@ -73,7 +73,7 @@ Geometry geometry(const sg_shape* s)
     g.tile_sites = 128;
     g.ntiles = (g.Nh + g.tile_sites - 1) / g.tile_sites;
     // measure chunks
-    g.nchunk = g.N / 512; if (g.nchunk < 1) g.nchunk = 1; if (g.nchunk > 256) g.nchunk = 256;
+    g.nchunk = g.N / 32; if (g.nchunk < 1) g.nchunk = 1; if (g.nchunk > 256) g.nchunk = 256;   // >= 2 batches of sites per CTA, enough CTAs for small lattices
     g.chunk_sites = (g.N + g.nchunk - 1) / g.nchunk;
     g.MS = 11500 / (3 * g.Cp); if (g.MS < 1) g.MS = 1; if (g.MS > 16) g.MS = 16;
     return g;
