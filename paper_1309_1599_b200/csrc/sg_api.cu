@@ -21,6 +21,8 @@ struct sg_ctx {
     // device arrays (carved from the caller's workspace)
     float* spins; float* Jg; float* Jt; float* Mraw; float* staging; float* beta_slot;
     double* betas; double* E; double* Epart; double* SDpart; double* phase; double* Mpart; double* result;
+    double* h_result = nullptr;   // pinned host mirror of `result`: one device-to-host copy per measurement call
+    size_t result_doubles = 0;
     int* slot_of_temp; int* temp_of_slot;
     unsigned long long* attempts; unsigned long long* accepts;
     // sweep geometry
@@ -307,6 +309,18 @@ int half_sweep(sg_ctx* ctx, int kind, int colour, bool with_energy)
     return SG_OK;
 }
 
+// n doubles of ctx->result to the host and a stream synchronisation; returns where they are (pinned mirror), or
+// nullptr with *rc set on failure / when no mirror exists (the caller then copies piecewise)
+const double* fetch_result(sg_ctx* ctx, size_t n, int* rc)
+{
+    *rc = SG_OK;
+    if (!ctx->h_result || n > ctx->result_doubles) return nullptr;
+    cudaError_t e = cudaMemcpyAsync(ctx->h_result, ctx->result, n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { *rc = cuda_fail(ctx, e); return nullptr; }
+    return ctx->h_result;
+}
+
 int all_inited(const sg_ctx* ctx)
 {
     for (char c : ctx->inited)
@@ -453,6 +467,11 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->SDpart = (double*)(base + o.SDpart);
     ctx->phase = (double*)(base + o.phase); ctx->Mpart = (double*)(base + o.Mpart);
     ctx->result = (double*)(base + o.result);
+    ctx->result_doubles = (size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + 1;
+    if (cudaHostAlloc((void**)&ctx->h_result, ctx->result_doubles * sizeof(double), cudaHostAllocDefault) != cudaSuccess) {
+        ctx->h_result = nullptr;   // fall back to direct copies into the caller's arrays
+        cudaGetLastError();
+    }
     ctx->slot_of_temp = (int*)(base + o.sot); ctx->temp_of_slot = (int*)(base + o.tos);
     ctx->attempts = (unsigned long long*)(base + o.att); ctx->accepts = (unsigned long long*)(base + o.acc);
     ctx->h_betas.assign(betas, betas + g.T);
@@ -493,6 +512,7 @@ int sg_destroy(sg_ctx* ctx)
 {
     if (!ctx) return SG_EINVAL;
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->h_result) cudaFreeHost(ctx->h_result);
     delete ctx;
     return SG_OK;
 }
@@ -638,6 +658,16 @@ int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
     k_reduce_measure<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->Mpart, ctx->E, ctx->slot_of_temp, ctx->result, ctx->S,
                                                                  ctx->R, ctx->T, ctx->P, ctx->Cp, ctx->nchunk, ctx->N);
     SG_LAUNCHED(ctx);
+    {
+        int rc;
+        if (const double* h = fetch_result(ctx, (size_t)nE + (size_t)nQ * 7, &rc)) {
+            if (e) std::memcpy(e, h, (size_t)nE * sizeof(double));
+            if (q0 && nQ) std::memcpy(q0, h + nE, (size_t)nQ * sizeof(double));
+            if (qk && nQ) std::memcpy(qk, h + nE + nQ, (size_t)nQ * 6 * sizeof(double));
+            return SG_OK;
+        }
+        if (rc != SG_OK) return rc;
+    }
     if (e) SG_CUDA(ctx, cudaMemcpyAsync(e, ctx->result, (size_t)nE * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (q0 && nQ) SG_CUDA(ctx, cudaMemcpyAsync(q0, ctx->result + nE, (size_t)nQ * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (qk && nQ) SG_CUDA(ctx, cudaMemcpyAsync(qk, ctx->result + nE + nQ, (size_t)nQ * 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
@@ -666,6 +696,15 @@ int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck)
     SG_LAUNCHED(ctx);
     k_reduce_chiral<<<(nQ * 21 + 127) / 128, 128, 0, ctx->stream>>>(ctx->Mpart, ctx->result, ctx->S, PT, ctx->nchunk, ctx->N);
     SG_LAUNCHED(ctx);
+    {
+        int rc;
+        if (const double* h = fetch_result(ctx, (size_t)nQ * 21, &rc)) {
+            if (qc0) std::memcpy(qc0, h, (size_t)nQ * 3 * sizeof(double));
+            if (qck) std::memcpy(qck, h + (size_t)nQ * 3, (size_t)nQ * 18 * sizeof(double));
+            return SG_OK;
+        }
+        if (rc != SG_OK) return rc;
+    }
     if (qc0) SG_CUDA(ctx, cudaMemcpyAsync(qc0, ctx->result, (size_t)nQ * 3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (qck) SG_CUDA(ctx, cudaMemcpyAsync(qck, ctx->result + (size_t)nQ * 3, (size_t)nQ * 18 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -685,6 +724,11 @@ int sg_schwinger_dyson(sg_ctx* ctx, double* sd)
     k_reduce_sd<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->SDpart, ctx->slot_of_temp, ctx->result, ctx->S, ctx->R, ctx->T,
                                                               ctx->NG, ctx->ntiles, ctx->N);
     SG_LAUNCHED(ctx);
+    {
+        int rc;
+        if (const double* h = fetch_result(ctx, (size_t)total, &rc)) { std::memcpy(sd, h, (size_t)total * sizeof(double)); return SG_OK; }
+        if (rc != SG_OK) return rc;
+    }
     SG_CUDA(ctx, cudaMemcpyAsync(sd, ctx->result, (size_t)total * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
