@@ -490,3 +490,26 @@ void sgo_sd_terms(int L, const double* M, const double* s, double out[2])
     out[0] /= (double)N;
     out[1] /= (double)N;
 }
+
+/* ------------------------------------------------------------------------------------------ */
+/* Random walk in temperature (Sect. III: "the random walk in temperatures of     */
+/* each sample"; "all the replicas stay a significant amount of time at each temperature").     */
+/* ------------------------------------------------------------------------------------------ */
+/* Bookkeeping after one PT sweep of one chain.  Every configuration (slot) carries a label: 0 = has not
+ * touched an end of the ladder yet, 1 = last touched temperature index 0, 2 = last touched index T-1.
+ * A ROUND TRIP of a configuration is index 0 -> index T-1 -> index 0; round_trips counts the completions,
+ * summed over the chain's T configurations.  visits[slot*T + t] (may be NULL) counts the sweeps after which
+ * the configuration in `slot` sat at temperature index t (the histogram of its walk). */
+void sgo_pt_walk_update(int T, const int* temp_of_slot, int* label, uint64_t* round_trips, uint64_t* visits)
+{
+    for (int slot = 0; slot < T; ++slot) {
+        int t = temp_of_slot[slot];
+        if (t == 0) {
+            if (label[slot] == 2) *round_trips += 1;
+            label[slot] = 1;
+        } else if (t == T - 1) {
+            if (label[slot] == 1) label[slot] = 2;        /* a trip starts at index 0 only: label 0 stays 0 */
+        }
+        if (visits) visits[(size_t)slot * T + t] += 1;
+    }
+}

@@ -67,6 +67,7 @@ def lib():
         L.sgo_chiral_overlap.argtypes = [i, dp, dp, dp]
         L.sgo_xi.argtypes = [i, d, d]; L.sgo_xi.restype = d
         L.sgo_sd_terms.argtypes = [i, dp, dp, dp]
+        L.sgo_pt_walk_update.argtypes = [i, ip, ip, u64p, u64p]
         _lib = L
     return _lib
 
@@ -217,6 +218,14 @@ def sd_terms(L, M, s):
     return out
 
 
+def pt_walk_update(temp_of_slot, label, round_trips, visits=None):
+    """Round-trip / histogram bookkeeping of one chain after a PT sweep; arrays updated in place:
+    temp_of_slot int32 [T], label int32 [T], round_trips uint64 [1], visits uint64 [T][T] or None."""
+    T = len(temp_of_slot)
+    lib().sgo_pt_walk_update(T, _ip(temp_of_slot), _ip(label), _u64p(round_trips),
+                             _u64p(visits) if visits is not None else None)
+
+
 def replica_pairs(R):
     """Pairs a<b in the order (0,1),(0,2),...,(R-2,R-1) (reading R15)."""
     return [(a, b) for a in range(R) for b in range(a + 1, R)]
@@ -249,6 +258,8 @@ class OracleSim:
         self.pt_counter = 0
         self.attempts = np.zeros((self.S, self.R, max(self.T - 1, 1)), dtype=np.uint64)
         self.accepts = np.zeros_like(self.attempts)
+        self.walk_label = np.zeros((self.S, self.R, self.T), dtype=np.int32)
+        self.round_trips = np.zeros((self.S, self.R, 1), dtype=np.uint64)
 
     def g0(self, sample):
         return (self.first_sample + sample) * self.C
@@ -307,6 +318,7 @@ class OracleSim:
                 pt_sweep(self.betas, E[s, r * self.T:(r + 1) * self.T], self.slot_of_temp[s, r],
                          self.temp_of_slot[s, r], self.seed, chain, self.pt_counter,
                          self.attempts[s, r], self.accepts[s, r])
+                pt_walk_update(self.temp_of_slot[s, r], self.walk_label[s, r], self.round_trips[s, r])
         self.pt_counter += 1
 
     def measure(self):

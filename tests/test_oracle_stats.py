@@ -282,3 +282,48 @@ def test_pt_never_moves_spins_and_counts(oracle):
             assert sorted(sim.slot_of_temp[s, r]) == list(range(4))
             assert np.array_equal(sim.temp_of_slot[s, r][sim.slot_of_temp[s, r]], np.arange(4))
     assert sim.accepts.sum() > 0
+
+
+# ---------------------------------------------------------------------------------------------
+# random walk in temperature: pins of oracle.pt_walk_update
+# ---------------------------------------------------------------------------------------------
+def test_pt_walk_round_trips_by_hand_and_brute_force(oracle):
+    """T = 2, every swap accepted: a configuration alternates 0, 1, 0, 1, ...; the one starting at index 1 touches
+    index 0 after sweep 1 (label 1), index 1 after sweep 2 (label 2) and completes its first round trip after sweep 3.
+    Then: an arbitrary recorded walk against a brute-force count of the pattern 0 ... T-1 ... 0 per configuration."""
+    tos = np.array([0, 1], dtype=np.int32); label = np.zeros(2, dtype=np.int32); trips = np.zeros(1, dtype=np.uint64)
+    seen = []
+    for sweep in range(1, 8):
+        tos = tos[::-1].copy()
+        oracle.pt_walk_update(tos, label, trips)
+        seen.append(int(trips[0]))
+    # slot 0: at index 1 after odd sweeps, 0 after even: touches 0 first at sweep 2 -> trips at sweeps 4, 6
+    # slot 1: at index 0 after odd sweeps: label 1 at sweep 1 -> trips at sweeps 3, 5, 7
+    assert seen == [0, 0, 1, 2, 3, 4, 5]
+    rng = np.random.default_rng(2)
+    T, n = 5, 4000
+    perm = np.arange(T, dtype=np.int32)
+    label = np.zeros(T, dtype=np.int32); trips = np.zeros(1, dtype=np.uint64); visits = np.zeros((T, T), dtype=np.uint64)
+    hist = []
+    for _ in range(n):
+        t = rng.integers(0, T - 1)
+        if rng.random() < 0.6:
+            a, b = np.where(perm == t)[0][0], np.where(perm == t + 1)[0][0]
+            perm[a], perm[b] = t + 1, t
+        oracle.pt_walk_update(perm, label, trips, visits)
+        hist.append(perm.copy())
+    hist = np.array(hist)                                         # [n][slot] -> temperature index
+    brute = 0
+    for slot in range(T):
+        ends = [t for t in hist[:, slot] if t in (0, T - 1)]
+        state = None
+        for t in ends:
+            if t == 0:
+                if state == "top":
+                    brute += 1
+                state = "bottom"
+            elif state == "bottom":
+                state = "top"
+    assert int(trips[0]) == brute and brute > 5
+    assert np.array_equal(visits, np.array([[np.sum(hist[:, s] == t) for t in range(T)] for s in range(T)], dtype=np.uint64))
+    assert visits.sum() == n * T
