@@ -152,6 +152,14 @@ int sg_set_counters(sg_ctx* ctx, uint64_t hb_counter, uint64_t pt_counter);
 int sg_halfsweep(sg_ctx* ctx, int kind, int colour);
 /* PT statistics since creation, uint64 [S][R][T-1] each (either may be NULL). */
 int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts);
+/* Random walk in temperature (Sect. III: "the random walk in temperatures
+ * of each sample"), kept by every sg_pt_swap since creation.  Each configuration (slot) of a chain (sample, replica)
+ * carries a label: 0 = has not touched an end of the ladder yet, 1 = last touched temperature index 0, 2 = last touched
+ * index T-1.  A round trip is index 0 -> index T-1 -> index 0.
+ *   round_trips uint64 [S][R]     completed round trips, summed over the chain's T configurations
+ *   label       int32  [S][R][T]  current label of every slot
+ * Host outputs, either may be NULL.  Integer work: bit-exact against the oracle.  Synchronises. */
+int sg_pt_walk(sg_ctx* ctx, uint64_t* round_trips, int32_t* label);
 
 /* ---- tuning (results do not depend on it beyond floating-point summation order) ----
  * SG_TUNE_SWEEP_IMPL: which half-sweep kernel serves sg_sweep_or / sg_sweep_hb / the energy pass.

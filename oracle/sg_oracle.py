@@ -226,6 +226,35 @@ def pt_walk_update(temp_of_slot, label, round_trips, visits=None):
                              _u64p(visits) if visits is not None else None)
 
 
+def logbin_index(n):
+    """Bin of the n-th measurement (n = 1, 2, ...) in the logarithmic binning of Sect. III: "each bin
+    had twice the length of the previous"; bin i holds the measurements 2^i <= n < 2^(i+1), so that after 2^k - 1
+    measurements the last bin k-1 is the last half of the series, bin k-2 the second quarter, and so on."""
+    assert n >= 1
+    i = 0
+    while (n >> (i + 1)) > 0:
+        i += 1
+    return i
+
+
+def logbin_observables(e, q0, qk):
+    """The per (sample, temperature) observables O that are binned, [S][T][4], from one measurement (e [S][R][T],
+    q0 [S][P][T], qk [S][P][T][3][2]): mean over replicas of e; mean over pairs of q0^2; mean over pairs and the three
+    k_min directions of |q(k_mu)|^2 (the chi(0), chi(k_min) estimators of Eq. (3), PAPER.md:87-91, up to the factor N);
+    mean over pairs of q0^4.  No replica pair (R = 1): the three overlap entries are 0."""
+    S, R, T = e.shape
+    out = np.zeros((S, T, 4))
+    out[..., 0] = e.mean(axis=1)
+    if q0.shape[1] > 0:
+        out[..., 1] = (q0 ** 2).mean(axis=1)
+        out[..., 2] = (qk ** 2).sum(axis=-1).mean(axis=-1).mean(axis=1)
+        out[..., 3] = (q0 ** 4).mean(axis=1)
+    return out
+
+
+LOGBINS = 32
+
+
 def replica_pairs(R):
     """Pairs a<b in the order (0,1),(0,2),...,(R-2,R-1) (reading R15)."""
     return [(a, b) for a in range(R) for b in range(a + 1, R)]
@@ -260,6 +289,9 @@ class OracleSim:
         self.accepts = np.zeros_like(self.attempts)
         self.walk_label = np.zeros((self.S, self.R, self.T), dtype=np.int32)
         self.round_trips = np.zeros((self.S, self.R, 1), dtype=np.uint64)
+        self.n_acc = 0
+        self.logbin_sums = np.zeros((LOGBINS, self.S, self.T, 4))
+        self.logbin_counts = np.zeros(LOGBINS, dtype=np.uint64)
 
     def g0(self, sample):
         return (self.first_sample + sample) * self.C
@@ -341,6 +373,13 @@ class OracleSim:
                     q0[s, p, t] = o[0]
                     qk[s, p, t] = o[1:].reshape(3, 2)
         return e, q0, qk
+
+    def accumulate(self):
+        """Measure and add into the logarithmic bins: the n-th call goes to bin logbin_index(n)."""
+        self.n_acc += 1
+        b = logbin_index(self.n_acc)
+        self.logbin_sums[b] += logbin_observables(*self.measure())
+        self.logbin_counts[b] += 1
 
     def measure_chiral(self):
         """qc0[S][P][T][3], qck[S][P][T][3][3][2]: chiral-glass overlaps of the replica pairs a<b with both

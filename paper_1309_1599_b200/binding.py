@@ -20,7 +20,7 @@ DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_sweep_or", "sg_sweep_hb",
     "sg_pt_swap", "sg_run_units", "sg_measure", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
-    "sg_halfsweep", "sg_pt_stats", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
+    "sg_halfsweep", "sg_pt_stats", "sg_pt_walk", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
 ]
 
@@ -75,6 +75,7 @@ def load_library():
     L.sg_set_counters.argtypes = [vp, u64, u64]; L.sg_set_counters.restype = i
     L.sg_halfsweep.argtypes = [vp, i, i]; L.sg_halfsweep.restype = i
     L.sg_pt_stats.argtypes = [vp, vp, vp]; L.sg_pt_stats.restype = i
+    L.sg_pt_walk.argtypes = [vp, vp, vp]; L.sg_pt_walk.restype = i
     L.sg_tune.argtypes = [vp, i, i]; L.sg_tune.restype = i
     L.sg_sync.argtypes = [vp]; L.sg_sync.restype = i
     L.sg_kernel_launches.argtypes = [vp]; L.sg_kernel_launches.restype = u64
@@ -255,6 +256,12 @@ class SpinGlass:
         att = np.zeros((self.S, self.R, n), dtype=np.uint64); acc = np.zeros((self.S, self.R, n), dtype=np.uint64)
         self._check(self._lib.sg_pt_stats(self._ctx, _ptr(att), _ptr(acc)), "sg_pt_stats")
         return att, acc
+
+    def pt_walk(self):
+        """(round_trips uint64 [S][R], label int32 [S][R][T]) of the random walk in temperature."""
+        trips = np.zeros((self.S, self.R), dtype=np.uint64); lab = np.zeros((self.S, self.R, self.T), dtype=np.int32)
+        self._check(self._lib.sg_pt_walk(self._ctx, _ptr(trips), _ptr(lab)), "sg_pt_walk")
+        return trips, lab
 
     def tune(self, knob, value):
         self._check(self._lib.sg_tune(self._ctx, int(knob), int(value)), "sg_tune")

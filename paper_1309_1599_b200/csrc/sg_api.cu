@@ -25,6 +25,7 @@ struct sg_ctx {
     size_t result_doubles = 0;
     int* slot_of_temp; int* temp_of_slot;
     unsigned long long* attempts; unsigned long long* accepts;
+    int* walk_label; unsigned long long* round_trips;
     // sweep geometry
     int tile_sites, ntiles, log2L;
     // z-marching sweep (L a multiple of 8): tuning knobs and the derived chunking
@@ -87,7 +88,7 @@ struct Carve {
 };
 
 struct Offsets {
-    size_t spins, Jg, Jt, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, total;
+    size_t spins, Jg, Jt, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, total;
 };
 
 Offsets offsets(const Geometry& g)
@@ -112,6 +113,8 @@ Offsets offsets(const Geometry& g)
     size_t st = (size_t)g.S * g.R * (g.T > 1 ? g.T - 1 : 1) * sizeof(unsigned long long);
     o.att = c.take(st);
     o.acc = c.take(st);
+    o.wlab = c.take((size_t)g.S * g.R * g.T * sizeof(int));
+    o.trips = c.take((size_t)g.S * g.R * sizeof(unsigned long long));
     o.total = c.off;
     return o;
 }
@@ -474,6 +477,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     }
     ctx->slot_of_temp = (int*)(base + o.sot); ctx->temp_of_slot = (int*)(base + o.tos);
     ctx->attempts = (unsigned long long*)(base + o.att); ctx->accepts = (unsigned long long*)(base + o.acc);
+    ctx->walk_label = (int*)(base + o.wlab); ctx->round_trips = (unsigned long long*)(base + o.trips);
     ctx->h_betas.assign(betas, betas + g.T);
     ctx->inited.assign(g.S, 0);
     ctx->hb_counter = ctx->pt_counter = ctx->launches = 0;
@@ -499,6 +503,8 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     const size_t st = (size_t)g.S * g.R * (g.T > 1 ? g.T - 1 : 1) * sizeof(unsigned long long);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->attempts, 0, st, ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->accepts, 0, st, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->walk_label, 0, (size_t)g.S * g.R * g.T * sizeof(int), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->round_trips, 0, (size_t)g.S * g.R * sizeof(unsigned long long), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->E, 0, (size_t)g.S * g.Cp * sizeof(double), ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // the host vectors above go out of scope
     if (e != cudaSuccess) { delete ctx; return SG_ECUDA; }
@@ -612,6 +618,7 @@ int sg_pt_swap(sg_ctx* ctx)
     PtParams p;
     p.betas = ctx->betas; p.E = ctx->E; p.slot_of_temp = ctx->slot_of_temp; p.temp_of_slot = ctx->temp_of_slot;
     p.beta_slot = ctx->beta_slot; p.attempts = ctx->attempts; p.accepts = ctx->accepts;
+    p.walk_label = ctx->walk_label; p.round_trips = ctx->round_trips;
     p.S = ctx->S; p.R = ctx->R; p.T = ctx->T; p.Cp = ctx->Cp;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.pt_counter = (uint32_t)ctx->pt_counter;
@@ -821,6 +828,15 @@ int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts)
     const size_t n = (size_t)ctx->S * ctx->R * (ctx->T - 1) * sizeof(unsigned long long);
     if (attempts) SG_CUDA(ctx, cudaMemcpyAsync(attempts, ctx->attempts, n, cudaMemcpyDeviceToHost, ctx->stream));
     if (accepts) SG_CUDA(ctx, cudaMemcpyAsync(accepts, ctx->accepts, n, cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_pt_walk(sg_ctx* ctx, uint64_t* round_trips, int32_t* label)
+{
+    if (!ctx) return SG_EINVAL;
+    if (round_trips) SG_CUDA(ctx, cudaMemcpyAsync(round_trips, ctx->round_trips, (size_t)ctx->S * ctx->R * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
+    if (label) SG_CUDA(ctx, cudaMemcpyAsync(label, ctx->walk_label, (size_t)ctx->S * ctx->R * ctx->T * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
 }

@@ -269,6 +269,8 @@ struct PtParams {
     float* beta_slot;      // [S][Cp]
     unsigned long long* attempts;  // [S][R][T-1]
     unsigned long long* accepts;
+    int* walk_label;                 // [S][R][T]: 0 = no end touched yet, 1 = last touched index 0, 2 = last touched index T-1
+    unsigned long long* round_trips; // [S][R]: completed walks 0 -> T-1 -> 0, summed over the chain's configurations
     int S, R, T, Cp;
     uint32_t key0, key1, pt_counter, chain_first;   // chain id of (local sample 0, r = 0) = first_sample*R
 };
@@ -297,6 +299,19 @@ __global__ void k_pt_swap(const PtParams p)
             p.accepts[(size_t)chain * (p.T - 1) + t] += 1ull;
         }
     }
+    // random walk in temperature of every configuration of the chain
+    int* lab = p.walk_label + (size_t)chain * p.T;
+    unsigned long long trips = 0ull;
+    for (int slot = 0; slot < p.T; ++slot) {
+        const int t = tos[slot];
+        if (t == 0) {
+            if (lab[slot] == 2) trips += 1ull;
+            lab[slot] = 1;
+        } else if (t == p.T - 1 && lab[slot] == 1) {
+            lab[slot] = 2;
+        }
+    }
+    p.round_trips[chain] += trips;
 }
 
 // beta_slot[sample][r*T + slot] = beta[temp_of_slot], for all chains (after init / set_perm)

@@ -313,6 +313,23 @@ def test_pt_decisions_identical_on_identical_energies(sg, oracle, sh):
     assert gpu.get_counters() == (0, 40)
 
 
+@pytest.mark.parametrize("sh", [SHAPES[0], SHAPES[2]])
+def test_pt_random_walk_in_temperature_bit_exact(sg, oracle, sh):
+    """Round-trip bookkeeping of the walk in temperature against the oracle, sweep by sweep: integer work."""
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=13, first_sample=1, tune=sh.get("tune"))
+    rng = np.random.default_rng(6)
+    trips0, lab0 = gpu.pt_walk()
+    assert trips0.sum() == 0 and not lab0.any()
+    for k in range(60 * T):
+        E = rng.normal(0.0, 0.5 / abs(betas_of(sh)[1] - betas_of(sh)[0]), size=(S, R * T))   # acceptance well above 1/2
+        gpu.set_energies(E); gpu.pt_swap(); sim.pt_swap(energies=E)
+        if k % 37 == 0 or k == 60 * T - 1:
+            trips, lab = gpu.pt_walk()
+            assert np.array_equal(trips, sim.round_trips[..., 0]) and np.array_equal(lab, sim.walk_label), k
+    assert trips.sum() > 0 and set(np.unique(lab)) <= {0, 1, 2}
+
+
 def test_pt_moves_temperatures_not_spins_and_hb_follows(sg, oracle):
     """After PT the heat bath must use each slot's *new* temperature (beta by slot follows the swap)."""
     sh = SHAPES[0]
