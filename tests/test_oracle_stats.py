@@ -327,3 +327,51 @@ def test_pt_walk_round_trips_by_hand_and_brute_force(oracle):
     assert int(trips[0]) == brute and brute > 5
     assert np.array_equal(visits, np.array([[np.sum(hist[:, s] == t) for t in range(T)] for s in range(T)], dtype=np.uint64))
     assert visits.sum() == n * T
+
+
+# ---------------------------------------------------------------------------------------------
+# logarithmic data binning (Sect. III): pins of oracle.logbin_index / logbin_observables / accumulate
+# ---------------------------------------------------------------------------------------------
+def test_logbin_is_the_papers_halving_of_the_time_series(oracle):
+    """"i_f contains the last half of the Monte Carlo time series, i_f - 1 the second quarter, i_f - 2 the second octave,
+    and so on", each bin "twice the length of the previous": slice a series of 2^k - 1 values by hand."""
+    k = 7
+    M = 2 ** k - 1
+    bins = np.array([oracle.logbin_index(n) for n in range(1, M + 1)])
+    assert bins[-1] == k - 1
+    assert np.array_equal(np.where(bins == k - 1)[0], np.arange(M - 2 ** (k - 1), M))              # last half
+    assert np.array_equal(np.where(bins == k - 2)[0], np.arange(2 ** (k - 2) - 1, 2 ** (k - 1) - 1))  # second quarter
+    assert np.array_equal(np.where(bins == k - 3)[0], np.arange(2 ** (k - 3) - 1, 2 ** (k - 2) - 1))  # second octave
+    assert [int(np.sum(bins == i)) for i in range(k)] == [2 ** i for i in range(k)]
+    assert oracle.logbin_index(1) == 0 and oracle.logbin_index(2 ** 31 - 1) == 30 and oracle.logbin_index(2 ** 31) == 31
+
+
+def test_logbin_observables_by_hand(oracle):
+    """R = 2, T = 1, one pair: e = (1, 3) -> 2; q0 = 1/2 -> q0^2 = 1/4, q0^4 = 1/16; q(k) = (3+4i, 0, 1i) -> (25+0+1)/3.
+    R = 3: means over the three pairs.  R = 1: no overlap entries."""
+    e = np.array([[[1.0], [3.0]]]); q0 = np.array([[[0.5]]])
+    qk = np.zeros((1, 1, 1, 3, 2)); qk[0, 0, 0, 0] = (3.0, 4.0); qk[0, 0, 0, 2] = (0.0, 1.0)
+    assert np.allclose(oracle.logbin_observables(e, q0, qk)[0, 0], [2.0, 0.25, 26.0 / 3.0, 0.0625], rtol=0, atol=1e-15)
+    e3 = np.array([[[1.0], [2.0], [6.0]]]); q3 = np.array([[[1.0], [2.0], [3.0]]])
+    qk3 = np.zeros((1, 3, 1, 3, 2)); qk3[0, 1, 0, 1, 0] = 3.0
+    assert np.allclose(oracle.logbin_observables(e3, q3, qk3)[0, 0], [3.0, 14.0 / 3.0, 1.0, 98.0 / 3.0], rtol=0, atol=1e-14)
+    assert np.array_equal(oracle.logbin_observables(np.ones((2, 1, 3)), np.zeros((2, 0, 3)), np.zeros((2, 0, 3, 3, 2)))[..., 1:],
+                          np.zeros((2, 3, 3)))
+
+
+def test_accumulate_bins_a_recorded_series(oracle):
+    """OracleSim.accumulate over 15 units of a small chain: bin sums / counts equal the recorded measurements sliced
+    as in the paper (bin 3 = last 8, bin 2 = the 4 before, ...)."""
+    betas = np.linspace(0.6, 1.6, 4)
+    sim = oracle.OracleSim(4, 1, 2, 4, betas, 3)
+    sim.init_sample(0)
+    rec = []
+    for _ in range(15):
+        sim.unit(2)
+        rec.append(oracle.logbin_observables(*sim.measure()))
+        sim.accumulate()
+    rec = np.array(rec)
+    assert sim.n_acc == 15 and list(sim.logbin_counts[:5]) == [1, 2, 4, 8, 0]
+    for i, (lo, hi) in enumerate([(0, 1), (1, 3), (3, 7), (7, 15)]):
+        assert np.allclose(sim.logbin_sums[i], rec[lo:hi].sum(axis=0), rtol=0, atol=1e-13)
+    assert not sim.logbin_sums[4:].any()
