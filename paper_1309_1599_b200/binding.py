@@ -13,12 +13,13 @@ GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2,
 KIND_OR, KIND_HB = 0, 1
 SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
 TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES = 0, 1, 2
+LOGBINS = 32
 SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT = 0, 1, 2, 3
 
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_sweep_or", "sg_sweep_hb",
-    "sg_pt_swap", "sg_run_units", "sg_measure", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
+    "sg_pt_swap", "sg_run_units", "sg_measure", "sg_accumulate", "sg_get_logbins", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
     "sg_halfsweep", "sg_pt_stats", "sg_pt_walk", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
@@ -75,6 +76,8 @@ def load_library():
     L.sg_set_counters.argtypes = [vp, u64, u64]; L.sg_set_counters.restype = i
     L.sg_halfsweep.argtypes = [vp, i, i]; L.sg_halfsweep.restype = i
     L.sg_pt_stats.argtypes = [vp, vp, vp]; L.sg_pt_stats.restype = i
+    L.sg_accumulate.argtypes = [vp]; L.sg_accumulate.restype = i
+    L.sg_get_logbins.argtypes = [vp, vp, vp]; L.sg_get_logbins.restype = i
     L.sg_pt_walk.argtypes = [vp, vp, vp]; L.sg_pt_walk.restype = i
     L.sg_tune.argtypes = [vp, i, i]; L.sg_tune.restype = i
     L.sg_sync.argtypes = [vp]; L.sg_sync.restype = i
@@ -256,6 +259,16 @@ class SpinGlass:
         att = np.zeros((self.S, self.R, n), dtype=np.uint64); acc = np.zeros((self.S, self.R, n), dtype=np.uint64)
         self._check(self._lib.sg_pt_stats(self._ctx, _ptr(att), _ptr(acc)), "sg_pt_stats")
         return att, acc
+
+    def accumulate(self):
+        """Measure and add into the device-side logarithmic bins; asynchronous."""
+        self._check(self._lib.sg_accumulate(self._ctx), "sg_accumulate")
+
+    def get_logbins(self):
+        """(sums float64 [LOGBINS][S][T][4], counts uint64 [LOGBINS])."""
+        sums = np.zeros((LOGBINS, self.S, self.T, 4)); counts = np.zeros(LOGBINS, dtype=np.uint64)
+        self._check(self._lib.sg_get_logbins(self._ctx, _ptr(sums), _ptr(counts)), "sg_get_logbins")
+        return sums, counts
 
     def pt_walk(self):
         """(round_trips uint64 [S][R], label int32 [S][R][T]) of the random walk in temperature."""

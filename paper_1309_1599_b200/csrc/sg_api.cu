@@ -26,6 +26,7 @@ struct sg_ctx {
     int* slot_of_temp; int* temp_of_slot;
     unsigned long long* attempts; unsigned long long* accepts;
     int* walk_label; unsigned long long* round_trips;
+    double* logbin; uint64_t n_acc;
     // sweep geometry
     int tile_sites, ntiles, log2L;
     // z-marching sweep (L a multiple of 8): tuning knobs and the derived chunking
@@ -88,7 +89,7 @@ struct Carve {
 };
 
 struct Offsets {
-    size_t spins, Jg, Jt, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, total;
+    size_t spins, Jg, Jt, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, logbin, total;
 };
 
 Offsets offsets(const Geometry& g)
@@ -115,6 +116,7 @@ Offsets offsets(const Geometry& g)
     o.acc = c.take(st);
     o.wlab = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     o.trips = c.take((size_t)g.S * g.R * sizeof(unsigned long long));
+    o.logbin = c.take((size_t)SG_LOGBINS * g.S * g.T * 4 * sizeof(double));
     o.total = c.off;
     return o;
 }
@@ -478,6 +480,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->slot_of_temp = (int*)(base + o.sot); ctx->temp_of_slot = (int*)(base + o.tos);
     ctx->attempts = (unsigned long long*)(base + o.att); ctx->accepts = (unsigned long long*)(base + o.acc);
     ctx->walk_label = (int*)(base + o.wlab); ctx->round_trips = (unsigned long long*)(base + o.trips);
+    ctx->logbin = (double*)(base + o.logbin); ctx->n_acc = 0;
     ctx->h_betas.assign(betas, betas + g.T);
     ctx->inited.assign(g.S, 0);
     ctx->hb_counter = ctx->pt_counter = ctx->launches = 0;
@@ -505,6 +508,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->accepts, 0, st, ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->walk_label, 0, (size_t)g.S * g.R * g.T * sizeof(int), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->round_trips, 0, (size_t)g.S * g.R * sizeof(unsigned long long), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->logbin, 0, (size_t)SG_LOGBINS * g.S * g.T * 4 * sizeof(double), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->E, 0, (size_t)g.S * g.Cp * sizeof(double), ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // the host vectors above go out of scope
     if (e != cudaSuccess) { delete ctx; return SG_ECUDA; }
@@ -641,13 +645,13 @@ int sg_run_units(sg_ctx* ctx, int n_units, int n_or)
     return SG_OK;
 }
 
-int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
+// S3 + S5 into ctx->result = [ e | q0 | qk ] (asynchronous); with_q = false skips the overlap pass
+static int launch_measure(sg_ctx* ctx, bool with_q)
 {
-    if (!ctx) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     if (int rc = ensure_energies(ctx)) return rc;
     const int PT = ctx->P * ctx->T;
-    if (PT > 0 && (q0 || qk)) {
+    if (PT > 0 && with_q) {
         MeasureParams p;
         p.spins = ctx->spins; p.slot_of_temp = ctx->slot_of_temp; p.phase = ctx->phase; p.Mpart = ctx->Mpart;
         p.L = ctx->L; p.N = ctx->N; p.NG = ctx->NG; p.Cp = ctx->Cp; p.R = ctx->R; p.T = ctx->T; p.P = ctx->P;
@@ -665,6 +669,15 @@ int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
     k_reduce_measure<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->Mpart, ctx->E, ctx->slot_of_temp, ctx->result, ctx->S,
                                                                  ctx->R, ctx->T, ctx->P, ctx->Cp, ctx->nchunk, ctx->N);
     SG_LAUNCHED(ctx);
+    return SG_OK;
+}
+
+int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
+{
+    if (!ctx) return SG_EINVAL;
+    if (int rc = launch_measure(ctx, q0 || qk)) return rc;
+    const int PT = ctx->P * ctx->T;
+    const int nE = ctx->S * ctx->R * ctx->T, nQ = ctx->S * PT;
     {
         int rc;
         if (const double* h = fetch_result(ctx, (size_t)nE + (size_t)nQ * 7, &rc)) {
@@ -678,6 +691,34 @@ int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
     if (e) SG_CUDA(ctx, cudaMemcpyAsync(e, ctx->result, (size_t)nE * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (q0 && nQ) SG_CUDA(ctx, cudaMemcpyAsync(q0, ctx->result + nE, (size_t)nQ * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (qk && nQ) SG_CUDA(ctx, cudaMemcpyAsync(qk, ctx->result + nE + nQ, (size_t)nQ * 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_accumulate(sg_ctx* ctx)
+{
+    if (!ctx) return SG_EINVAL;
+    if (int rc = launch_measure(ctx, true)) return rc;
+    const uint64_t n = ctx->n_acc + 1;
+    int b = 0;
+    while (b + 1 < SG_LOGBINS && (n >> (b + 1)) != 0) ++b;
+    const int items = ctx->S * ctx->T;
+    k_logbin_add<<<(items + 127) / 128, 128, 0, ctx->stream>>>(ctx->result, ctx->logbin + (size_t)b * items * 4, ctx->S, ctx->R, ctx->T, ctx->P);
+    SG_LAUNCHED(ctx);
+    ctx->n_acc = n;
+    return SG_OK;
+}
+
+int sg_get_logbins(sg_ctx* ctx, double* sums, uint64_t* counts)
+{
+    if (!ctx) return SG_EINVAL;
+    if (counts) {
+        for (int b = 0; b < SG_LOGBINS; ++b) {
+            const uint64_t lo = 1ull << b, hi = (b + 1 < SG_LOGBINS) ? (1ull << (b + 1)) : ~0ull;   // measurements lo <= n < hi
+            counts[b] = (ctx->n_acc < lo) ? 0 : ((ctx->n_acc < hi ? ctx->n_acc + 1 : hi) - lo);
+        }
+    }
+    if (sums) SG_CUDA(ctx, cudaMemcpyAsync(sums, ctx->logbin, (size_t)SG_LOGBINS * ctx->S * ctx->T * 4 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
 }

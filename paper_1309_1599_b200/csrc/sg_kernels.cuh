@@ -417,6 +417,33 @@ __global__ void k_reduce_measure(const double* __restrict__ Mpart, const double*
     }
 }
 
+// Logarithmic data binning (Sect. III): adds the observables of one measurement (the `result` of
+// k_reduce_measure) into bin[S][T][4]: mean over replicas of e, mean over pairs of q0^2, mean over pairs and the
+// three k_min directions of |q(k_mu)|^2, mean over pairs of q0^4.  Thread = (sample, temperature); fp64, fixed order.
+__global__ void k_logbin_add(const double* __restrict__ result, double* __restrict__ bin, int S, int R, int T, int P)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= S * T) return;
+    const int sample = u / T, t = u % T;
+    const int nE = S * R * T, PT = P * T, nQ = S * PT;
+    double e = 0.0, q2 = 0.0, qk2 = 0.0, q4 = 0.0;
+    for (int r = 0; r < R; ++r) e += result[((size_t)sample * R + r) * T + t];
+    e /= (double)R;
+    for (int pr = 0; pr < P; ++pr) {
+        const size_t item = (size_t)sample * PT + (size_t)pr * T + t;
+        const double q = result[nE + item];
+        q2 += q * q;
+        q4 += (q * q) * (q * q);
+        const double* k = result + nE + nQ + item * 6;
+        double m = 0.0;
+        for (int mu = 0; mu < 3; ++mu) m += k[2 * mu] * k[2 * mu] + k[2 * mu + 1] * k[2 * mu + 1];
+        qk2 += m / 3.0;
+    }
+    if (P > 0) { q2 /= (double)P; qk2 /= (double)P; q4 /= (double)P; }
+    double* o = bin + (size_t)u * 4;
+    o[0] += e; o[1] += q2; o[2] += qk2; o[3] += q4;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Chirality observables (Eq. (2)): zeta_{x,mu} = s_{x+e_mu} . (s_x x s_{x-e_mu}),
 // kappa_{x,mu} = zeta^a zeta^b, q^_CG^mu(k) = sum_x kappa_{x,mu} e^{ik.x}/N at k = 0 and k_nu = 2 pi e_nu/L.

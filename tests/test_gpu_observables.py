@@ -152,3 +152,32 @@ def test_schwinger_dyson_at_full_size(sg, oracle):
     for r, t in [(0, 0), (3, 47), (1, 16), (2, 31)]:
         want = oracle.sd_terms(L, M, X[r * T + t].astype(np.float64))
         assert np.all(np.abs(got[0, r, t] - want) <= 1e-6 * np.maximum(1.0, np.abs(want)))
+
+
+# ---------------------------------------------------------------------------------------------
+# sg_accumulate / sg_get_logbins: logarithmic data binning on the device (Sect. III)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("sh", [SHAPES[0], SHAPES[2], dict(L=4, S=2, R=1, T=3)])
+def test_logbins_match_oracle(sg, oracle, sh):
+    """11 measurements of an evolving chain: the oracle advances (HB + OR + PT), its state is copied to the device
+    before every measurement (inputs flow oracle -> CUDA), both sides bin.  Bins 0..3 hold 1, 2, 4, 4 measurements."""
+    L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, np.linspace(0.5, 2.0, T), seed=23)
+    for n in range(11):
+        sim.unit(1)
+        for s in range(S):
+            gpu.set_spins(s, sim.spins[s].astype(np.float32))
+            gpu.set_perm(s, sim.temp_of_slot[s])
+        gpu.accumulate()
+        sim.accumulate()
+    sums, counts = gpu.get_logbins()
+    assert list(counts[:5]) == [1, 2, 4, 4, 0] and np.array_equal(counts, sim.logbin_counts)
+    scale = np.maximum(1.0, np.abs(sim.logbin_sums))
+    assert (np.abs(sums - sim.logbin_sums) <= 4 * TOL * scale).all()          # <= 4 measurements of 1e-6 each per bin
+    assert not sums[4:].any()
+    if R > 1:
+        assert (sums[:4, :, :, 1:] > 0).all()                                # the comparison is not vacuous
+    else:
+        assert not sums[..., 1:].any()
+    e, _, _ = gpu.measure()                                                    # sg_measure still serves after sg_accumulate
+    assert np.abs(e - sim.measure()[0]).max() <= TOL * max(1.0, np.abs(e).max())
