@@ -116,6 +116,38 @@ def gen_couplings(L, seed, sample, mode=OFFDIAG_SYM, sigma_D=1.0):
     return M
 
 
+def bimodal_couplings(L, links, D):
+    """The paper's own couplings from their packed form (Sect. II.A: J_xy = +-1, D_xy symmetric with
+    six independent elements +-D; App. A.3: "a full coupling in a single byte").  links uint8 [3][N]:
+    bit 0 of the byte of link (x, mu) is the sign of J (1: +1), bits 1, 2, 3 the signs of D^00, D^11, D^22, bits 4, 5, 6
+    those of D^01 = D^10, D^02 = D^20, D^12 = D^21 (1: +D).  Returns M [3][N][3][3] = J 1 + D, every entry rounded to
+    fp32 (reading R20) -- the bit assignment is that of gen_couplings(mode=BIMODAL) on the word it draws."""
+    links = np.asarray(links, dtype=np.uint8).reshape(3, L ** 3)
+    M = np.zeros((3, L ** 3, 3, 3))
+    for mu in range(3):
+        for i in range(L ** 3):
+            b = int(links[mu, i])
+            J = 1.0 if (b & 1) else -1.0
+            d = [float(D) if ((b >> (k + 1)) & 1) else -float(D) for k in range(6)]
+            m = np.array([[J + d[0], d[3], d[4]],
+                          [d[3], J + d[1], d[5]],
+                          [d[4], d[5], J + d[2]]])
+            M[mu, i] = m.astype(np.float32).astype(np.float64)
+    return M
+
+
+def bimodal_links(L, seed, sample):
+    """The bytes gen_couplings(mode=BIMODAL) uses: the low 7 bits of word 0 of the coupling stream's first block,
+    counter (3 i + mu, sample, 0, 4)."""
+    N = L ** 3
+    out = np.zeros((3, N), dtype=np.uint8)
+    key = (int(seed) & 0xffffffff, int(seed) >> 32)
+    for i in range(N):
+        for mu in range(3):
+            out[mu, i] = philox4x32_10((3 * i + mu, int(sample), 0, 4), key)[0] & 0x7f
+    return out
+
+
 def gen_spins(L, seed, g):
     s = np.zeros((3, L ** 3))
     lib().sgo_gen_spins(L, int(seed), int(g), _dp(s))

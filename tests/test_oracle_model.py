@@ -412,3 +412,31 @@ def test_sd_terms_closed_forms_and_energy_relation(oracle):
         sh = (s * h).sum(axis=0)
         assert abs(b - ((h * h).sum(axis=0) - sh ** 2).mean()) < 1e-12
         assert b >= 0.0                                                                 # |h|^2 >= (s.h)^2 for unit s
+
+
+# ---------------------------------------------------------------------------------------------
+# packed bimodal couplings: pins of oracle.bimodal_couplings / bimodal_links
+# ---------------------------------------------------------------------------------------------
+def test_bimodal_byte_decodes_to_the_papers_coupling(oracle):
+    """Every one of the 128 bytes: M = J 1 + D with J = +-1 and D symmetric, six independent elements +-D (PAPER.md:65,
+    73); the map byte -> matrix is injective (7 bits = 7 signs); two bytes worked by hand; and the decoder reproduces
+    the BIMODAL generator from the bytes of its own Philox word."""
+    D = 0.5
+    links = np.zeros((3, 64), dtype=np.uint8)
+    links[0] = np.arange(64); links[1] = np.arange(64, 128); links[2, 0] = 0b1011010
+    M = oracle.bimodal_couplings(4, links, D)
+    mats = np.concatenate([M[0], M[1]])                     # bytes 0 .. 127
+    assert np.array_equal(mats, mats.transpose(0, 2, 1))
+    off = mats[:, [0, 0, 1], [1, 2, 2]]
+    assert np.array_equal(np.abs(off), np.full((128, 3), D))
+    J = np.where(np.arange(128) & 1, 1.0, -1.0)
+    dd = mats[:, [0, 1, 2], [0, 1, 2]] - J[:, None]
+    assert np.array_equal(np.abs(dd), np.full((128, 3), D))
+    assert len({m.tobytes() for m in mats}) == 128
+    # byte 0: J = -1, all D elements -D.  byte 0b1011010: J = -1; D00 = +, D11 = -, D22 = +; D01 = +, D02 = -, D12 = +
+    assert np.array_equal(mats[0], [[-1.5, -0.5, -0.5], [-0.5, -1.5, -0.5], [-0.5, -0.5, -1.5]])
+    assert np.array_equal(M[2, 0], [[-0.5, 0.5, -0.5], [0.5, -1.5, 0.5], [-0.5, 0.5, -0.5]])
+    for L, seed, sample, Dg in [(4, 9, 3, 0.5), (2, 1, 0, 1.0), (4, 77, 1, 0.3)]:
+        bits = oracle.bimodal_links(L, seed, sample)
+        assert np.array_equal(oracle.bimodal_couplings(L, bits, Dg), oracle.gen_couplings(L, seed, sample, oracle.BIMODAL, Dg))
+        assert 0.4 < np.unpackbits(bits).mean() * 8 / 7 < 0.6      # the signs are balanced (the top bit is always 0)
