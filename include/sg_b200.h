@@ -88,6 +88,19 @@ int sg_destroy(sg_ctx* ctx);
 int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const float* couplings,
                    const float* spins);
 
+/* The paper's own couplings in their packed form (Sect. II.A: J_xy = +-1 and a
+ * symmetric D_xy with six independent elements +-D; App. A.3: "a full coupling in a single byte").
+ *   links: host uint8 [3][N], one byte per forward link (x, mu); bit 0 = sign of J (1: +1), bits 1, 2, 3 = signs of
+ *          D^00, D^11, D^22, bits 4, 5, 6 = signs of D^01 = D^10, D^02 = D^20, D^12 = D^21 (1: +D); bit 7 must be 0 (else
+ *          SG_EINVAL).  NULL: the bytes generator mode SG_GEN_BIMODAL draws for (seed, first_sample + sample).  Copied.
+ *   D >= 0, finite.  spins as in sg_init_sample.
+ * The sample behaves exactly as after sg_init_sample with the fp32 matrices M = fl32(J 1 + D) (which are stored too and
+ * serve sg_get_couplings and every kernel but the one below).  When EVERY sample of the context has been initialised
+ * this way with the same D, L is a multiple of 8 and sg_tune(SG_TUNE_PACKED, 1) was called, the z-marching sweep reads
+ * 8 bytes per site (6 link bytes + pad) instead of 224 and its producer warp decodes them into the shared-memory blocks
+ * the updating warps read: the same fp32 operands, hence the same spins bit for bit. */
+int sg_init_sample_bimodal(sg_ctx* ctx, int sample, double D, const uint8_t* links, const float* spins);
+
 /* S1 (Eq. (A2)).  n_sweeps full overrelaxation sweeps of every copy of every sample:
  * colour 0 half-sweep then colour 1.  The last half-sweep also reduces the total energy of every copy. */
 int sg_sweep_or(sg_ctx* ctx, int n_sweeps);
@@ -186,8 +199,11 @@ int sg_pt_walk(sg_ctx* ctx, uint64_t* round_trips, int32_t* label);
  * All kernels perform the same arithmetic in the same order: the spins do not depend on the choice.
  * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else even, >= 4 and a divisor of L.
  * SG_TUNE_RES_COPIES: copies per CTA of the resident kernel: 0 = automatic, else 4, 8, 16 or 32 (SG_EINVAL if the lattice
- *   of that many copies does not fit in shared memory). */
-enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2 };
+ *   of that many copies does not fit in shared memory).
+ * SG_TUNE_PACKED: 1 = the z-marching sweep reads the packed bytes when every sample was initialised by
+ *   sg_init_sample_bimodal with one and the same D; 0 (default) = always the fp32 matrices, which measured 3-7 % faster
+ *   at 32 and more copies per sample.  Same spins bit for bit. */
+enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2, SG_TUNE_PACKED = 3 };
 enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2, SG_SWEEP_RESIDENT = 3 };
 int sg_tune(sg_ctx* ctx, int knob, int value);
 

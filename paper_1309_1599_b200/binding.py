@@ -12,13 +12,13 @@ _LIB_PATH = os.path.join(_HERE, "libsg_b200.so")
 GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2, 3, 4
 KIND_OR, KIND_HB = 0, 1
 SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
-TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES = 0, 1, 2
+TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES, TUNE_PACKED = 0, 1, 2, 3
 LOGBINS = 32
 SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT = 0, 1, 2, 3
 
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [
-    "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_sweep_or", "sg_sweep_hb",
+    "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_init_sample_bimodal", "sg_sweep_or", "sg_sweep_hb",
     "sg_pt_swap", "sg_run_units", "sg_measure", "sg_accumulate", "sg_get_logbins", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
     "sg_halfsweep", "sg_pt_stats", "sg_pt_walk", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
@@ -57,6 +57,7 @@ def load_library():
     L.sg_create.argtypes = [ctypes.POINTER(vp), shp, vp, vp, ctypes.c_size_t, vp]; L.sg_create.restype = i
     L.sg_destroy.argtypes = [vp]; L.sg_destroy.restype = i
     L.sg_init_sample.argtypes = [vp, i, i, d, vp, vp]; L.sg_init_sample.restype = i
+    L.sg_init_sample_bimodal.argtypes = [vp, i, d, vp, vp]; L.sg_init_sample_bimodal.restype = i
     L.sg_sweep_or.argtypes = [vp, i]; L.sg_sweep_or.restype = i
     L.sg_sweep_hb.argtypes = [vp, i]; L.sg_sweep_hb.restype = i
     L.sg_pt_swap.argtypes = [vp]; L.sg_pt_swap.restype = i
@@ -169,6 +170,17 @@ class SpinGlass:
             assert spins.size == 3 * self.N * self.C
         self._check(self._lib.sg_init_sample(self._ctx, int(sample), int(gen_mode), float(sigma_D), _ptr(couplings),
                                              _ptr(spins)), "sg_init_sample")
+
+    def init_sample_bimodal(self, sample, D, links=None, spins=None):
+        """The paper's J = +-1, D^ab = +-D couplings from one byte per link (uint8 [3][N]; None: the generator's bytes)."""
+        if links is not None:
+            links = np.ascontiguousarray(links, dtype=np.uint8)
+            assert links.size == 3 * self.N
+        if spins is not None:
+            spins = np.ascontiguousarray(spins, dtype=np.float32)
+            assert spins.size == 3 * self.N * self.C
+        self._check(self._lib.sg_init_sample_bimodal(self._ctx, int(sample), float(D), _ptr(links), _ptr(spins)),
+                    "sg_init_sample_bimodal")
 
     def sweep_or(self, n_sweeps=1):
         self._check(self._lib.sg_sweep_or(self._ctx, int(n_sweeps)), "sg_sweep_or")

@@ -19,7 +19,7 @@ struct sg_ctx {
     int L, N, Nh, S, R, T, C, NG, Cp, P;
     cudaStream_t stream;
     // device arrays (carved from the caller's workspace)
-    float* spins; float* Jg; float* Jt; float* Mraw; float* staging; float* beta_slot;
+    float* spins; float* Jg; float* Jt; unsigned char* Jp; float* Mraw; float* staging; float* beta_slot;
     double* betas; double* E; double* Epart; double* SDpart; double* phase; double* Mpart; double* result;
     double* h_result = nullptr;   // pinned host mirror of `result`: one device-to-host copy per measurement call
     size_t result_doubles = 0;
@@ -40,6 +40,8 @@ struct sg_ctx {
     // host state
     std::vector<double> h_betas;
     std::vector<char> inited;
+    std::vector<double> bimodal_D;   // per sample: D of its packed bimodal couplings (sg_init_sample_bimodal), NaN if not packed
+    int packed_on;                   // SG_TUNE_PACKED: 1 = the z-marching sweep reads the packed bytes when every sample is packed
     uint64_t hb_counter, pt_counter, launches;
     bool energies_fresh;
     int last_cuda;
@@ -89,7 +91,7 @@ struct Carve {
 };
 
 struct Offsets {
-    size_t spins, Jg, Jt, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, logbin, total;
+    size_t spins, Jg, Jt, Jp, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, logbin, total;
 };
 
 Offsets offsets(const Geometry& g)
@@ -98,6 +100,7 @@ Offsets offsets(const Geometry& g)
     o.spins = c.take((size_t)g.S * g.NG * g.N * SITE_FLOATS * sizeof(float));
     o.Jg = c.take((size_t)g.S * 2 * g.Nh * JG * sizeof(float));
     o.Jt = c.take((g.L % 8 == 0) ? (size_t)g.S * 2 * g.Nh * JG * sizeof(float) : 0);
+    o.Jp = c.take((g.L % 8 == 0) ? (size_t)g.S * g.N * 8 : 0);
     o.Mraw = c.take((size_t)g.S * 3 * g.N * 9 * sizeof(float));
     size_t stg = (size_t)G * 3 * g.N * sizeof(float);
     o.staging = c.take(stg);
@@ -167,6 +170,16 @@ void link_normals(uint64_t seed, uint32_t link, uint32_t sample, double n[12], u
     }
 }
 
+// the paper's coupling of one link from its byte (layout in include/sg_b200.h)
+void bimodal_matrix(uint32_t b, double D, double m[9])
+{
+    const double J = (b & 1u) ? 1.0 : -1.0;
+    double d[6];
+    for (int k = 0; k < 6; ++k) d[k] = ((b >> (k + 1)) & 1u) ? D : -D;
+    m[0] = J + d[0]; m[4] = J + d[1]; m[8] = J + d[2];
+    m[1] = m[3] = d[3]; m[2] = m[6] = d[4]; m[5] = m[7] = d[5];
+}
+
 void generate_couplings(int L, uint64_t seed, uint32_t sample, int mode, double sd, float* M)
 {
     const int N = L * L * L;
@@ -187,14 +200,9 @@ void generate_couplings(int L, uint64_t seed, uint32_t sample, int mode, double 
             case SG_GEN_GENERAL9:
                 for (int e = 0; e < 9; ++e) m[e] = sd * n[e];
                 break;
-            case SG_GEN_BIMODAL: {
-                const double J = (w0[0] & 1u) ? 1.0 : -1.0;
-                double d[6];
-                for (int k = 0; k < 6; ++k) d[k] = ((w0[0] >> (k + 1)) & 1u) ? sd : -sd;
-                m[0] = J + d[0]; m[4] = J + d[1]; m[8] = J + d[2];
-                m[1] = m[3] = d[3]; m[2] = m[6] = d[4]; m[5] = m[7] = d[5];
+            case SG_GEN_BIMODAL:
+                bimodal_matrix(w0[0] & 0x7fu, sd, m);
                 break;
-            }
             default:
                 m[0] = m[4] = m[8] = 1.0;
             }
@@ -240,10 +248,10 @@ void zm_plan(sg_ctx* ctx)
     ctx->zm_ZC = ZC; ctx->zm_nzc = L / ZC;
 }
 
-template <int KIND, bool WITH_E>
-int launch_zm(sg_ctx* ctx, const ZmParams& p, dim3 grid)
+template <int KIND, bool WITH_E, bool PACKED>
+int launch_zm_p(sg_ctx* ctx, const ZmParams& p, dim3 grid)
 {
-    auto kern = k_sweep_zm<KIND, WITH_E, ZM_TX, ZM_TY, ZM_NST, ZM_NJ>;
+    auto kern = k_sweep_zm<KIND, WITH_E, ZM_TX, ZM_TY, ZM_NST, ZM_NJ, PACKED>;
     constexpr size_t smem = zm_smem_bytes<ZM_TX, ZM_TY, ZM_NST, ZM_NJ>();
     static bool attr_done = false;   // per process and template instance; the attribute is per function
     if (!attr_done) {
@@ -254,10 +262,27 @@ int launch_zm(sg_ctx* ctx, const ZmParams& p, dim3 grid)
     return SG_OK;
 }
 
+// the caller asked for the packed path and every sample holds packed bimodal couplings of one and the same D
+bool use_packed(const sg_ctx* ctx)
+{
+    if (!ctx->packed_on || !ctx->Jp) return false;
+    for (double d : ctx->bimodal_D)
+        if (!(d == ctx->bimodal_D[0])) return false;     // NaN (not packed) fails too
+    return true;
+}
+
+template <int KIND, bool WITH_E>
+int launch_zm(sg_ctx* ctx, const ZmParams& p, dim3 grid)
+{
+    return use_packed(ctx) ? launch_zm_p<KIND, WITH_E, true>(ctx, p, grid) : launch_zm_p<KIND, WITH_E, false>(ctx, p, grid);
+}
+
 int half_sweep_zm(sg_ctx* ctx, int kind, int colour, bool with_energy)
 {
     ZmParams p;
     p.spins = ctx->spins; p.Jt = ctx->Jt; p.beta_slot = ctx->beta_slot; p.Epart = ctx->Epart;
+    p.Jp = ctx->Jp; p.bimA = p.bimB = p.bimD = 0.f;
+    if (use_packed(ctx)) { const double D = ctx->bimodal_D[0]; p.bimA = (float)(1.0 + D); p.bimB = (float)(1.0 - D); p.bimD = (float)D; }
     p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.C = ctx->C;
     p.ntx = ctx->L / ZM_TX; p.nty = ctx->L / ZM_TY; p.nzc = ctx->zm_nzc; p.ZC = ctx->zm_ZC;
     p.colour = colour;
@@ -466,7 +491,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->nchunk = g.nchunk; ctx->chunk_sites = g.chunk_sites; ctx->MS = g.MS;
     ctx->stream = (cudaStream_t)cuda_stream;
     char* base = (char*)dev_workspace;
-    ctx->spins = (float*)(base + o.spins); ctx->Jg = (float*)(base + o.Jg); ctx->Jt = (g.L % 8 == 0) ? (float*)(base + o.Jt) : nullptr; ctx->Mraw = (float*)(base + o.Mraw);
+    ctx->spins = (float*)(base + o.spins); ctx->Jg = (float*)(base + o.Jg); ctx->Jt = (g.L % 8 == 0) ? (float*)(base + o.Jt) : nullptr; ctx->Jp = (g.L % 8 == 0) ? (unsigned char*)(base + o.Jp) : nullptr; ctx->Mraw = (float*)(base + o.Mraw);
     ctx->staging = (float*)(base + o.staging); ctx->beta_slot = (float*)(base + o.beta_slot);
     ctx->betas = (double*)(base + o.betas); ctx->E = (double*)(base + o.E); ctx->Epart = (double*)(base + o.Epart);
     ctx->SDpart = (double*)(base + o.SDpart);
@@ -483,6 +508,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->logbin = (double*)(base + o.logbin); ctx->n_acc = 0;
     ctx->h_betas.assign(betas, betas + g.T);
     ctx->inited.assign(g.S, 0);
+    ctx->bimodal_D.assign(g.S, std::nan("")); ctx->packed_on = 0;
     ctx->hb_counter = ctx->pt_counter = ctx->launches = 0;
     ctx->sweep_impl = SG_SWEEP_AUTO; ctx->zm_zc_req = 0;
     ctx->res_cpc_req = 0;
@@ -575,6 +601,7 @@ int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const 
         generate_couplings(ctx->L, ctx->shape.seed, (uint32_t)(ctx->shape.first_sample + sample), gen_mode, sigma_D, gen.data());
         src = gen.data();
     }
+    ctx->bimodal_D[sample] = std::nan("");
     SG_CUDA(ctx, cudaMemcpyAsync(Mdev, src, mfloats * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     k_gather_couplings<<<(ctx->N + 127) / 128, 128, 0, ctx->stream>>>(Mdev, ctx->Jg + (size_t)sample * 2 * ctx->Nh * JG,
@@ -601,6 +628,57 @@ int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const 
     if (int rc = fill_beta_slot(ctx)) return rc;
     ctx->inited[sample] = 1;
     ctx->energies_fresh = false;
+    return SG_OK;
+}
+
+int sg_init_sample_bimodal(sg_ctx* ctx, int sample, double D, const uint8_t* links, const float* spins)
+{
+    if (!ctx || sample < 0 || sample >= ctx->S || !std::isfinite(D) || D < 0.0) return SG_EINVAL;
+    const int L = ctx->L, N = ctx->N;
+    std::vector<uint8_t> bits((size_t)3 * N);
+    if (links) {
+        for (size_t k = 0; k < bits.size(); ++k) {
+            if (links[k] & 0x80u) return SG_EINVAL;
+            bits[k] = links[k];
+        }
+    } else {   // the bytes of generator mode SG_GEN_BIMODAL: low 7 bits of word 0 of the link's first Philox block
+        const uint32_t k0 = (uint32_t)(ctx->shape.seed & 0xffffffffu), k1 = (uint32_t)(ctx->shape.seed >> 32);
+        for (int i = 0; i < N; ++i)
+            for (int mu = 0; mu < 3; ++mu) {
+                uint32_t w[4];
+                philox4x32_10((uint32_t)(3 * i + mu), (uint32_t)(ctx->shape.first_sample + sample), 0u, STREAM_COUPLINGS, k0, k1, w);
+                bits[(size_t)mu * N + i] = (uint8_t)(w[0] & 0x7fu);
+            }
+    }
+    // the fp32 matrices serve every kernel but the packed z-marching sweep (and sg_get_couplings)
+    std::vector<float> M((size_t)3 * N * 9);
+    for (size_t k = 0; k < bits.size(); ++k) {
+        double m[9];
+        bimodal_matrix(bits[k], D, m);
+        for (int e = 0; e < 9; ++e) M[k * 9 + e] = (float)m[e];
+    }
+    if (int rc = sg_init_sample(ctx, sample, SG_GEN_FERRO, 0.0, M.data(), spins)) return rc;
+    if (ctx->Jp) {
+        // per-site gathered bytes in the tile-major order of Jt: (+x1, -x1, +x2, -x2, +x3, -x3, 0, 0); D is symmetric,
+        // so the backward link's byte serves as it is
+        std::vector<uint8_t> pk((size_t)N * 8, 0);
+        const int nt = L >> 3;
+        for (int z = 0; z < L; ++z)
+            for (int y = 0; y < L; ++y)
+                for (int x = 0; x < L; ++x) {
+                    const int i = x + L * (y + L * z), colour = (x + y + z) & 1;
+                    const int bw[3] = { ((x == 0) ? L - 1 : x - 1) + L * (y + L * z), x + L * (((y == 0) ? L - 1 : y - 1) + L * z),
+                                        x + L * (y + L * ((z == 0) ? L - 1 : z - 1)) };
+                    const size_t t = ((((size_t)colour * nt + (y >> 3)) * nt + (x >> 3)) * L + z) * 32 + (y & 7) * 4 + ((x & 7) >> 1);
+                    for (int mu = 0; mu < 3; ++mu) {
+                        pk[t * 8 + 2 * mu] = bits[(size_t)mu * N + i];
+                        pk[t * 8 + 2 * mu + 1] = bits[(size_t)mu * N + bw[mu]];
+                    }
+                }
+        SG_CUDA(ctx, cudaMemcpyAsync(ctx->Jp + (size_t)sample * N * 8, pk.data(), pk.size(), cudaMemcpyHostToDevice, ctx->stream));
+        SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    }
+    ctx->bimodal_D[sample] = D;
     return SG_OK;
 }
 
@@ -897,6 +975,10 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
         if (value > 0 && res_smem_bytes(ctx->N, value) > RES_SMEM_MAX) return SG_EINVAL;
         ctx->res_cpc_req = value;
         res_plan(ctx);
+        return SG_OK;
+    case SG_TUNE_PACKED:
+        if (value != 0 && value != 1) return SG_EINVAL;
+        ctx->packed_on = value;
         return SG_OK;
     case SG_TUNE_ZCHUNK:
         if (value < 0) return SG_EINVAL;

@@ -70,6 +70,8 @@ struct ZmGeom {
     static constexpr int STAGE_BYTES = SLOTS * SITE_BYTES;        // 18432 for 8 x 8
     static constexpr int JSITE_BYTES = JG * 4;                    // 224
     static constexpr int JSTAGE_BYTES = OWN * JSITE_BYTES;        // 7168 for 8 x 8
+    static constexpr int PJSITE_BYTES = 8;                        // packed bimodal couplings: 6 link bytes + 2 pad
+    static constexpr int PJSTAGE_BYTES = OWN * PJSITE_BYTES;      // 256 for 8 x 8
     static constexpr int CONSUMERS = OWN * 8;                     // threads: (site, copy quad)
     static constexpr int THREADS = CONSUMERS + 32;                // + one producer warp
     static constexpr int NWARPS_C = CONSUMERS / 32;
@@ -84,6 +86,8 @@ constexpr size_t zm_smem_bytes()
 struct ZmParams {
     float* spins;            // [S][NG][2][Nh][3][G]
     const float* Jt;         // [S][2][L/TY][L/TX][L][TY][TX/2][JG]
+    const unsigned char* Jp; // [S][2][L/TY][L/TX][L][TY][TX/2][8]: packed bimodal couplings (PACKED kernels only)
+    float bimA, bimB, bimD;  // fl32(1 + D), fl32(1 - D), fl32(D) of the packed couplings
     const float* beta_slot;  // [S][Cp]
     double* Epart;           // [S][NG][nblk][G]
     int L, N, Nh, NG, C;
@@ -118,14 +122,35 @@ __device__ __forceinline__ void zm_update(const float (&hf)[3][4], float (&s)[3]
     }
 }
 
-template <int KIND, bool WITH_E, int TX, int TY, int NST, int NJ>
+// The paper's bimodal coupling from its byte: bit 0 the sign of J = +-1 (1: +), bits 1-3 the
+// signs of D^00, D^11, D^22, bits 4-6 those of D^01, D^02, D^12 (1: +D); M = J 1 + D, D symmetric.  The nine fp32
+// values are those of the unpacked array (fl32(J + d) = +-A or +-B), so the field FMAs see identical operands.
+__device__ __forceinline__ void bimodal_decode(uint32_t b, float A, float B, float D, float* __restrict__ m)
+{
+    const uint32_t jb = b & 1u;
+    const uint32_t sj = (jb ^ 1u) << 31;
+    float dg[3], of[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const uint32_t db = (b >> (1 + a)) & 1u;
+        dg[a] = __uint_as_float(__float_as_uint(db == jb ? A : B) ^ sj);      // J + d = J (1 + d/J)
+        of[a] = __uint_as_float(__float_as_uint(D) ^ ((((b >> (4 + a)) & 1u) ^ 1u) << 31));
+    }
+    m[0] = dg[0]; m[1] = of[0]; m[2] = of[1];
+    m[3] = of[0]; m[4] = dg[1]; m[5] = of[2];
+    m[6] = of[1]; m[7] = of[2]; m[8] = dg[2];
+}
+
+template <int KIND, bool WITH_E, int TX, int TY, int NST, int NJ, bool PACKED = false>
 __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const ZmParams p)
 {
     using Gm = ZmGeom<TX, TY>;
+    constexpr int JST = Gm::JSTAGE_BYTES;                                  // bytes of one coupling stage in shared memory
+    static_assert(!PACKED || Gm::OWN == 32, "the packed path decodes one site per producer lane");
     extern __shared__ __align__(128) unsigned char smem[];
     unsigned char* const ring = smem;                                       // NST stages of other-colour planes
     unsigned char* const jring = smem + (size_t)NST * Gm::STAGE_BYTES;      // NJ stages of coupling blocks
-    const uint32_t bars = smem_u32(jring + (size_t)NJ * Gm::JSTAGE_BYTES);  // full_o[NST] empty_o[NST] full_j[NJ] empty_j[NJ]
+    const uint32_t bars = smem_u32(jring + (size_t)NJ * JST);  // full_o[NST] empty_o[NST] full_j[NJ] empty_j[NJ]
     auto full_o = [&](int s) { return bars + 8u * s; };
     auto empty_o = [&](int s) { return bars + 8u * (NST + s); };
     auto full_j = [&](int s) { return bars + 8u * (2 * NST + s); };
@@ -159,7 +184,13 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
         // and the couplings of a plane are one block of the tile-major array: 11 to 19 bulk copies per step.
         const int lane = tid - Gm::CONSUMERS;
         const float* const other = spins_grp + (size_t)(1 - p.colour) * p.Nh * SITE_FLOATS;
-        const float* const Jtile = p.Jt + ((((size_t)(sample * 2 + p.colour) * p.nty + Y0 / TY) * p.ntx + X0 / TX) * L) * (size_t)(Gm::OWN * JG);
+        const size_t tile_first = (((size_t)(sample * 2 + p.colour) * p.nty + Y0 / TY) * p.ntx + X0 / TX) * L;   // in plane blocks
+        const unsigned char* const Jtile = reinterpret_cast<const unsigned char*>(p.Jt) + tile_first * JST;
+        // packed bimodal couplings: lane = site of the plane, 8 bytes per site read straight from global memory one step
+        // ahead and decoded by this (otherwise idle) warp into the fp32 blocks the consumers read
+        const uint2* const Ptile = reinterpret_cast<const uint2*>(p.Jp + tile_first * Gm::PJSTAGE_BYTES) + lane;
+        uint2 pk_next = make_uint2(0u, 0u);
+        if constexpr (PACKED) pk_next = __ldg(Ptile + (size_t)z0 * Gm::OWN);
         for (int n = 0; n < ZC + 2; ++n) {
             // other-colour plane n of the chunk: x3 = z0 - 1 + n (periodic)
             {
@@ -206,12 +237,28 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
             const int k = n - 2;
             if (k >= 0) {
                 const int st = k % NJ;
-                if (k >= NJ) mbar_wait(empty_j(st), ((k / NJ) - 1) & 1);
-                if (lane == 0) {
-                    mbar_expect_tx(full_j(st), Gm::JSTAGE_BYTES);
-                    bulk_g2s(smem_u32(jring + (size_t)st * Gm::JSTAGE_BYTES), Jtile + (size_t)(z0 + k) * (Gm::OWN * JG), Gm::JSTAGE_BYTES, full_j(st));
+                if constexpr (PACKED) {
+                    const uint2 pk = pk_next;
+                    if (k + 1 < ZC) pk_next = __ldg(Ptile + (size_t)(z0 + k + 1) * Gm::OWN);
+                    float J[JG];
+#pragma unroll
+                    for (int nbk = 0; nbk < 6; ++nbk)     // bytes 0-3: +x1, -x1, +x2, -x2; 4-5: +x3, -x3
+                        bimodal_decode(((nbk < 4) ? (pk.x >> (8 * nbk)) : (pk.y >> (8 * (nbk - 4)))) & 0x7fu, p.bimA, p.bimB, p.bimD, &J[9 * nbk]);
+                    J[54] = 0.f; J[55] = 0.f;
+                    if (k >= NJ) mbar_wait(empty_j(st), ((k / NJ) - 1) & 1);
+                    float* const dstJ = reinterpret_cast<float*>(jring + (size_t)st * JST) + lane * JG;
+#pragma unroll
+                    for (int v = 0; v < JG / 4; ++v) st4(dstJ + 4 * v, make_float4(J[4 * v], J[4 * v + 1], J[4 * v + 2], J[4 * v + 3]));
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(full_j(st));
+                } else {
+                    if (k >= NJ) mbar_wait(empty_j(st), ((k / NJ) - 1) & 1);
+                    if (lane == 0) {
+                        mbar_expect_tx(full_j(st), JST);
+                        bulk_g2s(smem_u32(jring + (size_t)st * JST), Jtile + (size_t)(z0 + k) * JST, JST, full_j(st));
+                    }
+                    __syncwarp();
                 }
-                __syncwarp();
             }
         }
         return;
@@ -276,7 +323,7 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
             const unsigned char* const Pp = ring + sp_ * Gm::STAGE_BYTES;
             const unsigned char* nbp[6] = { P0 + o_xm[d] + Gm::SITE_BYTES, P0 + o_xm[d], P0 + o_yp[d], P0 + o_ym[d],
                                             Pp + o_z[d], Pm + o_z[d] };
-            const unsigned char* const Jp = jring + sj_ * Gm::JSTAGE_BYTES + ks * Gm::JSITE_BYTES;
+            const unsigned char* const Jp = jring + sj_ * JST + ks * Gm::JSITE_BYTES;
 
             float hf[3][4];
 #pragma unroll
