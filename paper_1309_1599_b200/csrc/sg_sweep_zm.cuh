@@ -58,6 +58,22 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 }
 __device__ __forceinline__ float4 lds4(const unsigned char* p) { return *reinterpret_cast<const float4*>(p); }
 
+// L2 eviction policy for the bulk copies: other-colour planes and coupling blocks are re-read within microseconds (by the
+// neighbour tiles' halos, by the other copy groups of the tile), the own-colour stream is not: evict_last on the former
+// measured -0.9 % on the OR half-sweep at cfg 4 (616.2 -> 610.8 us); evict_first on the own loads / stores changed nothing.
+__device__ __forceinline__ uint64_t policy_evict_last()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+                 : "memory");
+}
+
 // Geometry of one ring stage: the other-colour sites of a plane, tile + halo.
 //   interior row yy (0..TY-1): ROW = TX/2+1 slots, slot = yy*ROW + ((xx+1)>>1), xx in [-1, TX]
 //   halo rows yy = -1, TY     : TX/2 slots each, slot = TY*ROW + (yy<0 ? 0 : TX/2) + (xx>>1)
@@ -157,11 +173,15 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
     auto empty_j = [&](int s) { return bars + 8u * (2 * NST + NJ + s); };
 
     const int tid = threadIdx.x;
-    // block -> (tile, chunk, group): the group is fastest so that the CTAs that share a tile's couplings
-    // run next to each other in time (one DRAM read of the couplings per tile, not per group)
+    // block -> (chunk, tile, group).  The group is fastest so that the CTAs that share a tile's couplings run next to each
+    // other in time (one DRAM read of the couplings per tile, not per group); the chunk is slowest, so that the ~296 CTAs
+    // in flight cover ~6 whole rows of neighbouring tiles in the SAME range of planes and find each other's x1 / x2 halo
+    // lines in L2 (tile-outer, chunk-inner order: 3 rows of tiles per range; measured 610 -> 593 us at cfg 4).
     int b = blockIdx.x;
+    const int ntile_ = p.ntx * p.nty;
     const int grp = b % p.NG; b /= p.NG;
-    const int zc = b % p.nzc; b /= p.nzc;
+    const int zc = b / ntile_; b -= zc * ntile_;
+    const int blk_ = zc * ntile_ + b;
     const int X0 = (b % p.ntx) * TX, Y0 = (b / p.ntx) * TY;
     const int sample = blockIdx.y;
     const int L = p.L, z0 = zc * p.ZC, ZC = p.ZC;
@@ -183,6 +203,7 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
         // TY row segments of ROW sites (split in two where the x1 halo wraps), two halo rows of TX/2 sites,
         // and the couplings of a plane are one block of the tile-major array: 11 to 19 bulk copies per step.
         const int lane = tid - Gm::CONSUMERS;
+        const uint64_t pol_last = policy_evict_last();
         const float* const other = spins_grp + (size_t)(1 - p.colour) * p.Nh * SITE_FLOATS;
         const size_t tile_first = (((size_t)(sample * 2 + p.colour) * p.nty + Y0 / TY) * p.ntx + X0 / TX) * L;   // in plane blocks
         const unsigned char* const Jtile = reinterpret_cast<const unsigned char*>(p.Jt) + tile_first * JST;
@@ -209,18 +230,18 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
                     if (e == 0) {
                         // sites X0-1, X0+1, .., X0+TX-1: the first one wraps for the leftmost tile
                         if (X0 == 0) {
-                            bulk_g2s(dst, other + (rowh + (Lh - 1)) * SITE_FLOATS, Gm::SITE_BYTES, full_o(st));
-                            bulk_g2s(dst + Gm::SITE_BYTES, other + (rowh + 0) * SITE_FLOATS, (Gm::ROW - 1) * Gm::SITE_BYTES, full_o(st));
+                            bulk_g2s_hint(dst, other + (rowh + (Lh - 1)) * SITE_FLOATS, Gm::SITE_BYTES, full_o(st), pol_last);
+                            bulk_g2s_hint(dst + Gm::SITE_BYTES, other + (rowh + 0) * SITE_FLOATS, (Gm::ROW - 1) * Gm::SITE_BYTES, full_o(st), pol_last);
                         } else {
-                            bulk_g2s(dst, other + (rowh + ((X0 - 1) >> 1)) * SITE_FLOATS, Gm::ROW * Gm::SITE_BYTES, full_o(st));
+                            bulk_g2s_hint(dst, other + (rowh + ((X0 - 1) >> 1)) * SITE_FLOATS, Gm::ROW * Gm::SITE_BYTES, full_o(st), pol_last);
                         }
                     } else {
                         // sites X0, X0+2, .., X0+TX: the last one wraps for the rightmost tile
                         if (X0 + TX == L) {
-                            bulk_g2s(dst, other + (rowh + (X0 >> 1)) * SITE_FLOATS, (Gm::ROW - 1) * Gm::SITE_BYTES, full_o(st));
-                            bulk_g2s(dst + (Gm::ROW - 1) * Gm::SITE_BYTES, other + rowh * SITE_FLOATS, Gm::SITE_BYTES, full_o(st));
+                            bulk_g2s_hint(dst, other + (rowh + (X0 >> 1)) * SITE_FLOATS, (Gm::ROW - 1) * Gm::SITE_BYTES, full_o(st), pol_last);
+                            bulk_g2s_hint(dst + (Gm::ROW - 1) * Gm::SITE_BYTES, other + rowh * SITE_FLOATS, Gm::SITE_BYTES, full_o(st), pol_last);
                         } else {
-                            bulk_g2s(dst, other + (rowh + (X0 >> 1)) * SITE_FLOATS, Gm::ROW * Gm::SITE_BYTES, full_o(st));
+                            bulk_g2s_hint(dst, other + (rowh + (X0 >> 1)) * SITE_FLOATS, Gm::ROW * Gm::SITE_BYTES, full_o(st), pol_last);
                         }
                     }
                 } else if (lane < TY + 2) {
@@ -229,8 +250,8 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
                     int y = up ? Y0 + TY : Y0 - 1;
                     y = (y < 0) ? y + L : ((y >= L) ? y - L : y);
                     const size_t rowh = (size_t)Lh * (y + (size_t)L * z);
-                    bulk_g2s(dst0 + (TY * Gm::ROW + up * (TX / 2)) * Gm::SITE_BYTES, other + (rowh + (X0 >> 1)) * SITE_FLOATS,
-                             (TX / 2) * Gm::SITE_BYTES, full_o(st));
+                    bulk_g2s_hint(dst0 + (TY * Gm::ROW + up * (TX / 2)) * Gm::SITE_BYTES, other + (rowh + (X0 >> 1)) * SITE_FLOATS,
+                             (TX / 2) * Gm::SITE_BYTES, full_o(st), pol_last);
                 }
             }
             // coupling blocks of step k = n - 2: one contiguous block of the tile-major array
@@ -255,7 +276,7 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
                     if (k >= NJ) mbar_wait(empty_j(st), ((k / NJ) - 1) & 1);
                     if (lane == 0) {
                         mbar_expect_tx(full_j(st), JST);
-                        bulk_g2s(smem_u32(jring + (size_t)st * JST), Jtile + (size_t)(z0 + k) * JST, JST, full_j(st));
+                        bulk_g2s_hint(smem_u32(jring + (size_t)st * JST), Jtile + (size_t)(z0 + k) * JST, JST, full_j(st), pol_last);
                     }
                     __syncwarp();
                 }
@@ -381,7 +402,7 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
             double acc = 0.0;
             for (int r = 0; r < Gm::OWN; ++r) acc += red[r * (G + 1) + tid];
             const int nblk = p.ntx * p.nty * p.nzc;
-            const int blk = blockIdx.x / p.NG;
+            const int blk = blk_;
             p.Epart[((size_t)(sample * p.NG + grp) * nblk + blk) * G + tid] = acc;
         }
     }
