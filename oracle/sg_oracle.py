@@ -269,18 +269,24 @@ def logbin_index(n):
     return i
 
 
-def logbin_observables(e, q0, qk):
-    """The per (sample, temperature) observables O that are binned, [S][T][4], from one measurement (e [S][R][T],
-    q0 [S][P][T], qk [S][P][T][3][2]): mean over replicas of e; mean over pairs of q0^2; mean over pairs and the three
-    k_min directions of |q(k_mu)|^2 (the chi(0), chi(k_min) estimators of Eq. (3), PAPER.md:87-91, up to the factor N);
-    mean over pairs of q0^4.  No replica pair (R = 1): the three overlap entries are 0."""
+def logbin_observables(e, q0, qk, qc0=None, qck=None):
+    """The per (sample, temperature) observables O that are binned, [S][T][6], from one measurement (e [S][R][T],
+    q0 [S][P][T], qk [S][P][T][3][2]; optionally the chiral-glass overlaps qc0 [S][P][T][3], qck [S][P][T][3][3][2]):
+    O[0] mean over replicas of e; O[1] mean over pairs of q0^2; O[2] mean over pairs and the three k_min directions of
+    |q(k_mu)|^2 (the chi(0), chi(k_min) estimators of Eq. (3), up to the factor N); O[3] mean over pairs
+    of q0^4; O[4] mean over pairs and the chirality direction mu of q_CG^mu(0)^2; O[5] mean over pairs, mu and the three
+    k_min directions nu of |q_CG^mu(k_nu)|^2 ("we averaged over all the values of mu", parallel and orthogonal to k_min,
+    PAPER.md:97).  No replica pair (R = 1): the overlap entries are 0.  Without qc0 / qck: O[4] = O[5] = 0."""
     S, R, T = e.shape
-    out = np.zeros((S, T, 4))
+    out = np.zeros((S, T, 6))
     out[..., 0] = e.mean(axis=1)
     if q0.shape[1] > 0:
         out[..., 1] = (q0 ** 2).mean(axis=1)
         out[..., 2] = (qk ** 2).sum(axis=-1).mean(axis=-1).mean(axis=1)
         out[..., 3] = (q0 ** 4).mean(axis=1)
+        if qc0 is not None:
+            out[..., 4] = (qc0 ** 2).mean(axis=-1).mean(axis=1)
+            out[..., 5] = (qck ** 2).sum(axis=-1).mean(axis=(-1, -2)).mean(axis=1)
     return out
 
 
@@ -322,8 +328,9 @@ class OracleSim:
         self.walk_label = np.zeros((self.S, self.R, self.T), dtype=np.int32)
         self.round_trips = np.zeros((self.S, self.R, 1), dtype=np.uint64)
         self.n_acc = 0
-        self.logbin_sums = np.zeros((LOGBINS, self.S, self.T, 4))
+        self.logbin_sums = np.zeros((LOGBINS, self.S, self.T, 6))
         self.logbin_counts = np.zeros(LOGBINS, dtype=np.uint64)
+        self.logbin_counts_cg = np.zeros(LOGBINS, dtype=np.uint64)
 
     def g0(self, sample):
         return (self.first_sample + sample) * self.C
@@ -406,12 +413,16 @@ class OracleSim:
                     qk[s, p, t] = o[1:].reshape(3, 2)
         return e, q0, qk
 
-    def accumulate(self):
-        """Measure and add into the logarithmic bins: the n-th call goes to bin logbin_index(n)."""
+    def accumulate(self, with_chirality=False):
+        """Measure and add into the logarithmic bins: the n-th call goes to bin logbin_index(n); the
+        chiral-glass entries O[4], O[5] only with `with_chirality` (their own count per bin)."""
         self.n_acc += 1
         b = logbin_index(self.n_acc)
-        self.logbin_sums[b] += logbin_observables(*self.measure())
+        cg = self.measure_chiral() if with_chirality else (None, None)
+        self.logbin_sums[b] += logbin_observables(*self.measure(), *cg)
         self.logbin_counts[b] += 1
+        if with_chirality:
+            self.logbin_counts_cg[b] += 1
 
     def measure_chiral(self):
         """qc0[S][P][T][3], qck[S][P][T][3][3][2]: chiral-glass overlaps of the replica pairs a<b with both

@@ -351,12 +351,16 @@ def test_logbin_observables_by_hand(oracle):
     R = 3: means over the three pairs.  R = 1: no overlap entries."""
     e = np.array([[[1.0], [3.0]]]); q0 = np.array([[[0.5]]])
     qk = np.zeros((1, 1, 1, 3, 2)); qk[0, 0, 0, 0] = (3.0, 4.0); qk[0, 0, 0, 2] = (0.0, 1.0)
-    assert np.allclose(oracle.logbin_observables(e, q0, qk)[0, 0], [2.0, 0.25, 26.0 / 3.0, 0.0625], rtol=0, atol=1e-15)
+    assert np.allclose(oracle.logbin_observables(e, q0, qk)[0, 0], [2.0, 0.25, 26.0 / 3.0, 0.0625, 0.0, 0.0], rtol=0, atol=1e-15)
+    # chiral-glass entries: q_CG^mu(0) = (1, 2, 3) -> (1 + 4 + 9)/3; q_CG^mu(k_nu): two non-zero entries 3+4i (mu=0, nu=1), 2 (mu=2, nu=2)
+    # -> (25 + 4)/9
+    qc0 = np.array([[[[1.0, 2.0, 3.0]]]]); qck = np.zeros((1, 1, 1, 3, 3, 2)); qck[0, 0, 0, 0, 1] = (3.0, 4.0); qck[0, 0, 0, 2, 2, 0] = 2.0
+    assert np.allclose(oracle.logbin_observables(e, q0, qk, qc0, qck)[0, 0, 4:], [14.0 / 3.0, 29.0 / 9.0], rtol=0, atol=1e-15)
     e3 = np.array([[[1.0], [2.0], [6.0]]]); q3 = np.array([[[1.0], [2.0], [3.0]]])
     qk3 = np.zeros((1, 3, 1, 3, 2)); qk3[0, 1, 0, 1, 0] = 3.0
-    assert np.allclose(oracle.logbin_observables(e3, q3, qk3)[0, 0], [3.0, 14.0 / 3.0, 1.0, 98.0 / 3.0], rtol=0, atol=1e-14)
+    assert np.allclose(oracle.logbin_observables(e3, q3, qk3)[0, 0, :4], [3.0, 14.0 / 3.0, 1.0, 98.0 / 3.0], rtol=0, atol=1e-14)
     assert np.array_equal(oracle.logbin_observables(np.ones((2, 1, 3)), np.zeros((2, 0, 3)), np.zeros((2, 0, 3, 3, 2)))[..., 1:],
-                          np.zeros((2, 3, 3)))
+                          np.zeros((2, 3, 5)))
 
 
 def test_accumulate_bins_a_recorded_series(oracle):
@@ -368,10 +372,11 @@ def test_accumulate_bins_a_recorded_series(oracle):
     rec = []
     for _ in range(15):
         sim.unit(2)
-        rec.append(oracle.logbin_observables(*sim.measure()))
-        sim.accumulate()
+        rec.append(oracle.logbin_observables(*sim.measure(), *sim.measure_chiral()))
+        sim.accumulate(with_chirality=True)
     rec = np.array(rec)
-    assert sim.n_acc == 15 and list(sim.logbin_counts[:5]) == [1, 2, 4, 8, 0]
+    assert sim.n_acc == 15 and list(sim.logbin_counts[:5]) == [1, 2, 4, 8, 0] and np.array_equal(sim.logbin_counts_cg, sim.logbin_counts)
+    assert (rec[..., 4] > 0).all() and (rec[..., 5] > 0).all()
     for i, (lo, hi) in enumerate([(0, 1), (1, 3), (3, 7), (7, 15)]):
         assert np.allclose(sim.logbin_sums[i], rec[lo:hi].sum(axis=0), rtol=0, atol=1e-13)
     assert not sim.logbin_sums[4:].any()
