@@ -129,15 +129,20 @@ int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk);
 /* Logarithmic data binning on the device (Sect. III: "Each bin had twice the
  * length of the previous ... i_f contains the last half of the Monte Carlo time series, i_f - 1 the second quarter").
  * sg_accumulate measures as sg_measure does (energies recomputed if stale, overlaps of all replica pairs) and adds, per
- * (sample, temperature), four observables into bin floor(log2 n) of the n-th call since creation (n = 1, 2, ...):
+ * (sample, temperature), the observables below into bin floor(log2 n) of the n-th call since creation (n = 1, 2, ...):
  *   O[0] = mean over replicas of e,  O[1] = mean over pairs of q^(0)^2,  O[2] = mean over pairs and the three k_min
- *   directions of |q^(k_mu)|^2 (Eq. (3) up to the factor N),  O[3] = mean over pairs of q^(0)^4   (0 when R = 1).
+ *   directions of |q^(k_mu)|^2 (Eq. (3) up to the factor N),  O[3] = mean over pairs of q^(0)^4   (0 when R = 1);
+ *   with_chirality != 0 also (as sg_measure_chiral measures them; "we averaged over all the values of mu")
+ *   O[4] = mean over pairs and mu of q^_CG^mu(0)^2,  O[5] = mean over pairs, mu and the three k_min directions nu of
+ *   |q^_CG^mu(k_nu)|^2.   chi = N <O>, xi by sg_correlation_length(L, <O[1]>, <O[2]>) resp. (L, <O[4]>, <O[5]>).
  * ASYNCHRONOUS on the stream: nothing crosses to the host.  fp64 sums in call order.  Errors: SG_EINVAL, SG_ESTATE.
- * sg_get_logbins: sums double [SG_LOGBINS][S][T][4], counts uint64 [SG_LOGBINS] (calls that fell into each bin; the
- * bin average is sums / counts); host outputs, either may be NULL; synchronises. */
+ * sg_get_logbins: sums double [SG_LOGBINS][S][T][SG_LOGBIN_OBS]; counts uint64 [SG_LOGBINS] = calls that fell into each
+ * bin, counts_cg = those of them made with chirality (the divisor of O[4], O[5]); host outputs, any may be NULL;
+ * synchronises. */
 #define SG_LOGBINS 32
-int sg_accumulate(sg_ctx* ctx);
-int sg_get_logbins(sg_ctx* ctx, double* sums, uint64_t* counts);
+#define SG_LOGBIN_OBS 6
+int sg_accumulate(sg_ctx* ctx, int with_chirality);
+int sg_get_logbins(sg_ctx* ctx, double* sums, uint64_t* counts, uint64_t* counts_cg);
 
 /* Chiral-glass overlaps (Sect. II.B, Eq. (2)):
  *   zeta_{x,mu}  = s_{x+e_mu} . (s_x x s_{x-e_mu}),  kappa_{x,mu} = zeta^a_{x,mu} zeta^b_{x,mu}

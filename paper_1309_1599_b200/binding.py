@@ -13,7 +13,7 @@ GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2,
 KIND_OR, KIND_HB = 0, 1
 SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
 TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES, TUNE_PACKED = 0, 1, 2, 3
-LOGBINS = 32
+LOGBINS, LOGBIN_OBS = 32, 6
 SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT = 0, 1, 2, 3
 
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
@@ -77,8 +77,8 @@ def load_library():
     L.sg_set_counters.argtypes = [vp, u64, u64]; L.sg_set_counters.restype = i
     L.sg_halfsweep.argtypes = [vp, i, i]; L.sg_halfsweep.restype = i
     L.sg_pt_stats.argtypes = [vp, vp, vp]; L.sg_pt_stats.restype = i
-    L.sg_accumulate.argtypes = [vp]; L.sg_accumulate.restype = i
-    L.sg_get_logbins.argtypes = [vp, vp, vp]; L.sg_get_logbins.restype = i
+    L.sg_accumulate.argtypes = [vp, i]; L.sg_accumulate.restype = i
+    L.sg_get_logbins.argtypes = [vp, vp, vp, vp]; L.sg_get_logbins.restype = i
     L.sg_pt_walk.argtypes = [vp, vp, vp]; L.sg_pt_walk.restype = i
     L.sg_tune.argtypes = [vp, i, i]; L.sg_tune.restype = i
     L.sg_sync.argtypes = [vp]; L.sg_sync.restype = i
@@ -272,15 +272,16 @@ class SpinGlass:
         self._check(self._lib.sg_pt_stats(self._ctx, _ptr(att), _ptr(acc)), "sg_pt_stats")
         return att, acc
 
-    def accumulate(self):
+    def accumulate(self, with_chirality=False):
         """Measure and add into the device-side logarithmic bins; asynchronous."""
-        self._check(self._lib.sg_accumulate(self._ctx), "sg_accumulate")
+        self._check(self._lib.sg_accumulate(self._ctx, int(bool(with_chirality))), "sg_accumulate")
 
     def get_logbins(self):
-        """(sums float64 [LOGBINS][S][T][4], counts uint64 [LOGBINS])."""
-        sums = np.zeros((LOGBINS, self.S, self.T, 4)); counts = np.zeros(LOGBINS, dtype=np.uint64)
-        self._check(self._lib.sg_get_logbins(self._ctx, _ptr(sums), _ptr(counts)), "sg_get_logbins")
-        return sums, counts
+        """(sums float64 [LOGBINS][S][T][LOGBIN_OBS], counts uint64 [LOGBINS], counts_cg uint64 [LOGBINS])."""
+        sums = np.zeros((LOGBINS, self.S, self.T, LOGBIN_OBS)); counts = np.zeros(LOGBINS, dtype=np.uint64)
+        counts_cg = np.zeros(LOGBINS, dtype=np.uint64)
+        self._check(self._lib.sg_get_logbins(self._ctx, _ptr(sums), _ptr(counts), _ptr(counts_cg)), "sg_get_logbins")
+        return sums, counts, counts_cg
 
     def pt_walk(self):
         """(round_trips uint64 [S][R], label int32 [S][R][T]) of the random walk in temperature."""

@@ -27,6 +27,7 @@ struct sg_ctx {
     unsigned long long* attempts; unsigned long long* accepts;
     int* walk_label; unsigned long long* round_trips;
     double* logbin; uint64_t n_acc;
+    uint64_t n_acc_cg[SG_LOGBINS];   // calls with chirality per bin
     // sweep geometry
     int tile_sites, ntiles, log2L;
     // z-marching sweep (L a multiple of 8): tuning knobs and the derived chunking
@@ -119,7 +120,7 @@ Offsets offsets(const Geometry& g)
     o.acc = c.take(st);
     o.wlab = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     o.trips = c.take((size_t)g.S * g.R * sizeof(unsigned long long));
-    o.logbin = c.take((size_t)SG_LOGBINS * g.S * g.T * 4 * sizeof(double));
+    o.logbin = c.take((size_t)SG_LOGBINS * g.S * g.T * SG_LOGBIN_OBS * sizeof(double));
     o.total = c.off;
     return o;
 }
@@ -506,6 +507,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->attempts = (unsigned long long*)(base + o.att); ctx->accepts = (unsigned long long*)(base + o.acc);
     ctx->walk_label = (int*)(base + o.wlab); ctx->round_trips = (unsigned long long*)(base + o.trips);
     ctx->logbin = (double*)(base + o.logbin); ctx->n_acc = 0;
+    for (int b = 0; b < SG_LOGBINS; ++b) ctx->n_acc_cg[b] = 0;
     ctx->h_betas.assign(betas, betas + g.T);
     ctx->inited.assign(g.S, 0);
     ctx->bimodal_D.assign(g.S, std::nan("")); ctx->packed_on = 0;
@@ -534,7 +536,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->accepts, 0, st, ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->walk_label, 0, (size_t)g.S * g.R * g.T * sizeof(int), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->round_trips, 0, (size_t)g.S * g.R * sizeof(unsigned long long), ctx->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->logbin, 0, (size_t)SG_LOGBINS * g.S * g.T * 4 * sizeof(double), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->logbin, 0, (size_t)SG_LOGBINS * g.S * g.T * SG_LOGBIN_OBS * sizeof(double), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->E, 0, (size_t)g.S * g.Cp * sizeof(double), ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // the host vectors above go out of scope
     if (e != cudaSuccess) { delete ctx; return SG_ECUDA; }
@@ -773,7 +775,9 @@ int sg_measure(sg_ctx* ctx, double* e, double* q0, double* qk)
     return SG_OK;
 }
 
-int sg_accumulate(sg_ctx* ctx)
+static int launch_measure_chiral(sg_ctx* ctx);
+
+int sg_accumulate(sg_ctx* ctx, int with_chirality)
 {
     if (!ctx) return SG_EINVAL;
     if (int rc = launch_measure(ctx, true)) return rc;
@@ -781,13 +785,22 @@ int sg_accumulate(sg_ctx* ctx)
     int b = 0;
     while (b + 1 < SG_LOGBINS && (n >> (b + 1)) != 0) ++b;
     const int items = ctx->S * ctx->T;
-    k_logbin_add<<<(items + 127) / 128, 128, 0, ctx->stream>>>(ctx->result, ctx->logbin + (size_t)b * items * 4, ctx->S, ctx->R, ctx->T, ctx->P);
+    double* bin = ctx->logbin + (size_t)b * items * SG_LOGBIN_OBS;
+    k_logbin_add<<<(items + 127) / 128, 128, 0, ctx->stream>>>(ctx->result, bin, ctx->S, ctx->R, ctx->T, ctx->P);
     SG_LAUNCHED(ctx);
+    if (with_chirality) {
+        if (ctx->P > 0) {     // the result buffer is reused: stream order keeps the two passes apart
+            if (int rc = launch_measure_chiral(ctx)) return rc;
+            k_logbin_add_chiral<<<(items + 127) / 128, 128, 0, ctx->stream>>>(ctx->result, bin, ctx->S, ctx->T, ctx->P);
+            SG_LAUNCHED(ctx);
+        }
+        ctx->n_acc_cg[b] += 1;
+    }
     ctx->n_acc = n;
     return SG_OK;
 }
 
-int sg_get_logbins(sg_ctx* ctx, double* sums, uint64_t* counts)
+int sg_get_logbins(sg_ctx* ctx, double* sums, uint64_t* counts, uint64_t* counts_cg)
 {
     if (!ctx) return SG_EINVAL;
     if (counts) {
@@ -796,18 +809,18 @@ int sg_get_logbins(sg_ctx* ctx, double* sums, uint64_t* counts)
             counts[b] = (ctx->n_acc < lo) ? 0 : ((ctx->n_acc < hi ? ctx->n_acc + 1 : hi) - lo);
         }
     }
-    if (sums) SG_CUDA(ctx, cudaMemcpyAsync(sums, ctx->logbin, (size_t)SG_LOGBINS * ctx->S * ctx->T * 4 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    if (counts_cg)
+        for (int b = 0; b < SG_LOGBINS; ++b) counts_cg[b] = ctx->n_acc_cg[b];
+    if (sums) SG_CUDA(ctx, cudaMemcpyAsync(sums, ctx->logbin, (size_t)SG_LOGBINS * ctx->S * ctx->T * SG_LOGBIN_OBS * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
 }
 
-int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck)
+// chiral-glass overlaps into ctx->result = [ qc0 | qck ] (asynchronous); requires P*T > 0
+static int launch_measure_chiral(sg_ctx* ctx)
 {
-    if (!ctx) return SG_EINVAL;
-    if (int rc = all_inited(ctx)) return rc;
     const int PT = ctx->P * ctx->T;
     const int nQ = ctx->S * PT;
-    if (PT == 0) return SG_OK;
     ChiralParams p;
     p.spins = ctx->spins; p.slot_of_temp = ctx->slot_of_temp; p.phase = ctx->phase; p.Mpart = ctx->Mpart;
     p.L = ctx->L; p.N = ctx->N; p.NG = ctx->NG; p.Cp = ctx->Cp; p.R = ctx->R; p.T = ctx->T; p.P = ctx->P;
@@ -822,6 +835,17 @@ int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck)
     SG_LAUNCHED(ctx);
     k_reduce_chiral<<<(nQ * 21 + 127) / 128, 128, 0, ctx->stream>>>(ctx->Mpart, ctx->result, ctx->S, PT, ctx->nchunk, ctx->N);
     SG_LAUNCHED(ctx);
+    return SG_OK;
+}
+
+int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck)
+{
+    if (!ctx) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    const int PT = ctx->P * ctx->T;
+    const int nQ = ctx->S * PT;
+    if (PT == 0) return SG_OK;
+    if (int rc = launch_measure_chiral(ctx)) return rc;
     {
         int rc;
         if (const double* h = fetch_result(ctx, (size_t)nQ * 21, &rc)) {

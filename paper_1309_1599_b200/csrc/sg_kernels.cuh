@@ -418,7 +418,7 @@ __global__ void k_reduce_measure(const double* __restrict__ Mpart, const double*
 }
 
 // Logarithmic data binning (Sect. III): adds the observables of one measurement (the `result` of
-// k_reduce_measure) into bin[S][T][4]: mean over replicas of e, mean over pairs of q0^2, mean over pairs and the
+// k_reduce_measure) into bin[S][T][6] (entries 0-3): mean over replicas of e, mean over pairs of q0^2, mean over pairs and the
 // three k_min directions of |q(k_mu)|^2, mean over pairs of q0^4.  Thread = (sample, temperature); fp64, fixed order.
 __global__ void k_logbin_add(const double* __restrict__ result, double* __restrict__ bin, int S, int R, int T, int P)
 {
@@ -440,8 +440,31 @@ __global__ void k_logbin_add(const double* __restrict__ result, double* __restri
         qk2 += m / 3.0;
     }
     if (P > 0) { q2 /= (double)P; qk2 /= (double)P; q4 /= (double)P; }
-    double* o = bin + (size_t)u * 4;
+    double* o = bin + (size_t)u * 6;
     o[0] += e; o[1] += q2; o[2] += qk2; o[3] += q4;
+}
+
+// The chiral-glass entries 4, 5 of the same bins from the `result` of k_reduce_chiral ([ qc0[S][P][T][3] | qck[S][P][T][3][3][2] ]):
+// mean over pairs and mu of q_CG^mu(0)^2; mean over pairs, mu and the three k_min directions of |q_CG^mu(k_nu)|^2.
+__global__ void k_logbin_add_chiral(const double* __restrict__ result, double* __restrict__ bin, int S, int T, int P)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= S * T || P == 0) return;
+    const int sample = u / T, t = u % T;
+    const int PT = P * T;
+    const size_t nQ = (size_t)S * PT;
+    double c0 = 0.0, ck = 0.0;
+    for (int pr = 0; pr < P; ++pr) {
+        const size_t item = (size_t)sample * PT + (size_t)pr * T + t;
+        const double* a = result + item * 3;
+        c0 += (a[0] * a[0] + a[1] * a[1] + a[2] * a[2]) / 3.0;
+        const double* k = result + nQ * 3 + item * 18;
+        double m = 0.0;
+        for (int j = 0; j < 18; ++j) m += k[j] * k[j];
+        ck += m / 9.0;
+    }
+    double* o = bin + (size_t)u * 6;
+    o[4] += c0 / (double)P; o[5] += ck / (double)P;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -168,15 +168,18 @@ def test_logbins_match_oracle(sg, oracle, sh):
         for s in range(S):
             gpu.set_spins(s, sim.spins[s].astype(np.float32))
             gpu.set_perm(s, sim.temp_of_slot[s])
-        gpu.accumulate()
-        sim.accumulate()
-    sums, counts = gpu.get_logbins()
+        gpu.accumulate(with_chirality=(n % 2 == 0))         # chirality on every other call: its own count per bin
+        sim.accumulate(with_chirality=(n % 2 == 0))
+    sums, counts, counts_cg = gpu.get_logbins()
     assert list(counts[:5]) == [1, 2, 4, 4, 0] and np.array_equal(counts, sim.logbin_counts)
+    assert list(counts_cg[:5]) == [1, 1, 2, 2, 0] and np.array_equal(counts_cg, sim.logbin_counts_cg)
     scale = np.maximum(1.0, np.abs(sim.logbin_sums))
     assert (np.abs(sums - sim.logbin_sums) <= 4 * TOL * scale).all()          # <= 4 measurements of 1e-6 each per bin
     assert not sums[4:].any()
     if R > 1:
-        assert (sums[:4, :, :, 1:] > 0).all()                                # the comparison is not vacuous
+        assert (sums[:4, :, :, 1:4] > 0).all()                               # the comparison is not vacuous
+        if L > 2:
+            assert (sums[:4, :, :, 4:] > 0).all()
     else:
         assert not sums[..., 1:].any()
     e, _, _ = gpu.measure()                                                    # sg_measure still serves after sg_accumulate
