@@ -46,8 +46,14 @@ typedef struct {
     int32_t n_temps;      /* T >= 1 */
     int32_t first_sample; /* global number of local sample 0 (enters every Philox counter; lets ranks
                              shard the samples and still draw the single-process numbers) */
-    int32_t reserved;     /* must be 0 */
-    uint64_t seed;        /* Philox key */
+    int32_t first_replica;     /* global number of local replica 0 (replica sharding of one sample, see n_replicas_total) */
+    int32_t n_replicas_total;  /* replicas of the whole job; 0 = n_replicas (no replica sharding).  A context that holds the
+                                  replicas [first_replica, first_replica + n_replicas) of every sample draws exactly the numbers
+                                  (initial spins, heat bath, PT) a single context holding all n_replicas_total would: the PT chains
+                                  of a sample are per replica, so its replicas can live on different GPUs with no
+                                  exchange inside the Monte Carlo; overlaps are measured between the replicas a context holds */
+    int32_t reserved;          /* must be 0 */
+    uint64_t seed;             /* Philox key */
 } sg_shape;
 
 enum {

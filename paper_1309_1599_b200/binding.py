@@ -28,7 +28,8 @@ DECLARED_SYMBOLS = [
 
 class SgShape(ctypes.Structure):
     _fields_ = [("L", ctypes.c_int32), ("n_samples", ctypes.c_int32), ("n_replicas", ctypes.c_int32),
-                ("n_temps", ctypes.c_int32), ("first_sample", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("n_temps", ctypes.c_int32), ("first_sample", ctypes.c_int32), ("first_replica", ctypes.c_int32),
+                ("n_replicas_total", ctypes.c_int32), ("reserved", ctypes.c_int32),
                 ("seed", ctypes.c_uint64)]
 
 
@@ -99,7 +100,7 @@ def _ptr(a):
 
 
 def workspace_bytes(L, n_samples, n_replicas, n_temps, seed=0, first_sample=0):
-    shape = SgShape(L, n_samples, n_replicas, n_temps, first_sample, 0, seed)
+    shape = SgShape(L, n_samples, n_replicas, n_temps, first_sample, 0, 0, 0, seed)
     return int(load_library().sg_workspace_bytes(ctypes.byref(shape)))
 
 
@@ -118,12 +119,13 @@ def philox4x32_10(ctr, key):
 class SpinGlass:
     """One context of the C-ABI library on the current CUDA device and torch's current stream."""
 
-    def __init__(self, L, n_samples, n_replicas, n_temps, betas, seed=1, first_sample=0, device=None, stream=None):
+    def __init__(self, L, n_samples, n_replicas, n_temps, betas, seed=1, first_sample=0, device=None, stream=None,
+                 first_replica=0, n_replicas_total=0):
         import torch
         self._lib = load_library()
         self.L, self.S, self.R, self.T = int(L), int(n_samples), int(n_replicas), int(n_temps)
         self.N, self.C, self.P = self.L ** 3, self.R * self.T, self.R * (self.R - 1) // 2
-        self.shape = SgShape(self.L, self.S, self.R, self.T, int(first_sample), 0, int(seed))
+        self.shape = SgShape(self.L, self.S, self.R, self.T, int(first_sample), int(first_replica), int(n_replicas_total), 0, int(seed))
         nbytes = int(self._lib.sg_workspace_bytes(ctypes.byref(self.shape)))
         if nbytes == 0:
             raise SgError(SG_EINVAL, "sg_workspace_bytes")

@@ -17,6 +17,8 @@ using namespace sg;
 struct sg_ctx {
     sg_shape shape;
     int L, N, Nh, S, R, T, C, NG, Cp, P;
+    int Rt, Cg;           // replicas / copies per sample of the whole job (replica sharding; = R, C otherwise)
+    uint32_t g_first;     // global copy id of (local sample 0, local copy 0)
     cudaStream_t stream;
     // device arrays (carved from the caller's workspace)
     float* spins; float* Jg; float* Jt; unsigned char* Jp; float* Mraw; float* staging; float* beta_slot;
@@ -57,7 +59,9 @@ bool shape_ok(const sg_shape* s)
     if (!s) return false;
     if (s->L < 2 || (s->L & 1) || s->L > 1024) return false;
     if (s->n_samples <= 0 || s->n_replicas <= 0 || s->n_temps <= 0 || s->first_sample < 0) return false;
-    if (s->reserved != 0) return false;
+    if (s->reserved != 0 || s->first_replica < 0) return false;
+    if (s->n_replicas_total != 0 && s->first_replica + s->n_replicas > s->n_replicas_total) return false;
+    if (s->n_replicas_total == 0 && s->first_replica != 0) return false;
     const double N = (double)s->L * s->L * s->L;
     const double C = (double)s->n_replicas * s->n_temps;
     if (N > 2.0e9 || C > 1.0e6) return false;
@@ -289,7 +293,7 @@ int half_sweep_zm(sg_ctx* ctx, int kind, int colour, bool with_energy)
     p.colour = colour;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.hb_counter = (uint32_t)ctx->hb_counter;
-    p.g_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->C;
+    p.g_first = ctx->g_first; p.Cg = ctx->Cg;
     const int nblk = p.ntx * p.nty * p.nzc;
     const dim3 grid(nblk * ctx->NG, ctx->S);
     int rc;
@@ -318,7 +322,7 @@ int half_sweep(sg_ctx* ctx, int kind, int colour, bool with_energy)
     p.tile_sites = ctx->tile_sites; p.colour = colour; p.C = ctx->C;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.hb_counter = (uint32_t)ctx->hb_counter;
-    p.g_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->C;
+    p.g_first = ctx->g_first; p.Cg = ctx->Cg;
     const dim3 grid(ctx->ntiles * ctx->NG, ctx->S);
     if (kind == KIND_OR) {
         if (with_energy) launch_sweep_l<KIND_OR, true>(ctx, p, grid);
@@ -434,7 +438,7 @@ int sweeps_resident(sg_ctx* ctx, int kind, int n_sweeps)
     p.n_sweeps = n_sweeps;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.hb_counter = (uint32_t)ctx->hb_counter;
-    p.g_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->C;
+    p.g_first = ctx->g_first; p.Cg = ctx->Cg;
     if (int rc = (kind == KIND_HB) ? launch_res<1>(ctx, p) : launch_res<0>(ctx, p)) return rc;
     SG_LAUNCHED(ctx);
     if (kind == KIND_HB) ctx->hb_counter += (uint64_t)n_sweeps;
@@ -488,6 +492,8 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->shape = *shape;
     ctx->L = g.L; ctx->N = g.N; ctx->Nh = g.Nh; ctx->S = g.S; ctx->R = g.R; ctx->T = g.T; ctx->C = g.C;
     ctx->NG = g.NG; ctx->Cp = g.Cp; ctx->P = g.P;
+    ctx->Rt = shape->n_replicas_total ? shape->n_replicas_total : g.R; ctx->Cg = ctx->Rt * g.T;
+    ctx->g_first = (uint32_t)shape->first_sample * (uint32_t)ctx->Cg + (uint32_t)shape->first_replica * (uint32_t)g.T;
     ctx->tile_sites = g.tile_sites; ctx->ntiles = g.ntiles; ctx->log2L = ilog2_exact(g.L);
     ctx->nchunk = g.nchunk; ctx->chunk_sites = g.chunk_sites; ctx->MS = g.MS;
     ctx->stream = (cudaStream_t)cuda_stream;
@@ -614,7 +620,7 @@ int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const 
         if (int rc = sg_set_spins(ctx, sample, spins)) return rc;
     } else {
         const size_t nthr = (size_t)ctx->NG * ctx->N * 8;
-        const uint32_t g_sample = (uint32_t)(ctx->shape.first_sample + sample) * (uint32_t)ctx->C;
+        const uint32_t g_sample = ctx->g_first + (uint32_t)sample * (uint32_t)ctx->Cg;
         k_init_spins<<<(unsigned)((nthr + 255) / 256), 256, 0, ctx->stream>>>(
             ctx->spins + (size_t)sample * ctx->NG * ctx->N * SITE_FLOATS, ctx->L, ctx->N, ctx->NG, ctx->C, g_sample,
             (uint32_t)(ctx->shape.seed & 0xffffffffu), (uint32_t)(ctx->shape.seed >> 32));
@@ -706,7 +712,7 @@ int sg_pt_swap(sg_ctx* ctx)
     p.S = ctx->S; p.R = ctx->R; p.T = ctx->T; p.Cp = ctx->Cp;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.pt_counter = (uint32_t)ctx->pt_counter;
-    p.chain_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->R;
+    p.chain_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->Rt + (uint32_t)ctx->shape.first_replica; p.Rt = ctx->Rt;
     const int chains = ctx->S * ctx->R;
     k_pt_swap<<<(chains + 63) / 64, 64, 0, ctx->stream>>>(p);
     SG_LAUNCHED(ctx);

@@ -26,6 +26,7 @@ struct SweepParams {
     int L, N, Nh, NG, ntiles, tile_sites;
     int colour;
     int C;                   // copies per sample (R*T); Cp = NG*G
+    int Cg;                  // copies per sample of the whole job (all replicas, sg_shape.n_replicas_total): stride of the global copy id
     uint32_t key0, key1, hb_counter;
     uint32_t g_first;        // global copy id of (local sample 0, copy 0) = first_sample*C
 };
@@ -109,7 +110,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS) k_sweep(const SweepParams p)
             }
         } else if (KIND == KIND_HB) {
             const float bt[4] = { beta4.x, beta4.y, beta4.z, beta4.w };
-            const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.C + (uint32_t)(grp * G + q * 4);
+            const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.Cg + (uint32_t)(grp * G + q * 4);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 uint32_t w[4];
@@ -271,8 +272,8 @@ struct PtParams {
     unsigned long long* accepts;
     int* walk_label;                 // [S][R][T]: 0 = no end touched yet, 1 = last touched index 0, 2 = last touched index T-1
     unsigned long long* round_trips; // [S][R]: completed walks 0 -> T-1 -> 0, summed over the chain's configurations
-    int S, R, T, Cp;
-    uint32_t key0, key1, pt_counter, chain_first;   // chain id of (local sample 0, r = 0) = first_sample*R
+    int S, R, T, Cp, Rt;   // Rt: replicas of the whole job (sg_shape.n_replicas_total)
+    uint32_t key0, key1, pt_counter, chain_first;   // chain id of (local sample 0, r = 0) = first_sample*Rt + first_replica
 };
 
 __global__ void k_pt_swap(const PtParams p)
@@ -288,7 +289,7 @@ __global__ void k_pt_swap(const PtParams p)
         const int i = sot[t], j = sot[t + 1];
         const double delta = (p.betas[t] - p.betas[t + 1]) * (E[i] - E[j]);
         uint32_t w[4];
-        philox4x32_10((uint32_t)t, p.chain_first + (uint32_t)chain, p.pt_counter, STREAM_PT, p.key0, p.key1, w);
+        philox4x32_10((uint32_t)t, p.chain_first + (uint32_t)(sample * p.Rt + r), p.pt_counter, STREAM_PT, p.key0, p.key1, w);
         const double rr = ((double)(w[0] >> 9) + 0.5) * (1.0 / 8388608.0);
         const bool accept = (delta >= 0.0) || (rr < exp(delta));
         p.attempts[(size_t)chain * (p.T - 1) + t] += 1ull;

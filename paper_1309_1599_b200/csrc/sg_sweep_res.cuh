@@ -24,7 +24,7 @@ struct ResParams {
     const float* Jg;         // [S][2][Nh][JG]
     const float* beta_slot;  // [S][Cp]
     double* E;               // [S][Cp]: total H of every slot, written by the last half-sweep
-    int L, N, Nh, NG, C, Cp;
+    int L, N, Nh, NG, C, Cp, Cg;   // Cg: copies per sample of the whole job (stride of the global copy id)
     int n_sweeps;
     uint32_t key0, key1, hb_counter, g_first;
 };
@@ -54,7 +54,7 @@ __global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
     float* const sp = lat + q * 4;
     float4 beta4 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (KIND_ == 1) beta4 = ldg4(p.beta_slot + (size_t)sample * p.Cp + c_first + q * 4);
-    const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.C + (uint32_t)(c_first + q * 4);
+    const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.Cg + (uint32_t)(c_first + q * 4);
     float eacc[4] = { 0.f, 0.f, 0.f, 0.f };
 
     for (int sw = 0; sw < p.n_sweeps; ++sw) {

@@ -106,7 +106,7 @@ struct ZmParams {
     float bimA, bimB, bimD;  // fl32(1 + D), fl32(1 - D), fl32(D) of the packed couplings
     const float* beta_slot;  // [S][Cp]
     double* Epart;           // [S][NG][nblk][G]
-    int L, N, Nh, NG, C;
+    int L, N, Nh, NG, C, Cg; // Cg: copies per sample of the whole job (stride of the global copy id)
     int ntx, nty, nzc, ZC;   // tiles along x1, x2; chunks along x3 of ZC planes each
     int colour;
     uint32_t key0, key1, hb_counter, g_first;
@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
     const int Y = Y0 + ky;
     float4 beta4 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (KIND == KIND_HB) beta4 = ldg4(p.beta_slot + (size_t)sample * p.NG * G + grp * G + q * 4);
-    const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.C + (uint32_t)(grp * G + q * 4);
+    const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.Cg + (uint32_t)(grp * G + q * 4);
     float eacc[4] = { 0.f, 0.f, 0.f, 0.f };
 
     // Own spin of step k: site (X0 + 2 kx + off, Y, z0 + k), off = (ky + z + colour) & 1.  In the colour-split

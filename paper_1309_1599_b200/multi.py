@@ -20,6 +20,36 @@ def first_sample_of_rank(rank, samples_per_rank):
     return rank * samples_per_rank
 
 
+def replica_window_of_rank(rank, world_size, n_replicas_total, min_replicas=2):
+    """(first_replica, n_replicas) of rank `rank` when the replicas of every sample are sharded over the ranks
+    (sg_shape.first_replica / n_replicas_total): the PT chains of a sample are per replica, so whole
+    chains live on one GPU and the Monte Carlo needs no exchange; a rank keeps at least `min_replicas` replicas so
+    that it can measure overlaps among its own (the paper uses two replicas per sample).  Contiguous,
+    disjoint windows that cover [0, n_replicas_total); world_size must divide n_replicas_total."""
+    if world_size <= 0 or not 0 <= rank < world_size:
+        raise ValueError("0 <= rank < world_size required")
+    if n_replicas_total % world_size != 0 or n_replicas_total // world_size < min_replicas:
+        raise ValueError("world_size must divide n_replicas_total and leave at least min_replicas replicas per rank")
+    n = n_replicas_total // world_size
+    return rank * n, n
+
+
+def gather_overlaps(local, world_size, device="cpu"):
+    """All ranks' arrays of per-pair overlaps, concatenated along the pair axis in rank order: local is a float64
+    array [S][P_local][...]; returns [S][world_size * P_local][...] on every rank (the only data-path collective of
+    the replica-sharded run: a few KB per measurement)."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    local = np.ascontiguousarray(local, dtype=np.float64)
+    if world_size == 1 or not (dist.is_available() and dist.is_initialized()):
+        return local
+    t = torch.from_numpy(local).to(device)
+    parts = [torch.empty_like(t) for _ in range(world_size)]
+    dist.all_gather(parts, t)
+    return np.concatenate([x.cpu().numpy() for x in parts], axis=1)
+
+
 def init_process_group(backend, world_size):
     """Joins the torchrun rendezvous (MASTER_ADDR / MASTER_PORT from the environment) when world_size > 1."""
     import torch.distributed as dist

@@ -54,7 +54,7 @@ def test_workspace_bytes_and_shape_validation(lib):
 
 def test_create_rejects_bad_arguments_without_a_device(lib):
     from paper_1309_1599_b200 import binding
-    shape = binding.SgShape(4, 1, 2, 4, 0, 0, 1)
+    shape = binding.SgShape(4, 1, 2, 4, 0, 0, 0, 0, 1)
     ctx = ctypes.c_void_p()
     betas = np.array([0.6, 0.9, 1.2, 1.6])
     fake = ctypes.c_void_p(256 * 1000)
@@ -68,7 +68,12 @@ def test_create_rejects_bad_arguments_without_a_device(lib):
     assert call(shape, bp(np.array([0.6, 0.9, 0.9, 1.6])), fake, big) == binding.SG_EINVAL         # not strictly monotone
     assert call(shape, bp(np.array([0.6, np.nan, 1.2, 1.6])), fake, big) == binding.SG_EINVAL
     assert call(shape, bp(np.array([0.6, 1.2, 0.9, 1.6])), fake, big) == binding.SG_EINVAL
-    assert call(binding.SgShape(3, 1, 2, 4, 0, 0, 1), bp(betas), fake, big) == binding.SG_EINVAL
+    assert call(binding.SgShape(3, 1, 2, 4, 0, 0, 0, 0, 1), bp(betas), fake, big) == binding.SG_EINVAL
+    # replica sharding: the window [first_replica, first_replica + n_replicas) must lie inside n_replicas_total
+    assert call(binding.SgShape(4, 1, 2, 4, 0, 3, 4, 0, 1), bp(betas), fake, big) == binding.SG_EINVAL
+    assert call(binding.SgShape(4, 1, 2, 4, 0, 1, 0, 0, 1), bp(betas), fake, big) == binding.SG_EINVAL
+    assert call(binding.SgShape(4, 1, 2, 4, 0, -1, 4, 0, 1), bp(betas), fake, big) == binding.SG_EINVAL
+    assert call(binding.SgShape(4, 1, 2, 4, 0, 0, 0, 7, 1), bp(betas), fake, big) == binding.SG_EINVAL   # reserved != 0
     assert ctx.value is None
     for fn in (lib.sg_sweep_or, lib.sg_sweep_hb):
         assert fn(None, 1) == binding.SG_EINVAL

@@ -470,3 +470,33 @@ def test_run_units_equals_the_three_calls(sg):
         assert np.array_equal(a.get_spins(s), b.get_spins(s))
         assert np.array_equal(a.get_perm(s)[0], b.get_perm(s)[0])
     assert np.array_equal(a.get_energies(), b.get_energies()) and a.get_counters() == b.get_counters() == (7, 7)
+
+
+@pytest.mark.parametrize("L,S,T,impl", [(8, 2, 5, 2), (6, 1, 7, 1), (4, 2, 4, 0), (16, 1, 20, 0)])
+def test_replica_shards_draw_the_single_context_numbers(sg, L, S, T, impl):
+    """sg_shape.first_replica / n_replicas_total: two contexts holding replicas (0, 1) and (2, 3) of every sample against
+    one context holding all four: initial spins, three units (HB draws by global copy id, PT by global chain id), spins,
+    permutations, energies and PT statistics of every replica identical bit for bit; overlaps of the local pairs too."""
+    betas = np.linspace(0.5, 2.0, T)
+    def run(R, first_replica, total):
+        gpu = sg.SpinGlass(L, S, R, T, betas, seed=77, first_sample=3, first_replica=first_replica, n_replicas_total=total)
+        gpu.tune(sg.TUNE_SWEEP_IMPL, impl)
+        for s in range(S):
+            gpu.init_sample(s, sg.GEN_OFFDIAG_SYM, 1.0)
+        start = np.stack([gpu.get_spins(s) for s in range(S)])
+        for _ in range(3):
+            gpu.unit(2)
+        e, q0, qk = gpu.measure()
+        out = dict(start=start.reshape(S, R, T, 3, -1), spins=np.stack([gpu.get_spins(s) for s in range(S)]).reshape(S, R, T, 3, -1),
+                   perm=np.stack([gpu.get_perm(s)[0] for s in range(S)]), E=gpu.get_energies().reshape(S, R, T),
+                   acc=gpu.pt_stats()[1], e=e, q0=q0)
+        gpu.close()
+        return out
+    whole = run(4, 0, 0)
+    lo, hi = run(2, 0, 4), run(2, 2, 4)
+    for key in ("start", "spins", "perm", "E", "acc", "e"):
+        assert np.array_equal(whole[key][:, 0:2], lo[key]), key
+        assert np.array_equal(whole[key][:, 2:4], hi[key]), key
+    # pairs in the order (0,1),(0,2),(0,3),(1,2),(1,3),(2,3): the shards hold the first and the last
+    assert np.array_equal(whole["q0"][:, 0], lo["q0"][:, 0]) and np.array_equal(whole["q0"][:, 5], hi["q0"][:, 0])
+    assert whole["acc"].sum() > 0

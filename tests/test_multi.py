@@ -24,7 +24,11 @@ def _worker(rank, world, port, out):
     first = multi.first_sample_of_rank(rank, 4)
     seconds = 1.0 + rank                       # rank 1 is the slow one
     rate, total, slowest = multi.whole_job_rate(100.0 * (rank + 1), seconds)
-    out.put((rank, first, multi.max_over_ranks(seconds), multi.sum_over_ranks(first), rate, total, slowest))
+    import numpy as np
+    window = multi.replica_window_of_rank(rank, world, 4)
+    q = multi.gather_overlaps(np.full((3, 1, 5), float(rank)), world)       # [S][P_local][T] of this rank's one pair
+    out.put((rank, first, multi.max_over_ranks(seconds), multi.sum_over_ranks(first), rate, total, slowest, window,
+             q.shape, q[:, :, 0].tolist()))
     multi.barrier()
     import torch.distributed as dist
     dist.destroy_process_group()
@@ -45,6 +49,8 @@ def test_two_rank_gloo_sharding_and_reduction():
     for g in got:
         assert g[2] == 2.0 and g[3] == 4.0                     # max / sum agree on every rank
         assert g[5] == 300.0 and g[6] == 2.0 and g[4] == 150.0  # all units / slowest rank
+        assert g[8] == (3, 2, 5) and g[9] == [[0.0, 1.0]] * 3   # every rank sees both ranks' pairs, in rank order
+    assert [g[7] for g in got] == [(0, 2), (2, 2)]             # replica windows: disjoint, contiguous, two replicas each
 
 
 def test_single_process_passthrough():
@@ -53,3 +59,8 @@ def test_single_process_passthrough():
     assert multi.first_sample_of_rank(3, 4) == 12
     with pytest.raises(ValueError):
         multi.first_sample_of_rank(-1, 4)
+    assert multi.replica_window_of_rank(0, 1, 4) == (0, 4) and multi.replica_window_of_rank(1, 2, 4) == (2, 2)
+    assert multi.replica_window_of_rank(2, 4, 4, min_replicas=1) == (2, 1)
+    for bad in ((0, 4, 4), (0, 3, 4), (2, 2, 4)):               # one replica per rank, not a divisor, rank out of range
+        with pytest.raises(ValueError):
+            multi.replica_window_of_rank(*bad)
