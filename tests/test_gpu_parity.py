@@ -500,3 +500,34 @@ def test_replica_shards_draw_the_single_context_numbers(sg, L, S, T, impl):
     # pairs in the order (0,1),(0,2),(0,3),(1,2),(1,3),(2,3): the shards hold the first and the last
     assert np.array_equal(whole["q0"][:, 0], lo["q0"][:, 0]) and np.array_equal(whole["q0"][:, 5], hi["q0"][:, 0])
     assert whole["acc"].sum() > 0
+
+
+@pytest.mark.parametrize("L,S,R,T,impl", [(8, 2, 2, 6, 2), (6, 2, 3, 5, 1), (4, 1, 2, 4, 0)])
+def test_checkpoint_resume_is_bit_exact(sg, L, S, R, T, impl):
+    """Philox is counter-based, so the chain's state is (couplings, spins, temperature permutation, HB and PT counters):
+    a second context restored from those through the state hooks continues exactly as the first one does."""
+    betas = np.linspace(0.5, 2.0, T)
+    a = sg.SpinGlass(L, S, R, T, betas, seed=5, first_sample=2)
+    a.tune(sg.TUNE_SWEEP_IMPL, impl)
+    for s in range(S):
+        a.init_sample(s, sg.GEN_OFFDIAG_SYM, 1.0)
+    for _ in range(3):
+        a.unit(3)
+    snap = dict(M=[a.get_couplings(s) for s in range(S)], spins=[a.get_spins(s) for s in range(S)],
+                perm=[a.get_perm(s)[0] for s in range(S)], ctr=a.get_counters())
+    assert snap["ctr"] == (3, 3)
+    for _ in range(3):
+        a.unit(3)
+    b = sg.SpinGlass(L, S, R, T, betas, seed=5, first_sample=2)
+    b.tune(sg.TUNE_SWEEP_IMPL, impl)
+    for s in range(S):
+        b.init_sample(s, couplings=snap["M"][s], spins=snap["spins"][s])
+        b.set_perm(s, snap["perm"][s])
+    b.set_counters(*snap["ctr"])
+    for _ in range(3):
+        b.unit(3)
+    assert a.get_counters() == b.get_counters() == (6, 6)
+    for s in range(S):
+        assert np.array_equal(a.get_spins(s), b.get_spins(s))
+        assert np.array_equal(a.get_perm(s)[0], b.get_perm(s)[0]) and np.array_equal(a.get_perm(s)[1], b.get_perm(s)[1])
+    assert np.array_equal(a.get_energies(), b.get_energies())
