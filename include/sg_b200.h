@@ -160,6 +160,18 @@ int sg_get_logbins(sg_ctx* ctx, double* sums, uint64_t* counts, uint64_t* counts
  * Synchronises the stream.  Errors: SG_EINVAL (ctx NULL), SG_ESTATE (a sample not initialised), SG_ECUDA. */
 int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck);
 
+/* Overlaps between replicas held by different contexts (replica sharding: sg_shape.first_replica; q_x = s^a_x . s^b_x,
+ * q^(k) as in sg_measure).
+ * sg_export_replica: the configurations of local replica r ordered by TEMPERATURE, float [S][3][N][T] (temperature index
+ *   fastest, site index i lexicographic), written to the DEVICE buffer dev_out (caller-owned, S*3*N*T floats; e.g. the
+ *   send buffer of an all-gather over NVLink).  Asynchronous on the stream.
+ * sg_measure_cross: between local replica r (through its own temperature permutation) and such a device buffer of a
+ *   partner replica (same sample numbers, same temperatures): q0 double [S][T], qk double [S][T][3][2] (Re, Im), host
+ *   outputs, either may be NULL.  fp32 products, fp64 sums in a fixed order.  Synchronises.
+ * Errors: SG_EINVAL (NULL, r out of range, T > 256 for sg_measure_cross), SG_ESTATE, SG_ECUDA. */
+int sg_export_replica(sg_ctx* ctx, int r, void* dev_out);
+int sg_measure_cross(sg_ctx* ctx, int r, const void* dev_remote, double* q0, double* qk);
+
 /* Schwinger-Dyson monitor (App. A.4, Eq. (A6)):
  *   2 T <s_x.h_x> - <(h_x)^2 - (s_x.h_x)^2> = 0 in equilibrium, "averaged over all the sites in the lattice".
  *   sd double [S][R][T][2]   sd[..][0] = sum_x s_x.h_x / N,  sd[..][1] = sum_x [h_x.h_x - (s_x.h_x)^2] / N

@@ -29,6 +29,7 @@ struct sg_ctx {
     unsigned long long* attempts; unsigned long long* accepts;
     int* walk_label; unsigned long long* round_trips;
     double* logbin; uint64_t n_acc;
+    double* Xpart;
     uint64_t n_acc_cg[SG_LOGBINS];   // calls with chirality per bin
     // sweep geometry
     int tile_sites, ntiles, log2L;
@@ -96,7 +97,7 @@ struct Carve {
 };
 
 struct Offsets {
-    size_t spins, Jg, Jt, Jp, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, logbin, total;
+    size_t spins, Jg, Jt, Jp, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, logbin, xpart, total;
 };
 
 Offsets offsets(const Geometry& g)
@@ -116,7 +117,7 @@ Offsets offsets(const Geometry& g)
     o.SDpart = c.take((size_t)g.S * g.NG * 2 * g.ntiles * G * 2 * sizeof(double));
     o.phase = c.take((size_t)g.L * 2 * sizeof(double));
     o.Mpart = c.take((size_t)g.S * g.nchunk * (g.P * g.T > 0 ? g.P * g.T : 1) * 21 * sizeof(double));   // 7 per item (overlap), 21 (chirality)
-    o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + 1) * sizeof(double));
+    o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + (size_t)g.S * g.T * 7 + 1) * sizeof(double));
     o.sot = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     o.tos = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     size_t st = (size_t)g.S * g.R * (g.T > 1 ? g.T - 1 : 1) * sizeof(unsigned long long);
@@ -125,6 +126,7 @@ Offsets offsets(const Geometry& g)
     o.wlab = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     o.trips = c.take((size_t)g.S * g.R * sizeof(unsigned long long));
     o.logbin = c.take((size_t)SG_LOGBINS * g.S * g.T * SG_LOGBIN_OBS * sizeof(double));
+    o.xpart = c.take((size_t)g.S * XCHUNKS * XTHREADS * 7 * sizeof(double));   // rows * T <= XTHREADS when T <= XTHREADS
     o.total = c.off;
     return o;
 }
@@ -504,7 +506,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->SDpart = (double*)(base + o.SDpart);
     ctx->phase = (double*)(base + o.phase); ctx->Mpart = (double*)(base + o.Mpart);
     ctx->result = (double*)(base + o.result);
-    ctx->result_doubles = (size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + 1;
+    ctx->result_doubles = (size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + (size_t)g.S * g.T * 7 + 1;
     if (cudaHostAlloc((void**)&ctx->h_result, ctx->result_doubles * sizeof(double), cudaHostAllocDefault) != cudaSuccess) {
         ctx->h_result = nullptr;   // fall back to direct copies into the caller's arrays
         cudaGetLastError();
@@ -513,6 +515,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->attempts = (unsigned long long*)(base + o.att); ctx->accepts = (unsigned long long*)(base + o.acc);
     ctx->walk_label = (int*)(base + o.wlab); ctx->round_trips = (unsigned long long*)(base + o.trips);
     ctx->logbin = (double*)(base + o.logbin); ctx->n_acc = 0;
+    ctx->Xpart = (double*)(base + o.xpart);
     for (int b = 0; b < SG_LOGBINS; ++b) ctx->n_acc_cg[b] = 0;
     ctx->h_betas.assign(betas, betas + g.T);
     ctx->inited.assign(g.S, 0);
@@ -863,6 +866,37 @@ int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck)
     }
     if (qc0) SG_CUDA(ctx, cudaMemcpyAsync(qc0, ctx->result, (size_t)nQ * 3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (qck) SG_CUDA(ctx, cudaMemcpyAsync(qck, ctx->result + (size_t)nQ * 3, (size_t)nQ * 18 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_export_replica(sg_ctx* ctx, int r, void* dev_out)
+{
+    if (!ctx || !dev_out || r < 0 || r >= ctx->R) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    const size_t n = (size_t)ctx->N * ctx->T;
+    k_export_by_temp<<<dim3((unsigned)((n + 255) / 256), ctx->S), 256, 0, ctx->stream>>>(ctx->spins, ctx->slot_of_temp, (float*)dev_out, ctx->L,
+                                                                                      ctx->N, ctx->NG, ctx->R, ctx->T, r);
+    SG_LAUNCHED(ctx);
+    return SG_OK;
+}
+
+int sg_measure_cross(sg_ctx* ctx, int r, const void* dev_remote, double* q0, double* qk)
+{
+    if (!ctx || !dev_remote || r < 0 || r >= ctx->R || ctx->T > XTHREADS) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    CrossParams p;
+    p.spins = ctx->spins; p.slot_of_temp = ctx->slot_of_temp; p.remote = (const float*)dev_remote; p.phase = ctx->phase; p.Xpart = ctx->Xpart;
+    p.L = ctx->L; p.N = ctx->N; p.NG = ctx->NG; p.R = ctx->R; p.T = ctx->T; p.r = r;
+    const int rows = XTHREADS / ctx->T;
+    k_overlap_cross<<<dim3(XCHUNKS, ctx->S), XTHREADS, 0, ctx->stream>>>(p);
+    SG_LAUNCHED(ctx);
+    const int total = ctx->S * ctx->T * 7;
+    k_reduce_cross<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->Xpart, ctx->result, ctx->S, ctx->T, XCHUNKS * rows, ctx->N);
+    SG_LAUNCHED(ctx);
+    const size_t nQ = (size_t)ctx->S * ctx->T;
+    if (q0) SG_CUDA(ctx, cudaMemcpyAsync(q0, ctx->result, nQ * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    if (qk) SG_CUDA(ctx, cudaMemcpyAsync(qk, ctx->result + nQ, nQ * 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
 }

@@ -418,6 +418,83 @@ __global__ void k_reduce_measure(const double* __restrict__ Mpart, const double*
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Overlaps between replicas held by DIFFERENT contexts (replica sharding; q_x = s^a_x . s^b_x,
+// PAPER.md:79).  k_export_by_temp writes the configurations of local replica r ordered by temperature,
+// out[sample][a][i][t] (t fastest), so that the partner needs no permutation; k_overlap_cross forms, per temperature,
+// the sums of q_x and q_x e^{i 2 pi x_mu / L} between local replica r (through its own permutation) and such a
+// buffer.  Thread = (site row, temperature): private fp64 sums, partials reduced in a fixed order by k_reduce_cross.
+// ------------------------------------------------------------------------------------------------
+__global__ void k_export_by_temp(const float* __restrict__ spins, const int* __restrict__ slot_of_temp, float* __restrict__ out,
+                                 int L, int N, int NG, int R, int T, int r)
+{
+    const int sample = blockIdx.y;
+    const size_t f = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // (site, temperature), temperature fastest
+    if (f >= (size_t)N * T) return;
+    const int i = (int)(f / T), t = (int)(f - (size_t)i * T);
+    const int c = r * T + slot_of_temp[((size_t)sample * R + r) * T + t];
+    const float* src = spins + (((size_t)sample * NG + c / G) * N + site_slot(i, L, N >> 1)) * SITE_FLOATS + (c % G);
+    float* dst = out + (size_t)sample * 3 * N * T + f;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) dst[(size_t)a * N * T] = src[a * G];
+}
+
+constexpr int XCHUNKS = 128, XTHREADS = 256;     // k_overlap_cross: site chunks per sample, threads per CTA
+
+struct CrossParams {
+    const float* spins;        // [S][NG][2][Nh][3][G]
+    const int* slot_of_temp;   // [S][R][T]
+    const float* remote;       // [S][3][N][T] by temperature (k_export_by_temp of the partner)
+    const double* phase;       // [L][2]
+    double* Xpart;             // [S][XCHUNKS * rows][T][7]
+    int L, N, NG, R, T, r;
+};
+
+__global__ void __launch_bounds__(XTHREADS) k_overlap_cross(const CrossParams p)
+{
+    const int chunk = blockIdx.x, sample = blockIdx.y;
+    const int Tw = min(p.T, XTHREADS), rows = XTHREADS / Tw;
+    const int tx = threadIdx.x % Tw, row = threadIdx.x / Tw;
+    if (row >= rows) return;
+    const int per = (p.N + XCHUNKS - 1) / XCHUNKS;
+    const int i_begin = chunk * per, i_end = min(p.N, i_begin + per);
+    const float* base = p.spins + (size_t)sample * p.NG * p.N * SITE_FLOATS;
+    const float* rem = p.remote + (size_t)sample * 3 * p.N * p.T;
+    const size_t plane = (size_t)p.N * p.T;
+    for (int t = tx; t < p.T; t += Tw) {
+        const int c = p.r * p.T + p.slot_of_temp[((size_t)sample * p.R + p.r) * p.T + t];
+        const float* loc = base + (size_t)(c / G) * p.N * SITE_FLOATS + (c % G);
+        double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };
+        for (int i = i_begin + row; i < i_end; i += rows) {
+            const float* s = loc + site_slot(i, p.L, p.N >> 1) * SITE_FLOATS;
+            const size_t f = (size_t)i * p.T + t;
+            const float qf = fmaf(s[0], rem[f], fmaf(s[G], rem[plane + f], s[2 * G] * rem[2 * plane + f]));
+            const double qx = (double)qf;
+            const int x = i % p.L, y = (i / p.L) % p.L, z = i / (p.L * p.L);
+            acc[0] += qx;
+            acc[1] = fma(qx, p.phase[2 * x], acc[1]); acc[2] = fma(qx, p.phase[2 * x + 1], acc[2]);
+            acc[3] = fma(qx, p.phase[2 * y], acc[3]); acc[4] = fma(qx, p.phase[2 * y + 1], acc[4]);
+            acc[5] = fma(qx, p.phase[2 * z], acc[5]); acc[6] = fma(qx, p.phase[2 * z + 1], acc[6]);
+        }
+        double* dst = p.Xpart + ((((size_t)sample * XCHUNKS + chunk) * rows + row) * p.T + t) * 7;
+#pragma unroll
+        for (int k = 0; k < 7; ++k) dst[k] = acc[k];
+    }
+}
+
+// result = [ q0[S][T] | qk[S][T][3][2] ]
+__global__ void k_reduce_cross(const double* __restrict__ Xpart, double* __restrict__ result, int S, int T, int nparts, int N)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= S * T * 7) return;
+    const int k = u % 7, t = (u / 7) % T, sample = u / (7 * T);
+    double acc = 0.0;
+    for (int c = 0; c < nparts; ++c) acc += Xpart[(((size_t)sample * nparts + c) * T + t) * 7 + k];
+    acc /= (double)N;
+    if (k == 0) result[(size_t)sample * T + t] = acc;
+    else result[(size_t)S * T + ((size_t)sample * T + t) * 6 + (k - 1)] = acc;
+}
+
 // Logarithmic data binning (Sect. III): adds the observables of one measurement (the `result` of
 // k_reduce_measure) into bin[S][T][6] (entries 0-3): mean over replicas of e, mean over pairs of q0^2, mean over pairs and the
 // three k_min directions of |q(k_mu)|^2, mean over pairs of q0^4.  Thread = (sample, temperature); fp64, fixed order.

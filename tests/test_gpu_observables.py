@@ -184,3 +184,46 @@ def test_logbins_match_oracle(sg, oracle, sh):
         assert not sums[..., 1:].any()
     e, _, _ = gpu.measure()                                                    # sg_measure still serves after sg_accumulate
     assert np.abs(e - sim.measure()[0]).max() <= TOL * max(1.0, np.abs(e).max())
+
+
+# ---------------------------------------------------------------------------------------------
+# sg_export_replica / sg_measure_cross: overlaps between replicas held by different contexts (replica sharding)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,S,T", [(4, 1, 4), (6, 2, 10), (8, 2, 16), (10, 1, 37)])
+def test_cross_context_overlaps(sg, oracle, L, S, T):
+    """Two contexts with replicas (0, 1) and (2, 3) of the same samples, evolved for three units (non-trivial temperature
+    permutations): the exported configurations are the spins reordered by temperature, bit for bit; the cross overlaps of
+    every pair (a local, b remote) equal the oracle's overlap of the two configurations at that temperature (<= 1e-6) and
+    what a single context holding all four replicas measures for the pair (summation order only)."""
+    betas = np.linspace(0.5, 2.0, T)
+    N = L ** 3
+    def make(R, first, total):
+        g = sg.SpinGlass(L, S, R, T, betas, seed=31, first_replica=first, n_replicas_total=total)
+        for s in range(S):
+            g.init_sample(s)
+        for _ in range(3):
+            g.unit(2)
+        return g
+    lo, hi, whole = make(2, 0, 4), make(2, 2, 4), make(4, 0, 0)
+    _, q0_w, qk_w = whole.measure()
+    pair_index = {(a, b): k for k, (a, b) in enumerate(oracle.replica_pairs(4))}
+    spins = {g: [g.get_spins(s).reshape(2, T, 3, N) for s in range(S)] for g in (lo, hi)}
+    perms = {g: [g.get_perm(s)[1] for s in range(S)] for g in (lo, hi)}           # slot_of_temp [R][T]
+    assert any((perms[g][s] != np.arange(T)).any() for g in (lo, hi) for s in range(S))
+    for b in range(2):
+        buf = hi.export_replica(b)
+        host = buf.cpu().numpy()                                                   # [S][3][N][T]
+        for s in range(S):
+            want = spins[hi][s][b][perms[hi][s][b]]                                # [T][3][N] by temperature
+            assert np.array_equal(host[s], want.transpose(1, 2, 0))
+        for a in range(2):
+            q0, qk = lo.measure_cross(a, buf)
+            k = pair_index[(a, b + 2)]
+            assert np.abs(q0 - q0_w[:, k]).max() <= 1e-12 and np.abs(qk - qk_w[:, k]).max() <= 1e-12
+            for s in range(S):
+                for t in range(0, T, max(1, T // 5)):
+                    o = oracle.overlap(L, spins[lo][s][a][perms[lo][s][a][t]].astype(np.float64),
+                                       spins[hi][s][b][perms[hi][s][b][t]].astype(np.float64))
+                    assert abs(o[0] - q0[s, t]) <= TOL and np.abs(o[1:].reshape(3, 2) - qk[s, t]).max() <= TOL
+    for g in (lo, hi, whole):
+        g.close()

@@ -15,6 +15,31 @@ def _free_port():
         return s.getsockname()[1]
 
 
+class _FakeShard:
+    """Stands in for a replica-sharded SpinGlass in the orchestration test: 'configurations' are tensors filled with the
+    global replica number, an 'overlap' of replicas a, b is 10 a + b (so who was paired with whom is visible)."""
+    S, T = 2, 3
+
+    def __init__(self, rank, n_local):
+        self.rank, self.n = rank, n_local
+
+    def measure(self):
+        import numpy as np
+        pairs = [(a, b) for a in range(self.n) for b in range(a + 1, self.n)]
+        v = np.array([10.0 * (self.rank * self.n + a) + (self.rank * self.n + b) for a, b in pairs])
+        q0 = np.broadcast_to(v[None, :, None], (self.S, len(pairs), self.T)).copy()
+        return None, q0, np.broadcast_to(q0[..., None, None], q0.shape + (3, 2)).copy()
+
+    def export_replica(self, r):
+        import torch
+        return torch.full((self.S, 3, 4, self.T), float(self.rank * self.n + r))
+
+    def measure_cross(self, a, buf):
+        import numpy as np
+        v = 10.0 * (self.rank * self.n + a) + float(buf[0, 0, 0, 0])
+        return np.full((self.S, self.T), v), np.full((self.S, self.T, 3, 2), v)
+
+
 def _worker(rank, world, port, out):
     os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
                       MASTER_PORT=str(port))
@@ -27,8 +52,9 @@ def _worker(rank, world, port, out):
     import numpy as np
     window = multi.replica_window_of_rank(rank, world, 4)
     q = multi.gather_overlaps(np.full((3, 1, 5), float(rank)), world)       # [S][P_local][T] of this rank's one pair
+    q0_all, qk_all = multi.measure_all_pairs(_FakeShard(rank, 2), rank, world, 2)
     out.put((rank, first, multi.max_over_ranks(seconds), multi.sum_over_ranks(first), rate, total, slowest, window,
-             q.shape, q[:, :, 0].tolist()))
+             q.shape, q[:, :, 0].tolist(), q0_all[0, :, 0].tolist(), qk_all.shape))
     multi.barrier()
     import torch.distributed as dist
     dist.destroy_process_group()
@@ -50,6 +76,8 @@ def test_two_rank_gloo_sharding_and_reduction():
         assert g[2] == 2.0 and g[3] == 4.0                     # max / sum agree on every rank
         assert g[5] == 300.0 and g[6] == 2.0 and g[4] == 150.0  # all units / slowest rank
         assert g[8] == (3, 2, 5) and g[9] == [[0.0, 1.0]] * 3   # every rank sees both ranks' pairs, in rank order
+        # all six pairs of the four replicas, in the global order, each formed from the right two replicas, on every rank
+        assert g[10] == [1.0, 2.0, 3.0, 12.0, 13.0, 23.0] and g[11] == (2, 6, 3, 3, 2)
     assert [g[7] for g in got] == [(0, 2), (2, 2)]             # replica windows: disjoint, contiguous, two replicas each
 
 
@@ -59,6 +87,8 @@ def test_single_process_passthrough():
     assert multi.first_sample_of_rank(3, 4) == 12
     with pytest.raises(ValueError):
         multi.first_sample_of_rank(-1, 4)
+    q0_one, _ = multi.measure_all_pairs(_FakeShard(0, 3), 0, 1, 3)
+    assert q0_one[0, :, 0].tolist() == [1.0, 2.0, 12.0]
     assert multi.replica_window_of_rank(0, 1, 4) == (0, 4) and multi.replica_window_of_rank(1, 2, 4) == (2, 2)
     assert multi.replica_window_of_rank(2, 4, 4, min_replicas=1) == (2, 1)
     for bad in ((0, 4, 4), (0, 3, 4), (2, 2, 4)):               # one replica per rank, not a divisor, rank out of range
