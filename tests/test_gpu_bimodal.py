@@ -133,3 +133,26 @@ def test_mixed_contexts_fall_back_to_the_matrices(sg, oracle):
         gpu.halfsweep(sg.KIND_OR, 0)
         err = np.abs(gpu_spins(gpu) - oracle_spins(sim)).max(axis=2)
         assert np.where(flags != 0, 0.0, err).max() <= SPIN_TOL, second
+
+
+def test_packed_sweep_full_size_lattice(sg):
+    """L = 64 (the headline lattice), 32 copies, the launch shape the bench uses (automatic chunking): packed against
+    matrix sweeps bit for bit, and against the properties that hold at any size (|s| = 1 after HB, OR conserves the energy)."""
+    L, S, R, T, D = 64, 1, 1, 32, 0.5
+    betas = np.linspace(0.5, 2.6, T)
+    out = []
+    for packed in (1, 0):
+        gpu = sg.SpinGlass(L, S, R, T, betas, seed=9)
+        gpu.tune(sg.TUNE_PACKED, packed)
+        gpu.init_sample_bimodal(0, D)
+        gpu.sweep_hb(1)
+        s1 = gpu.get_spins(0)
+        E1 = gpu.get_energies()
+        gpu.sweep_or(2)
+        out.append((s1, E1, gpu.get_spins(0), gpu.get_energies()))
+        gpu.close()
+    for k in range(4):
+        assert np.array_equal(out[0][k], out[1][k]), k
+    s1, E1, s2, E2 = out[0]
+    assert np.abs(np.linalg.norm(s1.astype(np.float64), axis=1) - 1.0).max() < 1e-6
+    assert np.abs(E2 - E1).max() <= 2e-6 * np.abs(E1).max()          # OR keeps H (fp32 rounding of 2 sweeps)
