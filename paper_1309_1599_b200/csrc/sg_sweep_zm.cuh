@@ -328,15 +328,8 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
     for (int k2 = 0; k2 < ZC; k2 += 2) {
 #pragma unroll
         for (int d = 0; d < 2; ++d) {
-            const int k = k2 + d;
-            if (k >= ZC) break;
+            const int k = k2 + d;      // ZC is even (sg_tune / zm_plan), so k < ZC for both steps of the pair
             float s[3][4];
-#pragma unroll
-            for (int a = 0; a < 3; ++a) { s[a][0] = pre[d][a].x; s[a][1] = pre[d][a].y; s[a][2] = pre[d][a].z; s[a][3] = pre[d][a].w; }
-            if (k + 2 < ZC) {
-#pragma unroll
-                for (int a = 0; a < 3; ++a) pre[d][a] = ld4(own + 2 * plane + a * G);
-            }
             mbar_wait(full_o(sp_), par_p);
             mbar_wait(full_j(sj_), par_j);
             const unsigned char* const Pm = ring + sm_ * Gm::STAGE_BYTES;
@@ -380,10 +373,21 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
             sj_ = (sj_ + 1 == NJ) ? 0 : sj_ + 1; par_j ^= (sj_ == 0) ? 1u : 0u;
 
             const uint32_t i = i0 + (uint32_t)((ky + z0 + d + p.colour) & 1) + (uint32_t)(L * L) * (uint32_t)k;
+            // the own spin is needed only now (s.h and the reflection): take it from the prefetch registers ...
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { s[a][0] = pre[d][a].x; s[a][1] = pre[d][a].y; s[a][2] = pre[d][a].z; s[a][3] = pre[d][a].w; }
             zm_update<KIND, WITH_E>(hf, s, eacc, beta4, i, g0, p);
             if (KIND != KIND_ENERGY) {
 #pragma unroll
                 for (int a = 0; a < 3; ++a) st4(own + a * G, make_float4(s[a][0], s[a][1], s[a][2], s[a][3]));
+            }
+            // ... and refill them for step k + 2 once they are dead: still two field computations ahead of the next use.
+            // Unconditional (a predicated load would force copies of the old values): past the end of the chunk it re-reads
+            // the plane just written, an L2 hit whose value is never used.
+            {
+                const float* const nxt = own + ((k + 2 < ZC) ? 2 * plane : 0);
+#pragma unroll
+                for (int a = 0; a < 3; ++a) pre[d][a] = ld4(nxt + a * G);
             }
             own += plane;
         }
