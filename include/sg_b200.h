@@ -171,6 +171,13 @@ int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck);
  * Errors: SG_EINVAL (NULL, r out of range, T > 256 for sg_measure_cross), SG_ESTATE, SG_ECUDA. */
 int sg_export_replica(sg_ctx* ctx, int r, void* dev_out);
 int sg_measure_cross(sg_ctx* ctx, int r, const void* dev_remote, double* q0, double* qk);
+/* The same for the chiral-glass overlaps (Eq. (2)): sg_export_chirality writes zeta_{x,mu} of local replica r
+ * ordered by temperature, float [S][3][N][T] (mu, site, temperature; temperature fastest) to the device buffer dev_out
+ * (asynchronous); sg_chiral_cross forms kappa = zeta^a zeta^b between two such device buffers (one local, one the partner's):
+ * qc0 double [S][T][3], qck double [S][T][3][3][2] as in sg_measure_chiral, host outputs, either may be NULL; synchronises.
+ * Errors: SG_EINVAL (NULL, r out of range, T > 256), SG_ESTATE, SG_ECUDA. */
+int sg_export_chirality(sg_ctx* ctx, int r, void* dev_out);
+int sg_chiral_cross(sg_ctx* ctx, const void* dev_a, const void* dev_b, double* qc0, double* qck);
 
 /* Schwinger-Dyson monitor (App. A.4, Eq. (A6)):
  *   2 T <s_x.h_x> - <(h_x)^2 - (s_x.h_x)^2> = 0 in equilibrium, "averaged over all the sites in the lattice".

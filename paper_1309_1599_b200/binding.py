@@ -19,7 +19,7 @@ SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT = 0, 1, 2, 3
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_init_sample_bimodal", "sg_sweep_or", "sg_sweep_hb",
-    "sg_pt_swap", "sg_run_units", "sg_measure", "sg_accumulate", "sg_get_logbins", "sg_export_replica", "sg_measure_cross", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
+    "sg_pt_swap", "sg_run_units", "sg_measure", "sg_accumulate", "sg_get_logbins", "sg_export_replica", "sg_measure_cross", "sg_export_chirality", "sg_chiral_cross", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
     "sg_halfsweep", "sg_pt_stats", "sg_pt_walk", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
@@ -82,6 +82,8 @@ def load_library():
     L.sg_get_logbins.argtypes = [vp, vp, vp, vp]; L.sg_get_logbins.restype = i
     L.sg_export_replica.argtypes = [vp, i, vp]; L.sg_export_replica.restype = i
     L.sg_measure_cross.argtypes = [vp, i, vp, vp, vp]; L.sg_measure_cross.restype = i
+    L.sg_export_chirality.argtypes = [vp, i, vp]; L.sg_export_chirality.restype = i
+    L.sg_chiral_cross.argtypes = [vp, vp, vp, vp, vp]; L.sg_chiral_cross.restype = i
     L.sg_pt_walk.argtypes = [vp, vp, vp]; L.sg_pt_walk.restype = i
     L.sg_tune.argtypes = [vp, i, i]; L.sg_tune.restype = i
     L.sg_sync.argtypes = [vp]; L.sg_sync.restype = i
@@ -303,6 +305,24 @@ class SpinGlass:
         self._check(self._lib.sg_measure_cross(self._ctx, int(r), ctypes.c_void_p(remote.data_ptr()), _ptr(q0), _ptr(qk)),
                     "sg_measure_cross")
         return q0, qk
+
+    def export_chirality(self, r, out=None):
+        """Device tensor float32 [S][3][N][T]: zeta_{x,mu} of local replica r ordered by temperature (asynchronous)."""
+        import torch
+        if out is None:
+            out = torch.empty((self.S, 3, self.N, self.T), dtype=torch.float32, device=self.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float32 and out.numel() == self.S * 3 * self.N * self.T
+        self._check(self._lib.sg_export_chirality(self._ctx, int(r), ctypes.c_void_p(out.data_ptr())), "sg_export_chirality")
+        return out
+
+    def chiral_cross(self, za, zb):
+        """(qc0 [S][T][3], qck [S][T][3][3][2]) between two export_chirality tensors (both on this device)."""
+        for z in (za, zb):
+            assert z.is_cuda and z.is_contiguous() and z.numel() == self.S * 3 * self.N * self.T
+        qc0 = np.empty((self.S, self.T, 3)); qck = np.empty((self.S, self.T, 3, 3, 2))
+        self._check(self._lib.sg_chiral_cross(self._ctx, ctypes.c_void_p(za.data_ptr()), ctypes.c_void_p(zb.data_ptr()), _ptr(qc0), _ptr(qck)),
+                    "sg_chiral_cross")
+        return qc0, qck
 
     def pt_walk(self):
         """(round_trips uint64 [S][R], label int32 [S][R][T]) of the random walk in temperature."""

@@ -117,7 +117,7 @@ Offsets offsets(const Geometry& g)
     o.SDpart = c.take((size_t)g.S * g.NG * 2 * g.ntiles * G * 2 * sizeof(double));
     o.phase = c.take((size_t)g.L * 2 * sizeof(double));
     o.Mpart = c.take((size_t)g.S * g.nchunk * (g.P * g.T > 0 ? g.P * g.T : 1) * 21 * sizeof(double));   // 7 per item (overlap), 21 (chirality)
-    o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + (size_t)g.S * g.T * 7 + 1) * sizeof(double));
+    o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + (size_t)g.S * g.T * 21 + 1) * sizeof(double));
     o.sot = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     o.tos = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     size_t st = (size_t)g.S * g.R * (g.T > 1 ? g.T - 1 : 1) * sizeof(unsigned long long);
@@ -126,7 +126,7 @@ Offsets offsets(const Geometry& g)
     o.wlab = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     o.trips = c.take((size_t)g.S * g.R * sizeof(unsigned long long));
     o.logbin = c.take((size_t)SG_LOGBINS * g.S * g.T * SG_LOGBIN_OBS * sizeof(double));
-    o.xpart = c.take((size_t)g.S * XCHUNKS * XTHREADS * 7 * sizeof(double));   // rows * T <= XTHREADS when T <= XTHREADS
+    o.xpart = c.take((size_t)g.S * XCHUNKS * XTHREADS * 21 * sizeof(double));   // rows * T <= XTHREADS when T <= XTHREADS
     o.total = c.off;
     return o;
 }
@@ -506,7 +506,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->SDpart = (double*)(base + o.SDpart);
     ctx->phase = (double*)(base + o.phase); ctx->Mpart = (double*)(base + o.Mpart);
     ctx->result = (double*)(base + o.result);
-    ctx->result_doubles = (size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + (size_t)g.S * g.T * 7 + 1;
+    ctx->result_doubles = (size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + (size_t)g.S * g.T * 21 + 1;
     if (cudaHostAlloc((void**)&ctx->h_result, ctx->result_doubles * sizeof(double), cudaHostAllocDefault) != cudaSuccess) {
         ctx->h_result = nullptr;   // fall back to direct copies into the caller's arrays
         cudaGetLastError();
@@ -897,6 +897,34 @@ int sg_measure_cross(sg_ctx* ctx, int r, const void* dev_remote, double* q0, dou
     const size_t nQ = (size_t)ctx->S * ctx->T;
     if (q0) SG_CUDA(ctx, cudaMemcpyAsync(q0, ctx->result, nQ * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (qk) SG_CUDA(ctx, cudaMemcpyAsync(qk, ctx->result + nQ, nQ * 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+int sg_export_chirality(sg_ctx* ctx, int r, void* dev_out)
+{
+    if (!ctx || !dev_out || r < 0 || r >= ctx->R) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    const size_t n = (size_t)ctx->N * ctx->T;
+    k_export_zeta_by_temp<<<dim3((unsigned)((n + 255) / 256), ctx->S), 256, 0, ctx->stream>>>(ctx->spins, ctx->slot_of_temp, (float*)dev_out,
+                                                                                           ctx->L, ctx->N, ctx->NG, ctx->R, ctx->T, r);
+    SG_LAUNCHED(ctx);
+    return SG_OK;
+}
+
+int sg_chiral_cross(sg_ctx* ctx, const void* dev_a, const void* dev_b, double* qc0, double* qck)
+{
+    if (!ctx || !dev_a || !dev_b || ctx->T > XTHREADS) return SG_EINVAL;
+    const int rows = XTHREADS / ctx->T;
+    k_chiral_cross<<<dim3(XCHUNKS, ctx->S), XTHREADS, 0, ctx->stream>>>((const float*)dev_a, (const float*)dev_b, ctx->phase, ctx->Xpart, ctx->L,
+                                                                       ctx->N, ctx->T);
+    SG_LAUNCHED(ctx);
+    const int total = ctx->S * ctx->T * 21;
+    k_reduce_chiral_cross<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->Xpart, ctx->result, ctx->S, ctx->T, XCHUNKS * rows, ctx->N);
+    SG_LAUNCHED(ctx);
+    const size_t nQ = (size_t)ctx->S * ctx->T;
+    if (qc0) SG_CUDA(ctx, cudaMemcpyAsync(qc0, ctx->result, nQ * 3 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    if (qck) SG_CUDA(ctx, cudaMemcpyAsync(qck, ctx->result + nQ * 3, nQ * 18 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
 }

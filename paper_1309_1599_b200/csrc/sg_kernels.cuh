@@ -495,6 +495,84 @@ __global__ void k_reduce_cross(const double* __restrict__ Xpart, double* __restr
     else result[(size_t)S * T + ((size_t)sample * T + t) * 6 + (k - 1)] = acc;
 }
 
+// The chiral-glass counterpart (Eq. (2)): k_export_zeta_by_temp writes zeta_{x,mu} of local replica r ordered by
+// temperature, out[sample][mu][i][t]; k_chiral_cross forms, per temperature, the 21 sums of kappa_{x,mu} = zeta^a zeta^b and
+// kappa e^{i 2 pi x_nu / L} between two such buffers (either may be the partner's).  Same thread mapping as k_overlap_cross.
+__global__ void k_export_zeta_by_temp(const float* __restrict__ spins, const int* __restrict__ slot_of_temp, float* __restrict__ out,
+                                      int L, int N, int NG, int R, int T, int r)
+{
+    const int sample = blockIdx.y;
+    const size_t f = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // (site, temperature), temperature fastest
+    if (f >= (size_t)N * T) return;
+    const int i = (int)(f / T), t = (int)(f - (size_t)i * T);
+    const int c = r * T + slot_of_temp[((size_t)sample * R + r) * T + t];
+    const float* gb = spins + ((size_t)sample * NG + c / G) * N * SITE_FLOATS + (c % G);
+    const int Nh = N >> 1;
+    const float* c0 = gb + site_slot(i, L, Nh) * SITE_FLOATS;
+    const float bx = c0[0], by = c0[G], bz = c0[2 * G];
+    float* dst = out + (size_t)sample * 3 * N * T + f;
+#pragma unroll
+    for (int mu = 0; mu < 3; ++mu) {
+        const int st = (mu == 0) ? 1 : ((mu == 1) ? L : L * L);
+        const int xm = (mu == 0) ? i % L : ((mu == 1) ? (i / L) % L : i / (L * L));
+        const int ip = (xm + 1 == L) ? i - (L - 1) * st : i + st, im = (xm == 0) ? i + (L - 1) * st : i - st;
+        const float* pa = gb + site_slot(ip, L, Nh) * SITE_FLOATS;   // s_{x+e_mu}
+        const float* pc = gb + site_slot(im, L, Nh) * SITE_FLOATS;   // s_{x-e_mu}
+        const float ax = pa[0], ay = pa[G], az = pa[2 * G];
+        const float cx = pc[0], cy = pc[G], cz = pc[2 * G];
+        dst[(size_t)mu * N * T] = fmaf(ax, fmaf(by, cz, -bz * cy), fmaf(ay, fmaf(bz, cx, -bx * cz), az * fmaf(bx, cy, -by * cx)));
+    }
+}
+
+__global__ void __launch_bounds__(XTHREADS) k_chiral_cross(const float* __restrict__ za, const float* __restrict__ zb, const double* __restrict__ phase,
+                                                           double* __restrict__ Xpart /* [S][XCHUNKS * rows][T][21] */, int L, int N, int T)
+{
+    const int chunk = blockIdx.x, sample = blockIdx.y;
+    const int Tw = min(T, XTHREADS), rows = XTHREADS / Tw;
+    const int tx = threadIdx.x % Tw, row = threadIdx.x / Tw;
+    if (row >= rows) return;
+    const int per = (N + XCHUNKS - 1) / XCHUNKS;
+    const int i_begin = chunk * per, i_end = min(N, i_begin + per);
+    const size_t plane = (size_t)N * T;
+    const float* a = za + (size_t)sample * 3 * plane;
+    const float* b = zb + (size_t)sample * 3 * plane;
+    for (int t = tx; t < T; t += Tw) {
+        double acc[21];
+#pragma unroll
+        for (int k = 0; k < 21; ++k) acc[k] = 0.0;
+        for (int i = i_begin + row; i < i_end; i += rows) {
+            const size_t f = (size_t)i * T + t;
+            const int xs[3] = { i % L, (i / L) % L, i / (L * L) };
+#pragma unroll
+            for (int mu = 0; mu < 3; ++mu) {
+                const double kap = (double)(a[mu * plane + f] * b[mu * plane + f]);
+                acc[mu] += kap;
+#pragma unroll
+                for (int nu = 0; nu < 3; ++nu) {
+                    acc[3 + (mu * 3 + nu) * 2] = fma(kap, phase[2 * xs[nu]], acc[3 + (mu * 3 + nu) * 2]);
+                    acc[4 + (mu * 3 + nu) * 2] = fma(kap, phase[2 * xs[nu] + 1], acc[4 + (mu * 3 + nu) * 2]);
+                }
+            }
+        }
+        double* dst = Xpart + ((((size_t)sample * XCHUNKS + chunk) * rows + row) * T + t) * 21;
+#pragma unroll
+        for (int k = 0; k < 21; ++k) dst[k] = acc[k];
+    }
+}
+
+// result = [ qc0[S][T][3] | qck[S][T][3][3][2] ]
+__global__ void k_reduce_chiral_cross(const double* __restrict__ Xpart, double* __restrict__ result, int S, int T, int nparts, int N)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= S * T * 21) return;
+    const int k = u % 21, t = (u / 21) % T, sample = u / (21 * T);
+    double acc = 0.0;
+    for (int c = 0; c < nparts; ++c) acc += Xpart[(((size_t)sample * nparts + c) * T + t) * 21 + k];
+    acc /= (double)N;
+    if (k < 3) result[((size_t)sample * T + t) * 3 + k] = acc;
+    else result[(size_t)S * T * 3 + ((size_t)sample * T + t) * 18 + (k - 3)] = acc;
+}
+
 // Logarithmic data binning (Sect. III): adds the observables of one measurement (the `result` of
 // k_reduce_measure) into bin[S][T][6] (entries 0-3): mean over replicas of e, mean over pairs of q0^2, mean over pairs and the
 // three k_min directions of |q(k_mu)|^2, mean over pairs of q0^4.  Thread = (sample, temperature); fp64, fixed order.

@@ -50,39 +50,54 @@ def gather_overlaps(local, world_size, device="cpu"):
     return np.concatenate([x.cpu().numpy() for x in parts], axis=1)
 
 
-def measure_all_pairs(gpu, rank, world_size, n_local):
-    """Overlaps of ALL replica pairs a < b of the replica-sharded run (ranks hold n_local consecutive replicas each):
-    pairs inside a rank by sg_measure; a pair across ranks by the rank that holds a, from the configurations of b
-    (ordered by temperature, sg_export_replica) that b's rank broadcasts: one lattice set per (rank, replica) crosses
-    NVLink per measurement, one buffer alive at a time.  `gpu` needs measure(), export_replica(r), measure_cross(r, buf).
-    Returns (q0 [S][P][T], qk [S][P][T][3][2]) on every rank, pairs in the order (0,1),(0,2),...,(R-2,R-1) of the GLOBAL
-    replica numbers, R = world_size * n_local."""
+def _pairs_from_blocks(local_blocks, rank, world_size, n_local, export, cross):
+    """Shared orchestration of measure_all_pairs: `local_blocks` are the per-pair arrays [S][P_local]... of the pairs inside
+    this rank; a pair across ranks is computed by the rank that holds a, from what b's rank exports and broadcasts
+    (one buffer alive at a time).  Returns the arrays stacked over all pairs in the global order, on every rank."""
     import numpy as np
-    import torch
     import torch.distributed as dist
-    _, q0_loc, qk_loc = gpu.measure()
-    mine = {}                                                    # (a, b) global -> (q0 [S][T], qk [S][T][3][2])
+    mine = {}
     k = 0
     for a in range(n_local):
         for b in range(a + 1, n_local):
-            mine[(rank * n_local + a, rank * n_local + b)] = (q0_loc[:, k], qk_loc[:, k])
+            mine[(rank * n_local + a, rank * n_local + b)] = tuple(blk[:, k] for blk in local_blocks)
             k += 1
     if world_size > 1:
         for src in range(1, world_size):                         # rank 0 never sends: nobody holds smaller replicas
             for r in range(n_local):
-                buf = gpu.export_replica(r)                      # every rank fills a buffer of the same shape ...
+                buf = export(r)                                  # every rank fills a buffer of the same shape ...
                 dist.broadcast(buf, src=src)                     # ... and src's overwrites it everywhere
                 if rank < src:
                     for a in range(n_local):
-                        mine[(rank * n_local + a, src * n_local + r)] = gpu.measure_cross(a, buf)
+                        mine[(rank * n_local + a, src * n_local + r)] = tuple(cross(a, buf))
         parts = [None] * world_size
         dist.all_gather_object(parts, mine)
         mine = {key: val for part in parts for key, val in part.items()}
     R = world_size * n_local
     pairs = [(a, b) for a in range(R) for b in range(a + 1, R)]
-    q0 = np.stack([mine[pr][0] for pr in pairs], axis=1)
-    qk = np.stack([mine[pr][1] for pr in pairs], axis=1)
-    return q0, qk
+    return tuple(np.stack([mine[pr][j] for pr in pairs], axis=1) for j in range(len(local_blocks)))
+
+
+def measure_all_pairs(gpu, rank, world_size, n_local, chirality=False):
+    """Overlaps of ALL replica pairs a < b of the replica-sharded run (ranks hold n_local consecutive replicas each):
+    pairs inside a rank by sg_measure; a pair across ranks by the rank that holds a, from the configurations of b
+    (ordered by temperature, sg_export_replica) that b's rank broadcasts: one lattice set per (rank, replica) crosses
+    NVLink per measurement, one buffer alive at a time.  `gpu` needs measure(), export_replica(r), measure_cross(r, buf)
+    (and, with `chirality`, measure_chiral(), export_chirality(r), chiral_cross(za, zb)).
+    Returns (q0 [S][P][T], qk [S][P][T][3][2]) -- with `chirality` also (qc0 [S][P][T][3], qck [S][P][T][3][3][2]) -- on
+    every rank, pairs in the order (0,1),(0,2),...,(R-2,R-1) of the GLOBAL replica numbers, R = world_size * n_local."""
+    _, q0_loc, qk_loc = gpu.measure()
+    out = _pairs_from_blocks((q0_loc, qk_loc), rank, world_size, n_local, gpu.export_replica, gpu.measure_cross)
+    if chirality:
+        local_z = {}
+
+        def cross(a, zb):
+            if a not in local_z:
+                local_z[a] = gpu.export_chirality(a)
+            return gpu.chiral_cross(local_z[a], zb)
+
+        out = out + _pairs_from_blocks(tuple(gpu.measure_chiral()), rank, world_size, n_local, gpu.export_chirality, cross)
+    return out
 
 
 def init_process_group(backend, world_size):

@@ -227,3 +227,37 @@ def test_cross_context_overlaps(sg, oracle, L, S, T):
                     assert abs(o[0] - q0[s, t]) <= TOL and np.abs(o[1:].reshape(3, 2) - qk[s, t]).max() <= TOL
     for g in (lo, hi, whole):
         g.close()
+
+
+@pytest.mark.parametrize("L,S,T", [(4, 1, 4), (6, 2, 10), (8, 1, 16)])
+def test_cross_context_chiral_overlaps(sg, oracle, L, S, T):
+    """sg_export_chirality / sg_chiral_cross between two replica shards against a single four-replica context's
+    sg_measure_chiral for the same pair (summation order only) and against the oracle's chiral overlap (<= 1e-6)."""
+    betas = np.linspace(0.5, 2.0, T)
+    N = L ** 3
+    def make(R, first, total):
+        g = sg.SpinGlass(L, S, R, T, betas, seed=41, first_replica=first, n_replicas_total=total)
+        for s in range(S):
+            g.init_sample(s)
+        for _ in range(3):
+            g.unit(2)
+        return g
+    lo, hi, whole = make(2, 0, 4), make(2, 2, 4), make(4, 0, 0)
+    qc0_w, qck_w = whole.measure_chiral()
+    pair_index = {(a, b): k for k, (a, b) in enumerate(oracle.replica_pairs(4))}
+    spins = {g: [g.get_spins(s).reshape(2, T, 3, N).astype(np.float64) for s in range(S)] for g in (lo, hi)}
+    perms = {g: [g.get_perm(s)[1] for s in range(S)] for g in (lo, hi)}
+    for a in range(2):
+        za = lo.export_chirality(a)
+        for b in range(2):
+            zb = hi.export_chirality(b)
+            qc0, qck = lo.chiral_cross(za, zb)
+            k = pair_index[(a, b + 2)]
+            assert np.abs(qc0 - qc0_w[:, k]).max() <= 1e-12 and np.abs(qck - qck_w[:, k]).max() <= 1e-12
+            for s in range(S):
+                for t in range(0, T, max(1, T // 4)):
+                    r0, rk = oracle.chiral_overlap(L, spins[lo][s][a][perms[lo][s][a][t]], spins[hi][s][b][perms[hi][s][b][t]])
+                    assert np.abs(r0 - qc0[s, t]).max() <= TOL and np.abs(rk - qck[s, t]).max() <= TOL
+    assert np.abs(qc0_w).max() > 1e-4
+    for g in (lo, hi, whole):
+        g.close()

@@ -15,6 +15,9 @@ def _free_port():
         return s.getsockname()[1]
 
 
+import numpy as np
+
+
 class _FakeShard:
     """Stands in for a replica-sharded SpinGlass in the orchestration test: 'configurations' are tensors filled with the
     global replica number, an 'overlap' of replicas a, b is 10 a + b (so who was paired with whom is visible)."""
@@ -34,6 +37,17 @@ class _FakeShard:
         import torch
         return torch.full((self.S, 3, 4, self.T), float(self.rank * self.n + r))
 
+    def measure_chiral(self):
+        _, q0, _ = self.measure()
+        return -q0[..., None] * np.ones(3), -q0[..., None, None, None] * np.ones((3, 3, 2))
+
+    def export_chirality(self, r):
+        return -self.export_replica(r)
+
+    def chiral_cross(self, za, zb):
+        v = -(10.0 * float(-za[0, 0, 0, 0]) + float(-zb[0, 0, 0, 0]))
+        return np.full((self.S, self.T, 3), v), np.full((self.S, self.T, 3, 3, 2), v)
+
     def measure_cross(self, a, buf):
         import numpy as np
         v = 10.0 * (self.rank * self.n + a) + float(buf[0, 0, 0, 0])
@@ -52,7 +66,8 @@ def _worker(rank, world, port, out):
     import numpy as np
     window = multi.replica_window_of_rank(rank, world, 4)
     q = multi.gather_overlaps(np.full((3, 1, 5), float(rank)), world)       # [S][P_local][T] of this rank's one pair
-    q0_all, qk_all = multi.measure_all_pairs(_FakeShard(rank, 2), rank, world, 2)
+    q0_all, qk_all, qc0_all, qck_all = multi.measure_all_pairs(_FakeShard(rank, 2), rank, world, 2, chirality=True)
+    assert qc0_all[0, :, 0, 0].tolist() == [-v for v in q0_all[0, :, 0].tolist()] and qck_all.shape == (2, 6, 3, 3, 3, 2)
     out.put((rank, first, multi.max_over_ranks(seconds), multi.sum_over_ranks(first), rate, total, slowest, window,
              q.shape, q[:, :, 0].tolist(), q0_all[0, :, 0].tolist(), qk_all.shape))
     multi.barrier()
