@@ -80,6 +80,13 @@ def test_create_rejects_bad_arguments_without_a_device(lib):
     assert lib.sg_pt_swap(None) == binding.SG_EINVAL
     assert lib.sg_measure(None, None, None, None) == binding.SG_EINVAL
     assert lib.sg_strerror(binding.SG_ECUDA).decode().startswith("CUDA")
+    # the widened entry points reject a NULL context too (no device needed)
+    assert lib.sg_accumulate(None, 0) == binding.SG_EINVAL and lib.sg_get_logbins(None, None, None, None) == binding.SG_EINVAL
+    assert lib.sg_pt_walk(None, None, None) == binding.SG_EINVAL
+    assert lib.sg_init_sample_bimodal(None, 0, 0.5, None, None) == binding.SG_EINVAL
+    assert lib.sg_export_replica(None, 0, None) == binding.SG_EINVAL and lib.sg_measure_cross(None, 0, None, None, None) == binding.SG_EINVAL
+    assert lib.sg_export_chirality(None, 0, None) == binding.SG_EINVAL and lib.sg_chiral_cross(None, None, None, None, None) == binding.SG_EINVAL
+    assert lib.sg_measure_chiral(None, None, None) == binding.SG_EINVAL and lib.sg_schwinger_dyson(None, None) == binding.SG_EINVAL
 
 
 def test_no_cpu_fallback():
