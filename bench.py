@@ -9,7 +9,9 @@ after every `measure_every`-th unit.  `value` = HB + OR single-spin updates per 
 `e2e` = the same unit through the C ABI with host buffers: every step uploads the spin state of every
 sample from pinned host memory (sg_set_spins), runs the unit and reads the measurement back (sg_measure);
 the samples are independent chains, each driven through its own context / stream / host thread.
-`roofline` = the OR half-sweep kernel against the measured HBM copy bandwidth.
+`roofline` = the OR half-sweep kernel against the measured HBM copy bandwidth (DESIGN.md section 10);
+`sustained` / `roofline.sustained_frac` = the same loop over >= 3 back-to-back segments of >= 50 units (about 10 s),
+median: what the box holds under its power cap, next to the burst the --steps loop times.
 `cpu_baseline` / `--impl reference` = the fp64 oracle (oracle/), as it stands, on the host cores.
 Prints ONE JSON line on rank 0.
 """
@@ -102,7 +104,8 @@ class ClockSampler:
 def oracle_unit_rate(cfg, n_or_timed):
     """The oracle, as it stands, on one L = cfg.L sample: `cores` copies (one per OpenMP thread), one HB
     sweep and n_or_timed OR sweeps, timed separately and combined in the unit's mix 1 HB : cfg.n_or OR.
-    Returns (updates/s, cores, description, seconds spent)."""
+    Returns (updates/s, cores, description, seconds spent, split) -- split: ns per update of OR, HB and the
+    unit mix, with all cores and per core."""
     from oracle import sg_oracle as oracle
     oracle.build()
     cores = oracle.num_threads()
@@ -120,7 +123,11 @@ def oracle_unit_rate(cfg, n_or_timed):
     rate = (1 + cfg.n_or) * cores * N / (t_hb + cfg.n_or * t_or)
     what = ("1 sample of L=%d, %d copies (one per thread): 1 HB sweep + %d OR sweeps timed, combined in the "
             "unit mix 1 HB : %d OR" % (L, cores, n_or_timed, cfg.n_or))
-    return rate, cores, what, t2 - t0
+    per = 1e9 / (cores * N)          # seconds per sweep of `cores` copies -> ns per update with all cores
+    split = {"or_ns_per_update": t_or * per, "hb_ns_per_update": t_hb * per, "unit_ns_per_update": 1e9 / rate,
+             "or_ns_per_update_per_core": t_or * per * cores, "hb_ns_per_update_per_core": t_hb * per * cores,
+             "unit_ns_per_update_per_core": 1e9 / rate * cores}
+    return rate, cores, what, t2 - t0, split
 
 
 def run_reference(args, cfg):
@@ -131,13 +138,13 @@ def run_reference(args, cfg):
     # size the per-step sample so that (warmup + steps) steps end within a few minutes
     from oracle import sg_oracle as oracle
     oracle.build()
-    probe_rate, cores, _, _ = oracle_unit_rate(cfg, 1)
+    probe_rate, cores, _, _, _ = oracle_unit_rate(cfg, 1)
     per_sweep = cores * cfg.n_sites / probe_rate
     budget = 150.0 / max(1, args.steps + args.warmup)
     n_or_timed = int(max(1, min(cfg.n_or, budget / per_sweep - 1)))
     rates, secs = [], []
     for k in range(args.warmup + args.steps):
-        r, cores, what, dt = oracle_unit_rate(cfg, n_or_timed)
+        r, cores, what, dt, split = oracle_unit_rate(cfg, n_or_timed)
         if k >= args.warmup:
             rates.append(r); secs.append(dt)
     value = float(len(rates) / np.sum(1.0 / np.asarray(rates)))      # steps / total normalised time
@@ -147,7 +154,7 @@ def run_reference(args, cfg):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "ps_per_update": 1e12 / value,
         "config": workload_config(cfg, args.gpus, "host cores only"),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+        "cpu_baseline": dict({"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}, **split),
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -246,6 +253,34 @@ def run_ours(args, cfg):
     peak, peak_src = measured_hbm_peak()
     achieved = alg_bytes / or_launch_s / 1e9
 
+    # ---- sustained leg: >= 3 timed segments of >= 50 units, median; what the box holds once the
+    # power cap has settled (the --steps loop above is a burst of about a second at cfg 4) ----
+    sustained = None
+    if args.sustain_segments > 0:
+        unit_s = seconds / args.steps
+        seg_units = max(50, int(np.ceil(args.sustain_seconds / args.sustain_segments / unit_s)))
+        every = 1 if events_inside else 64                      # short units: per-call events only on every 64th unit
+        sampler2 = ClockSampler(local_rank) if rank == 0 else None
+        multi.barrier(); torch.cuda.synchronize()
+        t_s0 = time.time()
+        seg_rates, seg_or_us = [], []
+        for seg in range(args.sustain_segments):
+            del or_pairs[:], hb_pairs[:]
+            a, b = ev(), ev()
+            a.record()
+            for k in range(seg_units):
+                unit(k, k % every == 0)
+            b.record()
+            torch.cuda.synchronize()
+            sec = multi.max_over_ranks(a.elapsed_time(b) * 1e-3, device)
+            seg_rates.append(multi.sum_over_ranks(seg_units * cfg.updates_per_unit, device) / sec)
+            seg_or_us.append(float(np.mean([x.elapsed_time(y) for x, y in or_pairs])) * 1e3)
+        t_s1 = time.time()
+        clocks2 = sampler2.stop(t_s0, t_s1) if sampler2 else None
+        sustained = {"segments": args.sustain_segments, "units_per_segment": seg_units, "seconds": t_s1 - t_s0,
+                     "value": float(np.median(seg_rates)), "values": [float(v) for v in seg_rates],
+                     "or_call_us": float(np.median(seg_or_us)), "clocks": clocks2}
+
     # ---- end to end through the C ABI with host buffers ----
     host = [torch.empty((C, 3, N), dtype=torch.float32).pin_memory() for _ in range(S)]
     for s in range(S):
@@ -303,7 +338,9 @@ def run_ours(args, cfg):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": int(d2h),
                 "steps": e2e_steps, "what": "per step and sample: sg_set_spins from pinned host memory, one unit, sg_measure to "
                                             "host; one single-sample context, stream and host thread per sample (independent "
-                                            "chains), so uploads overlap sweeps; wall clock over all samples and steps"},
+                                            "chains), so uploads overlap sweeps; wall clock over all samples and steps; every "
+                                            "step uploads the same host state (a fresh start of the chain) and reads back the "
+                                            "measurement only: no device-to-host copy of the spins is included"},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": kernel_name,
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
@@ -312,9 +349,17 @@ def run_ours(args, cfg):
                      "ps_per_update_or": or_launch_s / updates_per_launch * 1e12,
                      "hb_sweep_ms": hb_ms, "or_call_ms": or_ms},
     }
+    if sustained is not None:
+        # the same kernel, the same algorithmic bytes, over the median OR call of the sustained segments
+        sus_launch_s = sustained["or_call_us"] * 1e-6 / (1 if resident else 2 * cfg.n_or)
+        out["roofline"]["sustained_launch_us"] = sus_launch_s * 1e6
+        out["roofline"]["sustained_frac"] = alg_bytes / sus_launch_s / 1e9 / peak
+        out["sustained"] = dict(sustained, unit=UNIT, ps_per_update=1e12 / sustained["value"],
+                                what="median over %d back-to-back segments of %d units each, same loop as the timed steps"
+                                     % (sustained["segments"], sustained["units_per_segment"]))
     if world == 1 and not args.no_cpu_baseline:
-        rate, cores, what, _ = oracle_unit_rate(cfg, cfg.n_or if cfg.L >= 32 else 4 * cfg.n_or)
-        out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}
+        rate, cores, what, _, split = oracle_unit_rate(cfg, cfg.n_or if cfg.L >= 32 else 4 * cfg.n_or)
+        out["cpu_baseline"] = dict({"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what}, **split)
     traffic_path = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_path):     # DRAM bytes per launch of the dominant kernel, from the committed ncu capture
         try:
@@ -339,6 +384,8 @@ def main():
     ap.add_argument("--zchunk", type=int, default=0, help="sg_tune(SG_TUNE_ZCHUNK): planes per CTA of the z-marching kernel")
     ap.add_argument("--e2e-zchunk", type=int, default=0, help="sg_tune(SG_TUNE_ZCHUNK) of the single-sample contexts of the e2e leg (0: 32 planes when L is a multiple of 32)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing (profiling runs)")
+    ap.add_argument("--sustain-segments", type=int, default=4, help="segments of the sustained leg (0: skip it)")
+    ap.add_argument("--sustain-seconds", type=float, default=10.0, help="target duration of the whole sustained leg (each segment is at least 50 units)")
     args = ap.parse_args()
     if args.impl == "ours":
         args.warmup = max(args.warmup, 3)      # timing rule: at least 3 untimed warm-up steps

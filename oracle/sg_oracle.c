@@ -342,6 +342,19 @@ void sgo_halfsweep(int L, const double* M, double* s, int kind, int colour, doub
     }
 }
 
+/* Test diagnostic (no arithmetic of the method): the two uniforms the heat bath of sgo_halfsweep draws at every site of
+ * copy g in HB sweep hb_counter (stream 1 of SURVEY.md section 8(c) step 2: counter (i, g, hb_counter, 1), w0 -> r1, w1 -> r2).
+ * The tests use it to FIND sweeps in which r1 falls in its extreme tails (2^-24, 1 - 2^-24). */
+void sgo_hb_uniforms(int N, uint64_t seed, uint32_t g, uint32_t hb_counter, double* r1, double* r2)
+{
+    for (int i = 0; i < N; ++i) {
+        uint32_t w[4];
+        sgo_draw(seed, (uint32_t)i, g, hb_counter, SGO_STREAM_HB, w);
+        r1[i] = sgo_uniform23(w[0]);
+        r2[i] = sgo_uniform23(w[1]);
+    }
+}
+
 /* n_sweeps full sweeps (colour 0 then colour 1) of n_copies copies of one sample.
  * spins[n_copies][3][N]; beta_of_copy[n_copies] (ignored for OR); copy c has global id g0 + c;
  * HB sweep k uses hb_counter0 + k.  Copies are independent between PT sweeps, so the

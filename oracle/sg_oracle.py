@@ -58,6 +58,7 @@ def lib():
         L.sgo_or_update.argtypes = [dp, dp]
         L.sgo_hb_update.argtypes = [dp, d, d, d, dp]
         L.sgo_halfsweep.argtypes = [i, dp, dp, i, i, d, u64, u32, u32, i, u8p, dp, dp]
+        L.sgo_hb_uniforms.argtypes = [i, u64, u32, u32, dp, dp]
         L.sgo_sweep_copies.argtypes = [i, dp, dp, i, i, i, dp, u64, u32, u32, i]
         L.sgo_energy_copies.argtypes = [i, dp, dp, i, dp]
         L.sgo_num_threads.restype = i
@@ -194,6 +195,13 @@ def halfsweep(L, M, s, kind, colour, beta=0.0, seed=0, g=0, hb_counter=0, store_
                         _dp(hnorm_out) if hnorm_out is not None else None,
                         _dp(sd) if want_sd else None)
     return flags, sd
+
+
+def hb_uniforms(L, seed, g, hb_counter):
+    """(r1 [N], r2 [N]): the uniforms the heat bath draws at every site of copy g in HB sweep hb_counter (test diagnostic)."""
+    r1 = np.zeros(L ** 3); r2 = np.zeros(L ** 3)
+    lib().sgo_hb_uniforms(L ** 3, int(seed), int(g), int(hb_counter), _dp(r1), _dp(r2))
+    return r1, r2
 
 
 def sweep_copies(L, M, spins, kind, n_sweeps, beta_of_copy=None, seed=0, g0=0, hb_counter0=0,

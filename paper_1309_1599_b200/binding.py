@@ -289,6 +289,11 @@ class SpinGlass:
         self._check(self._lib.sg_get_logbins(self._ctx, _ptr(sums), _ptr(counts), _ptr(counts_cg)), "sg_get_logbins")
         return sums, counts, counts_cg
 
+    def export_buffer(self):
+        """Uninitialised device tensor of the shape export_replica / export_chirality fill (a receive buffer)."""
+        import torch
+        return torch.empty((self.S, 3, self.N, self.T), dtype=torch.float32, device=self.device)
+
     def export_replica(self, r, out=None):
         """Device tensor float32 [S][3][N][T]: the configurations of local replica r ordered by temperature (asynchronous)."""
         import torch

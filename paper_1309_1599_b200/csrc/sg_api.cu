@@ -39,6 +39,7 @@ struct sg_ctx {
     int res_cpc, res_cpc_req;   // copies per CTA of the resident kernel (4, 8, 16, 32); requested, 0 = automatic
     int zm_zc_req;    // requested planes per chunk, 0 = automatic
     int zm_ok, zm_ZC, zm_nzc;
+    uint32_t zm_attr_set = 0;   // template instances of k_sweep_zm whose shared-memory attribute this context has set on its device
     // measure geometry
     int nchunk, chunk_sites, MS;
     // host state
@@ -248,10 +249,18 @@ void zm_plan(sg_ctx* ctx)
     } else {
         // the longest chunk that still gives every SM several CTAs' worth of work in turn (2 CTAs per SM x 148 SMs
         // per wave); a chunk re-reads 2 planes of other-colour sites per ZC planes
+        // Candidates are the even divisors of L that are >= 4 (the kernel steps through a chunk in pairs of planes
+        // from an even z0): the longest one that reaches the CTA count, else the shortest candidate.
         const long per_plane_col = (long)ctx->S * ctx->NG * (L / ZM_TX) * (L / ZM_TY);
-        ZC = L;
-        while (ZC > 8 && per_plane_col * (L / ZC) < 6 * 296) ZC /= 2;
+        int shortest = L;
+        for (int cand = L; cand >= 4; --cand) {
+            if ((cand & 1) || L % cand != 0) continue;
+            shortest = cand;
+            if (cand <= 8 || per_plane_col * (L / cand) >= 6 * 296) { ZC = cand; break; }
+        }
+        if (ZC == 0) ZC = shortest;
     }
+    if (ZC < 2 || (ZC & 1) || L % ZC != 0) { ctx->zm_ok = 0; return; }     // never launch a chunking the kernel cannot step through
     ctx->zm_ZC = ZC; ctx->zm_nzc = L / ZC;
 }
 
@@ -260,10 +269,12 @@ int launch_zm_p(sg_ctx* ctx, const ZmParams& p, dim3 grid)
 {
     auto kern = k_sweep_zm<KIND, WITH_E, ZM_TX, ZM_TY, ZM_NST, ZM_NJ, PACKED>;
     constexpr size_t smem = zm_smem_bytes<ZM_TX, ZM_TY, ZM_NST, ZM_NJ>();
-    static bool attr_done = false;   // per process and template instance; the attribute is per function
-    if (!attr_done) {
+    // the attribute is per (function, device): remembered per context (a context lives on one device, is driven by one
+    // host thread at a time) and per template instance
+    constexpr uint32_t bit = 1u << ((KIND * 2 + (WITH_E ? 1 : 0)) * 2 + (PACKED ? 1 : 0));
+    if (!(ctx->zm_attr_set & bit)) {
         SG_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
+        ctx->zm_attr_set |= bit;
     }
     kern<<<grid, ZmGeom<ZM_TX, ZM_TY>::THREADS, smem, ctx->stream>>>(p);
     return SG_OK;

@@ -105,8 +105,8 @@ __global__ void __launch_bounds__(SWEEP_THREADS) k_sweep(const SweepParams p)
         if (KIND == KIND_OR) {
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
                 or_update(hf[0][j], hf[1][j], hf[2][j], s[0][j], s[1][j], s[2][j]);
+                if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));   // of the stored spin
             }
         } else if (KIND == KIND_HB) {
             const float bt[4] = { beta4.x, beta4.y, beta4.z, beta4.w };

@@ -106,8 +106,8 @@ __global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
                 if (KIND_ == 0) {
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
-                        if (last) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
                         or_update(hf[0][j], hf[1][j], hf[2][j], s[0][j], s[1][j], s[2][j]);
+                        if (last) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));   // of the stored spin
                     }
                 } else {
                     const float bt[4] = { beta4.x, beta4.y, beta4.z, beta4.w };

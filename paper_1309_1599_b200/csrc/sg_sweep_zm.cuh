@@ -114,8 +114,9 @@ __device__ __forceinline__ void zm_update(const float (&hf)[3][4], float (&s)[3]
     if (KIND == KIND_OR) {
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
             or_update(hf[0][j], hf[1][j], hf[2][j], s[0][j], s[1][j], s[2][j]);
+            // s.h of the STORED spin (equal to the old s.h only in exact arithmetic), so that E is the energy of the stored state
+            if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
         }
     } else if (KIND == KIND_HB) {
         const float bt[4] = { beta4.x, beta4.y, beta4.z, beta4.w };

@@ -50,11 +50,17 @@ def gather_overlaps(local, world_size, device="cpu"):
     return np.concatenate([x.cpu().numpy() for x in parts], axis=1)
 
 
-def _pairs_from_blocks(local_blocks, rank, world_size, n_local, export, cross):
+def _pairs_from_blocks(local_blocks, rank, world_size, n_local, export, cross, alloc=None, stream=None):
     """Shared orchestration of measure_all_pairs: `local_blocks` are the per-pair arrays [S][P_local]... of the pairs inside
-    this rank; a pair across ranks is computed by the rank that holds a, from what b's rank exports and broadcasts
-    (one buffer alive at a time).  Returns the arrays stacked over all pairs in the global order, on every rank."""
+    this rank; a pair across ranks is computed by the rank that holds a, from what b's rank exports and sends to every
+    rank below it (one buffer alive at a time; ranks above the source neither export nor receive).  `alloc()` returns an
+    uninitialised receive buffer of export()'s shape (default: export(0), which costs a kernel).  `stream`: the CUDA
+    stream the context's kernels run on -- export, the transfers and cross are issued with it as torch's current stream,
+    because torch.distributed orders its NCCL work against the current stream only.
+    Returns the arrays stacked over all pairs in the global order, on every rank."""
+    import contextlib
     import numpy as np
+    import torch
     import torch.distributed as dist
     mine = {}
     k = 0
@@ -63,13 +69,19 @@ def _pairs_from_blocks(local_blocks, rank, world_size, n_local, export, cross):
             mine[(rank * n_local + a, rank * n_local + b)] = tuple(blk[:, k] for blk in local_blocks)
             k += 1
     if world_size > 1:
-        for src in range(1, world_size):                         # rank 0 never sends: nobody holds smaller replicas
-            for r in range(n_local):
-                buf = export(r)                                  # every rank fills a buffer of the same shape ...
-                dist.broadcast(buf, src=src)                     # ... and src's overwrites it everywhere
-                if rank < src:
-                    for a in range(n_local):
-                        mine[(rank * n_local + a, src * n_local + r)] = tuple(cross(a, buf))
+        on_stream = torch.cuda.stream(stream) if isinstance(stream, torch.cuda.Stream) else contextlib.nullcontext()
+        with on_stream:
+            for src in range(1, world_size):                     # rank 0 never sends: nobody holds smaller replicas
+                for r in range(n_local):
+                    if rank == src:
+                        buf = export(r)
+                        for dst in range(src):
+                            dist.send(buf, dst=dst)
+                    elif rank < src:
+                        buf = alloc() if alloc is not None else export(0)
+                        dist.recv(buf, src=src)
+                        for a in range(n_local):
+                            mine[(rank * n_local + a, src * n_local + r)] = tuple(cross(a, buf))
         parts = [None] * world_size
         dist.all_gather_object(parts, mine)
         mine = {key: val for part in parts for key, val in part.items()}
@@ -87,7 +99,8 @@ def measure_all_pairs(gpu, rank, world_size, n_local, chirality=False):
     Returns (q0 [S][P][T], qk [S][P][T][3][2]) -- with `chirality` also (qc0 [S][P][T][3], qck [S][P][T][3][3][2]) -- on
     every rank, pairs in the order (0,1),(0,2),...,(R-2,R-1) of the GLOBAL replica numbers, R = world_size * n_local."""
     _, q0_loc, qk_loc = gpu.measure()
-    out = _pairs_from_blocks((q0_loc, qk_loc), rank, world_size, n_local, gpu.export_replica, gpu.measure_cross)
+    alloc, stream = getattr(gpu, "export_buffer", None), getattr(gpu, "stream", None)
+    out = _pairs_from_blocks((q0_loc, qk_loc), rank, world_size, n_local, gpu.export_replica, gpu.measure_cross, alloc, stream)
     if chirality:
         local_z = {}
 
@@ -96,7 +109,7 @@ def measure_all_pairs(gpu, rank, world_size, n_local, chirality=False):
                 local_z[a] = gpu.export_chirality(a)
             return gpu.chiral_cross(local_z[a], zb)
 
-        out = out + _pairs_from_blocks(tuple(gpu.measure_chiral()), rank, world_size, n_local, gpu.export_chirality, cross)
+        out = out + _pairs_from_blocks(tuple(gpu.measure_chiral()), rank, world_size, n_local, gpu.export_chirality, cross, alloc, stream)
     return out
 
 

@@ -5,9 +5,11 @@ giving every "sample" of the context the same couplings (their Philox streams di
 id), so the error bars need no autocorrelation model: each chain's second half
 (thermalisation) is cut into a few long bins and the K x bins bin means are the sample.
 The oracle and CUDA trajectories separate after a few sweeps (fp32 vs fp64 rounding amplified by the
-chaotic dynamics), so the two sides' errors are independent.  With n comparisons the bar is the SURVEY's
-(section 8(c)): max |z| < 4.5 (Student tails: ~40 degrees of freedom) and chi^2/n consistent with 1.
-Seeds are fixed, both chains are deterministic."""
+chaotic dynamics), so the two sides' errors are independent.  The bar is the SURVEY's (section 8(c)): every
+comparison within max |z| < 4 and chi^2/n consistent with 1 (n = 12 comparisons for cfg 0, 32 for cfg 1; the
+north star's 3 sigma is a per-comparison statement, P(|z| > 3) = 2.7e-3, so over n comparisons the family-wise
+bar at the same confidence is |z| < 4).  The observed max |z| and chi^2/n are printed (pytest -s / -rP shows them)
+and recorded in DESIGN.md section 6.  Seeds are fixed, both chains are deterministic."""
 import numpy as np
 import pytest
 
@@ -59,8 +61,11 @@ def compare(obs_gpu, obs_ref, names, n_bins):
         assert np.all(np.isfinite(z)), name
         zs.append(z.reshape(-1))
     z = np.concatenate(zs)
-    assert np.abs(z).max() < 4.5, (np.abs(z).max(), z)
-    assert (z ** 2).mean() < 1.1 + 4.0 * np.sqrt(2.0 / z.size), ((z ** 2).mean(), z.size)
+    chi2 = float((z ** 2).mean())
+    print("STATS-MARGIN %s: n = %d comparisons, max |z| = %.3f (bar 4), chi^2/n = %.3f (bar %.3f), fraction |z| > 3: %.3f"
+          % ("+".join(names), z.size, np.abs(z).max(), chi2, 1.1 + 4.0 * np.sqrt(2.0 / z.size), np.mean(np.abs(z) > 3)))
+    assert np.abs(z).max() < 4.0, ("max |z|", np.abs(z).max(), "chi2/n", chi2, z)
+    assert chi2 < 1.1 + 4.0 * np.sqrt(2.0 / z.size), ("chi2/n", chi2, z.size, "max |z|", np.abs(z).max())
     return z
 
 

@@ -119,6 +119,26 @@ def test_hb_distinct_streams(oracle):
     assert len({tuple(np.round(outs[0][:, i], 12)) for i in range(0, N) if outs[0][2, i] != 1.0}) == N // 2
 
 
+def test_hb_uniforms_are_the_numbers_the_half_sweep_draws(oracle):
+    """The test diagnostic hb_uniforms(seed, g, hb_counter) returns, site by site, the (r1, r2) of the lattice heat bath:
+    feeding them to the single-spin update with the site's field reproduces the half-sweep, and they are the exactly
+    representable 23-bit uniforms of stream 1 (counter (i, g, hb_counter, 1))."""
+    L, N = 4, 64
+    rng = np.random.default_rng(12)
+    M = W.random_couplings(rng, N, "general")
+    s0 = W.random_spins(rng, 1, N)[0]
+    r1, r2 = oracle.hb_uniforms(L, 5, 2, 7)
+    s = s0.copy()
+    oracle.halfsweep(L, M, s, oracle.KIND_HB, 1, beta=0.8, seed=5, g=2, hb_counter=7)
+    for i in range(N):
+        if oracle.lib().sgo_colour(L, i) == 1:
+            want = oracle.hb_update(oracle.local_field(L, M, s0, i), 0.8, r1[i], r2[i])
+            assert np.array_equal(s[:, i], want)
+    for i in (0, 17, 63):
+        w = oracle.philox4x32_10((i, 2, 7, 1), (5, 0))
+        assert r1[i] == ((w[0] >> 9) + 0.5) / 2 ** 23 and r2[i] == ((w[1] >> 9) + 0.5) / 2 ** 23
+
+
 # ---------------------------------------------------------------------------------------------
 # P9  Schwinger-Dyson (Eq. (A6), PAPER.md:410-414), site-averaged, any couplings
 # ---------------------------------------------------------------------------------------------
