@@ -232,8 +232,14 @@ int sg_pt_walk(sg_ctx* ctx, uint64_t* round_trips, int32_t* label);
  *   of that many copies does not fit in shared memory).
  * SG_TUNE_PACKED: 1 = the z-marching sweep reads the packed bytes when every sample was initialised by
  *   sg_init_sample_bimodal with one and the same D; 0 (default) = always the fp32 matrices, which measured 3-7 % faster
- *   at 32 and more copies per sample.  Same spins bit for bit. */
-enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2, SG_TUNE_PACKED = 3 };
+ *   at 32 and more copies per sample.  Same spins bit for bit.
+ * SG_TUNE_MEASURE_IMPL: which kernel forms the overlaps of sg_measure / sg_accumulate.
+ *   SG_MEASURE_AUTO    the streaming row kernel (thread = (lattice row, temperature), every replica's spin loaded once for
+ *                      all pairs) when 2 <= R <= 4, else the staged kernel (default)
+ *   SG_MEASURE_STAGED  the staged kernel (sites of all copies through shared memory; any R)
+ *   Same products, fp32 row sums in the streaming kernel: results agree to ~1e-8. */
+enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2, SG_TUNE_PACKED = 3, SG_TUNE_MEASURE_IMPL = 4 };
+enum { SG_MEASURE_AUTO = 0, SG_MEASURE_STAGED = 1 };
 enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2, SG_SWEEP_RESIDENT = 3 };
 int sg_tune(sg_ctx* ctx, int knob, int value);
 

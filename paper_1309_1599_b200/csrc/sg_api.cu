@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "sg_kernels.cuh"
+#include "sg_measure.cuh"
 #include "sg_sweep_res.cuh"
 
 using namespace sg;
@@ -42,10 +43,13 @@ struct sg_ctx {
     uint32_t zm_attr_set = 0;   // template instances of k_sweep_zm whose shared-memory attribute this context has set on its device
     // measure geometry
     int nchunk, chunk_sites, MS;
+    int mq_nchunk, mq_rows_per_cta, mq_Tw, mq_rows_t;   // k_measure_rows: row chunks per sample, rows per CTA, temperatures and rows per CTA pass
+    uint32_t mq_attr_set = 0;
     // host state
     std::vector<double> h_betas;
     std::vector<char> inited;
     std::vector<double> bimodal_D;   // per sample: D of its packed bimodal couplings (sg_init_sample_bimodal), NaN if not packed
+    int measure_impl = 0;            // SG_TUNE_MEASURE_IMPL
     int packed_on;                   // SG_TUNE_PACKED: 1 = the z-marching sweep reads the packed bytes when every sample is packed
     uint64_t hb_counter, pt_counter, launches;
     bool energies_fresh;
@@ -74,6 +78,7 @@ bool shape_ok(const sg_shape* s)
 
 struct Geometry {
     int L, N, Nh, S, R, T, C, NG, Cp, P, tile_sites, ntiles, nchunk, chunk_sites, MS;
+    int mq_nchunk, mq_rows_per_cta, mq_Tw, mq_rows_t;
 };
 
 Geometry geometry(const sg_shape* s)
@@ -89,6 +94,18 @@ Geometry geometry(const sg_shape* s)
     g.nchunk = g.N / 32; if (g.nchunk < 1) g.nchunk = 1; if (g.nchunk > 256) g.nchunk = 256;   // >= 2 batches of sites per CTA, enough CTAs for small lattices
     g.chunk_sites = (g.N + g.nchunk - 1) / g.nchunk;
     g.MS = 11500 / (3 * g.Cp); if (g.MS < 1) g.MS = 1; if (g.MS > 16) g.MS = 16;
+    // k_measure_rows: a CTA pass = rows_t lattice rows x Tw temperatures; a CTA takes `rounds` passes of consecutive rows.
+    // At most 256 chunks per sample (the partials array), at least ~4 CTAs per SM over the job when the lattice allows,
+    // and a few passes per CTA to amortise its final reduction.
+    g.mq_Tw = g.T < MROWS_THREADS ? g.T : MROWS_THREADS;
+    g.mq_rows_t = MROWS_THREADS / g.mq_Tw;
+    {
+        const int rows = g.L * g.L;
+        int rounds = (rows + 256 * g.mq_rows_t - 1) / (256 * g.mq_rows_t);
+        while (rounds < 4 && (long)g.S * (rows / (g.mq_rows_t * (rounds + 1))) >= 592) ++rounds;
+        g.mq_rows_per_cta = g.mq_rows_t * rounds;
+        g.mq_nchunk = (rows + g.mq_rows_per_cta - 1) / g.mq_rows_per_cta;
+    }
     return g;
 }
 
@@ -117,7 +134,11 @@ Offsets offsets(const Geometry& g)
     o.Epart = c.take((size_t)g.S * g.NG * g.ntiles * G * sizeof(double));
     o.SDpart = c.take((size_t)g.S * g.NG * 2 * g.ntiles * G * 2 * sizeof(double));
     o.phase = c.take((size_t)g.L * 2 * sizeof(double));
-    o.Mpart = c.take((size_t)g.S * g.nchunk * (g.P * g.T > 0 ? g.P * g.T : 1) * 21 * sizeof(double));   // 7 per item (overlap), 21 (chirality)
+    {   // 21 per item and chunk (chirality), 7 per item and row chunk (overlap)
+        const size_t items = (g.P * g.T > 0 ? (size_t)g.P * g.T : 1);
+        const size_t a = (size_t)g.nchunk * 21, b = (size_t)g.mq_nchunk * 7;
+        o.Mpart = c.take((size_t)g.S * items * (a > b ? a : b) * sizeof(double));
+    }
     o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + (size_t)g.S * g.T * 21 + 1) * sizeof(double));
     o.sot = c.take((size_t)g.S * g.R * g.T * sizeof(int));
     o.tos = c.take((size_t)g.S * g.R * g.T * sizeof(int));
@@ -472,6 +493,26 @@ int sweeps(sg_ctx* ctx, int kind, int n_sweeps)
     return SG_OK;
 }
 
+// the streaming overlap pass (sg_measure.cuh) for R = 2, 3, 4 replicas
+template <int R_>
+int launch_measure_rows(sg_ctx* ctx)
+{
+    MeasureRowsParams p;
+    p.spins = ctx->spins; p.slot_of_temp = ctx->slot_of_temp; p.phase = ctx->phase; p.Mpart = ctx->Mpart;
+    p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.R = ctx->R; p.T = ctx->T; p.P = ctx->P;
+    p.nchunk = ctx->mq_nchunk; p.rows_per_cta = ctx->mq_rows_per_cta; p.Tw = ctx->mq_Tw; p.rows_t = ctx->mq_rows_t;
+    const size_t smem = mrows_smem_bytes(ctx->L, R_);
+    auto kern = k_measure_rows<R_>;
+    if (!(ctx->mq_attr_set & (1u << R_))) {
+        SG_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ctx->mq_attr_set |= 1u << R_;
+    }
+    const int tz = (ctx->T + ctx->mq_Tw - 1) / ctx->mq_Tw;
+    kern<<<dim3(ctx->mq_nchunk, ctx->S, tz), MROWS_THREADS, smem, ctx->stream>>>(p);
+    SG_LAUNCHED(ctx);
+    return SG_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -509,6 +550,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->g_first = (uint32_t)shape->first_sample * (uint32_t)ctx->Cg + (uint32_t)shape->first_replica * (uint32_t)g.T;
     ctx->tile_sites = g.tile_sites; ctx->ntiles = g.ntiles; ctx->log2L = ilog2_exact(g.L);
     ctx->nchunk = g.nchunk; ctx->chunk_sites = g.chunk_sites; ctx->MS = g.MS;
+    ctx->mq_nchunk = g.mq_nchunk; ctx->mq_rows_per_cta = g.mq_rows_per_cta; ctx->mq_Tw = g.mq_Tw; ctx->mq_rows_t = g.mq_rows_t;
     ctx->stream = (cudaStream_t)cuda_stream;
     char* base = (char*)dev_workspace;
     ctx->spins = (float*)(base + o.spins); ctx->Jg = (float*)(base + o.Jg); ctx->Jt = (g.L % 8 == 0) ? (float*)(base + o.Jt) : nullptr; ctx->Jp = (g.L % 8 == 0) ? (unsigned char*)(base + o.Jp) : nullptr; ctx->Mraw = (float*)(base + o.Mraw);
@@ -751,23 +793,31 @@ static int launch_measure(sg_ctx* ctx, bool with_q)
     if (int rc = all_inited(ctx)) return rc;
     if (int rc = ensure_energies(ctx)) return rc;
     const int PT = ctx->P * ctx->T;
+    int nchunk = ctx->nchunk;
     if (PT > 0 && with_q) {
-        MeasureParams p;
-        p.spins = ctx->spins; p.slot_of_temp = ctx->slot_of_temp; p.phase = ctx->phase; p.Mpart = ctx->Mpart;
-        p.L = ctx->L; p.N = ctx->N; p.NG = ctx->NG; p.Cp = ctx->Cp; p.R = ctx->R; p.T = ctx->T; p.P = ctx->P;
-        p.nchunk = ctx->nchunk; p.chunk_sites = ctx->chunk_sites; p.MS = ctx->MS;
-        int threads = ((PT + 31) / 32) * 32;
-        if (threads > 512) threads = 512;
-        const int nbatch = (PT + threads - 1) / threads;
-        const size_t smem = (size_t)ctx->MS * 3 * ctx->Cp * sizeof(float) + (size_t)ctx->MS * 6 * sizeof(double);
-        if (smem > 48 * 1024) return SG_EINVAL;
-        k_measure<<<dim3(ctx->nchunk, ctx->S, nbatch), threads, smem, ctx->stream>>>(p);
-        SG_LAUNCHED(ctx);
+        const bool rows = ctx->measure_impl != SG_MEASURE_STAGED && ctx->R >= 2 && ctx->R <= 4 && mrows_smem_bytes(ctx->L, ctx->R) <= 200 * 1024;
+        if (rows) {
+            int rc = (ctx->R == 2) ? launch_measure_rows<2>(ctx) : (ctx->R == 3) ? launch_measure_rows<3>(ctx) : launch_measure_rows<4>(ctx);
+            if (rc != SG_OK) return rc;
+            nchunk = ctx->mq_nchunk;
+        } else {
+            MeasureParams p;
+            p.spins = ctx->spins; p.slot_of_temp = ctx->slot_of_temp; p.phase = ctx->phase; p.Mpart = ctx->Mpart;
+            p.L = ctx->L; p.N = ctx->N; p.NG = ctx->NG; p.Cp = ctx->Cp; p.R = ctx->R; p.T = ctx->T; p.P = ctx->P;
+            p.nchunk = ctx->nchunk; p.chunk_sites = ctx->chunk_sites; p.MS = ctx->MS;
+            int threads = ((PT + 31) / 32) * 32;
+            if (threads > 512) threads = 512;
+            const int nbatch = (PT + threads - 1) / threads;
+            const size_t smem = (size_t)ctx->MS * 3 * ctx->Cp * sizeof(float) + (size_t)ctx->MS * 6 * sizeof(double);
+            if (smem > 48 * 1024) return SG_EINVAL;
+            k_measure<<<dim3(ctx->nchunk, ctx->S, nbatch), threads, smem, ctx->stream>>>(p);
+            SG_LAUNCHED(ctx);
+        }
     }
     const int nE = ctx->S * ctx->R * ctx->T, nQ = ctx->S * PT;
     const int total = nE + nQ * 7;
     k_reduce_measure<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->Mpart, ctx->E, ctx->slot_of_temp, ctx->result, ctx->S,
-                                                                 ctx->R, ctx->T, ctx->P, ctx->Cp, ctx->nchunk, ctx->N);
+                                                                 ctx->R, ctx->T, ctx->P, ctx->Cp, nchunk, ctx->N);
     SG_LAUNCHED(ctx);
     return SG_OK;
 }
@@ -1082,6 +1132,10 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
     case SG_TUNE_PACKED:
         if (value != 0 && value != 1) return SG_EINVAL;
         ctx->packed_on = value;
+        return SG_OK;
+    case SG_TUNE_MEASURE_IMPL:
+        if (value != SG_MEASURE_AUTO && value != SG_MEASURE_STAGED) return SG_EINVAL;
+        ctx->measure_impl = value;
         return SG_OK;
     case SG_TUNE_ZCHUNK:
         if (value < 0) return SG_EINVAL;

@@ -119,8 +119,7 @@ def test_cfg3_full_size_sampled_copies(sg, oracle):
                     err[flags != 0] = 0.0
                     assert err.max() <= SPIN_TOL, (kind, colour, s, c, err.max())
                     assert (flags != 0).sum() <= 1e-3 * mask.sum()
-    for s in M:
-        gpu.set_spins(s, X[s])
+    E0 = gpu.get_energies()                                        # of the state the half-sweeps above left (stand-alone pass)
     gpu.sweep_or(1)                                                # OR conserves every copy's energy (fused reduction)
     E1 = gpu.get_energies()
     assert np.all(np.abs(E1 - E0) / N <= 1e-6 * np.maximum(1.0, np.abs(E0) / N))

@@ -205,7 +205,10 @@ def test_cross_context_overlaps(sg, oracle, L, S, T):
             g.unit(2)
         return g
     lo, hi, whole = make(2, 0, 4), make(2, 2, 4), make(4, 0, 0)
-    _, q0_w, qk_w = whole.measure()
+    _, q0_r, qk_r = whole.measure()                                             # streaming row kernel: fp32 row sums
+    whole.tune(sg.TUNE_MEASURE_IMPL, sg.MEASURE_STAGED)
+    _, q0_w, qk_w = whole.measure()                                             # staged kernel: fp64 sums of the same products
+    assert np.abs(q0_r - q0_w).max() <= 2e-7 and np.abs(qk_r - qk_w).max() <= 2e-7
     pair_index = {(a, b): k for k, (a, b) in enumerate(oracle.replica_pairs(4))}
     spins = {g: [g.get_spins(s).reshape(2, T, 3, N) for s in range(S)] for g in (lo, hi)}
     perms = {g: [g.get_perm(s)[1] for s in range(S)] for g in (lo, hi)}           # slot_of_temp [R][T]

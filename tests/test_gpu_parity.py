@@ -237,9 +237,12 @@ def test_time_reversal_and_involution_on_gpu(sg, oracle):
 # S3, S5: energies and overlaps
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("sh", SHAPES)
-def test_measure_matches_oracle(sg, oracle, sh):
+@pytest.mark.parametrize("staged", [False, True])
+def test_measure_matches_oracle(sg, oracle, sh, staged):
+    """Both overlap kernels: the streaming row kernel (default for R <= 4) and the staged one (any R)."""
     L, S, R, T = sh["L"], sh["S"], sh["R"], sh["T"]
     sim, gpu = make_pair(oracle, sg, L, S, R, T, betas_of(sh), seed=10, tune=sh.get("tune"))
+    gpu.tune(sg.TUNE_MEASURE_IMPL, sg.MEASURE_STAGED if staged else sg.MEASURE_AUTO)
     rng = np.random.default_rng(3)
     for s in range(S):                                    # a non-trivial temperature assignment
         tos = np.stack([rng.permutation(T) for _ in range(R)]).astype(np.int32)
@@ -252,6 +255,22 @@ def test_measure_matches_oracle(sg, oracle, sh):
     e_ref, q0_ref, qk_ref = sim.measure()
     assert np.all(np.abs(e - e_ref) <= 1e-6 * np.maximum(1.0, np.abs(e_ref)))
     assert np.abs(q0 - q0_ref).max() <= 1e-6 and np.abs(qk - qk_ref).max() <= 1e-6
+
+
+def test_measure_five_replicas_and_many_temperatures(sg, oracle):
+    """R = 5 (ten pairs: the staged kernel serves R > 4) and T = 300 > 256 (the row kernel tiles the temperatures)."""
+    for L, S, R, T in ((4, 1, 5, 3), (4, 1, 2, 300)):
+        betas = np.linspace(0.5, 1.5, T)
+        sim, gpu = make_pair(oracle, sg, L, S, R, T, betas, seed=14)
+        rng = np.random.default_rng(8)
+        tos = np.stack([rng.permutation(T) for _ in range(R)]).astype(np.int32)
+        gpu.set_perm(0, tos)
+        sim.temp_of_slot[0] = tos
+        sim.slot_of_temp[0] = np.argsort(tos, axis=1).astype(np.int32)
+        e, q0, qk = gpu.measure()
+        e_ref, q0_ref, qk_ref = sim.measure()
+        assert np.all(np.abs(e - e_ref) <= 1e-6 * np.maximum(1.0, np.abs(e_ref)))
+        assert np.abs(q0 - q0_ref).max() <= 1e-6 and np.abs(qk - qk_ref).max() <= 1e-6
 
 
 def test_measure_closed_forms_on_gpu(sg):
