@@ -301,6 +301,30 @@ def logbin_observables(e, q0, qk, qc0=None, qck=None):
 LOGBINS = 32
 
 
+def walk_tau_int(series, window_c=6.0):
+    """Integrated autocorrelation time of a recorded random walk in temperature (Sect. III: "we measured
+    the integrated autocorrelation time (mixing time) of the random walk in temperatures of each sample"; the paper
+    gives no formula and cites a textbook, Ref. 31 -- the reading taken, R24, is the standard estimator):
+        m = mean(x),  C(0) = sum_i (x_i - m)^2 / n,  C(k) = sum_{i < n-k} (x_i - m)(x_{i+k} - m) / (n - k),
+        tau(W) = 1/2 + sum_{k=1}^{W} C(k)/C(0),
+    summed up to the first W with W >= window_c * tau(W) (self-consistent window), at most n // 2.  In units of the
+    sampling interval of the series (one PT sweep = one MCS).  NaN for n < 4 or a constant series."""
+    x = np.asarray(series, dtype=np.float64)
+    n = x.size
+    if n < 4:
+        return float("nan")
+    d = x - x.mean()
+    c0 = float(np.dot(d, d)) / n
+    if not c0 > 0.0:
+        return float("nan")
+    tau = 0.5
+    for k in range(1, n // 2 + 1):
+        tau += float(np.dot(d[:n - k], d[k:])) / (n - k) / c0
+        if k >= window_c * tau:
+            break
+    return tau
+
+
 def replica_pairs(R):
     """Pairs a<b in the order (0,1),(0,2),...,(R-2,R-1) (reading R15)."""
     return [(a, b) for a in range(R) for b in range(a + 1, R)]
@@ -335,6 +359,7 @@ class OracleSim:
         self.accepts = np.zeros_like(self.attempts)
         self.walk_label = np.zeros((self.S, self.R, self.T), dtype=np.int32)
         self.round_trips = np.zeros((self.S, self.R, 1), dtype=np.uint64)
+        self.visits = np.zeros((self.S, self.R, self.T, self.T), dtype=np.uint64)   # [slot][t]
         self.n_acc = 0
         self.logbin_sums = np.zeros((LOGBINS, self.S, self.T, 6))
         self.logbin_counts = np.zeros(LOGBINS, dtype=np.uint64)
@@ -397,7 +422,7 @@ class OracleSim:
                 pt_sweep(self.betas, E[s, r * self.T:(r + 1) * self.T], self.slot_of_temp[s, r],
                          self.temp_of_slot[s, r], self.seed, chain, self.pt_counter,
                          self.attempts[s, r], self.accepts[s, r])
-                pt_walk_update(self.temp_of_slot[s, r], self.walk_label[s, r], self.round_trips[s, r])
+                pt_walk_update(self.temp_of_slot[s, r], self.walk_label[s, r], self.round_trips[s, r], self.visits[s, r])
         self.pt_counter += 1
 
     def measure(self):

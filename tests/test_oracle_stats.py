@@ -349,6 +349,47 @@ def test_pt_walk_round_trips_by_hand_and_brute_force(oracle):
     assert visits.sum() == n * T
 
 
+def test_walk_tau_int_by_hand_and_on_known_processes(oracle):
+    """Pins of oracle.walk_tau_int (reading R24).  (a) x = (0, 1, 1, 0) by hand: m = 1/2, C(0) = 1/4,
+    C(1) = (-1/4 + 1/4 - 1/4)/3 = -1/12, rho(1) = -1/3, tau(1) = 1/2 - 1/3 = 1/6 and the window closes (1 >= 6/6).
+    (b) white noise: tau = 1/2.  (c) AR(1) with coefficient phi: rho(k) = phi^k, tau = 1/2 + phi/(1 - phi).
+    (d) a symmetric +-1 walk on the ladder 0..T-1 reflected at the ends (what a chain with acceptance 1 on a flat
+    landscape does): rho(k) is the lazy-walk spectrum -- here checked against the exact autocorrelation from the
+    transition matrix.  (e) a constant or too short series gives NaN."""
+    assert oracle.walk_tau_int([0, 1, 1, 0]) == pytest.approx(1.0 / 6.0, abs=1e-15)
+    rng = np.random.default_rng(7)
+    n = 400000
+    assert oracle.walk_tau_int(rng.integers(0, 8, n)) == pytest.approx(0.5, abs=0.02)
+    for phi in (0.5, 0.9):
+        x = np.empty(n); x[0] = 0.0
+        eps = rng.standard_normal(n)
+        for i in range(1, n):
+            x[i] = phi * x[i - 1] + eps[i]
+        exact = 0.5 + phi / (1.0 - phi)
+        assert oracle.walk_tau_int(x) == pytest.approx(exact, rel=0.06)
+    # (d) lazy reflecting walk on T sites: P(i -> i+-1) = 1/2, a move off the ladder stays
+    T = 6
+    P = np.zeros((T, T))
+    for i in range(T):
+        for j in (i - 1, i + 1):
+            P[i, j if 0 <= j < T else i] += 0.5
+    pi = np.full(T, 1.0 / T); lab = np.arange(T) - (T - 1) / 2.0
+    c0 = float(pi @ lab ** 2)
+    rho, v = [], lab.copy()
+    for k in range(1, 2000):
+        v = P @ v
+        rho.append(float(pi @ (lab * v)) / c0)
+    exact = 0.5 + sum(rho)                      # rho decays like cos(pi/T)^k: converged long before k = 2000
+    steps = rng.integers(0, 2, n) * 2 - 1
+    x = np.empty(n, dtype=np.int32); pos = 0
+    for i in range(n):
+        j = pos + steps[i]
+        pos = j if 0 <= j < T else pos
+        x[i] = pos
+    assert oracle.walk_tau_int(x, window_c=10.0) == pytest.approx(exact, rel=0.08)
+    assert np.isnan(oracle.walk_tau_int([3, 3, 3, 3, 3])) and np.isnan(oracle.walk_tau_int([0, 1, 0]))
+
+
 # ---------------------------------------------------------------------------------------------
 # logarithmic data binning (Sect. III, PAPER.md:107): pins of oracle.logbin_index / logbin_observables / accumulate
 # ---------------------------------------------------------------------------------------------
