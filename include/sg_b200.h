@@ -54,6 +54,17 @@ typedef struct {
                                   exchange inside the Monte Carlo; overlaps are measured between the replicas a context holds */
     int32_t reserved;          /* must be 0 */
     uint64_t seed;             /* Philox key */
+    int32_t first_slot;        /* temperature-slot sharding of one chain (App. A.3: "each GPU updates only 2
+                                  lattices ... N_GPU = N_T"): the context holds the configurations (slots) [first_slot, first_slot +
+                                  n_temps) of every replica; the chain itself has n_temps_total temperatures */
+    int32_t n_temps_total;     /* length of the chain; 0 = n_temps (no slot sharding).  Else a multiple of n_temps, first_slot a
+                                  multiple of n_temps, betas passed to sg_create has n_temps_total entries.  Such a context draws
+                                  the numbers a single context holding the whole chain would (heat bath and initial spins are
+                                  keyed by the global copy id); it keeps the WHOLE temperature assignment of its chains, and
+                                  the PT step is sg_pt_publish -> all-gather of the energies -> sg_pt_swap_gathered, the same
+                                  decisions on every shard (identical Philox counters).  sg_pt_swap, sg_run_units, sg_measure,
+                                  sg_accumulate, sg_measure_chiral, sg_schwinger_dyson, sg_export_chirality return SG_EINVAL in
+                                  such a context; overlaps go through sg_export_replica / sg_measure_cross */
 } sg_shape;
 
 enum {
@@ -120,9 +131,27 @@ int sg_sweep_hb(sg_ctx* ctx, int n_sweeps);
  * are recomputed first if stale.  The PT counter advances by one. */
 int sg_pt_swap(sg_ctx* ctx);
 
+/* S4 when the slots of a chain are sharded over contexts (sg_shape.first_slot / n_temps_total; "the
+ * exchange with the master of a double precision number" per lattice and MCS, here an all-gather).
+ * sg_pt_publish: the total energies of this context's slots, double [S][R][n_temps] (recomputed first if stale), written
+ *   to the DEVICE buffer dev_out (caller-owned; the send buffer of the all-gather).  Asynchronous on the stream.
+ * sg_pt_swap_gathered: one PT sweep of every chain from the all-gathered energies, DEVICE buffer double [W][S][R][n_temps],
+ *   W = n_temps_total / n_temps, block w written by the context with first_slot = w * n_temps.  Every shard must call it
+ *   with the same buffer contents: all take the same decisions (PT stream keyed by chain, pair and PT counter), each keeps
+ *   the whole assignment and the statistics, and updates the betas of its own slots.  The PT counter advances by one.
+ *   Also valid without slot sharding (W = 1).  Asynchronous.
+ * sg_energy_by_temp: e = H/N of the copy of replica r at temperature t from such a gathered buffer through the current
+ *   assignment, host double [S][R][n_temps_total]; synchronises.
+ * Errors: SG_EINVAL (NULL), SG_ESTATE, SG_ECUDA. */
+int sg_pt_publish(sg_ctx* ctx, void* dev_out);
+int sg_pt_swap_gathered(sg_ctx* ctx, const void* dev_all);
+int sg_energy_by_temp(sg_ctx* ctx, const void* dev_all, double* e);
+
 /* n_units Monte Carlo steps (MCS, Sect. III, App. A.1): each is sg_sweep_hb(ctx, 1);
  * sg_sweep_or(ctx, n_or); sg_pt_swap(ctx), issued from native code so that small lattices are not bound by the
- * caller's per-call overhead.  Asynchronous on the stream; identical results to the three calls made one by one. */
+ * caller's per-call overhead; for small lattices (resident kernel) and n_units >= 8 one unit is captured in a CUDA graph and
+ * replayed (SG_TUNE_GRAPH).  Asynchronous on the stream; identical results to the three calls made
+ * one by one. */
 int sg_run_units(sg_ctx* ctx, int n_units, int n_or);
 
 /* S3 + S5.  Host outputs (any may be NULL):
@@ -216,6 +245,18 @@ int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts);
  *   label       int32  [S][R][T]  current label of every slot
  * Host outputs, either may be NULL.  Integer work: bit-exact against the oracle.  Synchronises. */
 int sg_pt_walk(sg_ctx* ctx, uint64_t* round_trips, int32_t* label);
+/* Histogram of that walk ("In a thermalized sample, all the replicas stay a significant amount of time at each
+ * temperature"): visits uint64 [S][R][T][T], visits[..][slot][t] = PT sweeps since creation after which the
+ * configuration in `slot` sat at temperature index t.  Kept on the device by every PT sweep when S*R*T*T*8 bytes <= 64 MiB
+ * (else SG_EINVAL).  Host output, required.  Integer work: bit-exact against the oracle.  Synchronises. */
+int sg_pt_visits(sg_ctx* ctx, uint64_t* visits);
+/* Integrated autocorrelation time of a recorded random walk in temperature ("the integrated autocorrelation
+ * time (mixing time) of the random walk in temperatures of each sample"; host arithmetic, no device work).
+ *   series: host int32 [n], the temperature index of one configuration after each PT sweep (e.g. temp_of_slot over time)
+ *   tau = 1/2 + sum_{k=1}^{W} rho(k),  rho(k) = C(k)/C(0),  C(k) = sum_{i<n-k} (x_i - m)(x_{i+k} - m) / (n - k),
+ *   m the mean of the series, summed up to the first W with W >= window_c * tau(W) (self-consistent window; window_c <= 0
+ *   means 6) or W = n/2.  Returns tau in PT sweeps; NaN when n < 4 or the series is constant. */
+double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c);
 
 /* ---- tuning (results do not depend on it beyond floating-point summation order) ----
  * SG_TUNE_SWEEP_IMPL: which half-sweep kernel serves sg_sweep_or / sg_sweep_hb / the energy pass.
@@ -237,8 +278,11 @@ int sg_pt_walk(sg_ctx* ctx, uint64_t* round_trips, int32_t* label);
  *   SG_MEASURE_AUTO    the streaming row kernel (thread = (lattice row, temperature), every replica's spin loaded once for
  *                      all pairs) when 2 <= R <= 4, else the staged kernel (default)
  *   SG_MEASURE_STAGED  the staged kernel (sites of all copies through shared memory; any R)
- *   Same products, fp32 row sums in the streaming kernel: results agree to ~1e-8. */
-enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2, SG_TUNE_PACKED = 3, SG_TUNE_MEASURE_IMPL = 4 };
+ *   Same products, fp32 row sums in the streaming kernel: results agree to ~1e-8.
+ * SG_TUNE_GRAPH: 1 (default) = sg_run_units captures one unit in a CUDA graph and replays it (the sweep counters patched in
+ *   the captured parameter blocks) when the resident kernel serves the sweeps and n_units >= 8; 0 = always issue the launches
+ *   one by one.  Same launches, same results. */
+enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2, SG_TUNE_PACKED = 3, SG_TUNE_MEASURE_IMPL = 4, SG_TUNE_GRAPH = 5 };
 enum { SG_MEASURE_AUTO = 0, SG_MEASURE_STAGED = 1 };
 enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2, SG_SWEEP_RESIDENT = 3 };
 int sg_tune(sg_ctx* ctx, int knob, int value);

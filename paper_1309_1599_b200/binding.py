@@ -12,7 +12,7 @@ _LIB_PATH = os.path.join(_HERE, "libsg_b200.so")
 GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2, 3, 4
 KIND_OR, KIND_HB = 0, 1
 SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
-TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES, TUNE_PACKED, TUNE_MEASURE_IMPL = 0, 1, 2, 3, 4
+TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES, TUNE_PACKED, TUNE_MEASURE_IMPL, TUNE_GRAPH = 0, 1, 2, 3, 4, 5
 MEASURE_AUTO, MEASURE_STAGED = 0, 1
 LOGBINS, LOGBIN_OBS = 32, 6
 SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT = 0, 1, 2, 3
@@ -20,9 +20,9 @@ SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT = 0, 1, 2, 3
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_init_sample_bimodal", "sg_sweep_or", "sg_sweep_hb",
-    "sg_pt_swap", "sg_run_units", "sg_measure", "sg_accumulate", "sg_get_logbins", "sg_export_replica", "sg_measure_cross", "sg_export_chirality", "sg_chiral_cross", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
+    "sg_pt_swap", "sg_pt_publish", "sg_pt_swap_gathered", "sg_energy_by_temp", "sg_run_units", "sg_measure", "sg_accumulate", "sg_get_logbins", "sg_export_replica", "sg_measure_cross", "sg_export_chirality", "sg_chiral_cross", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
-    "sg_halfsweep", "sg_pt_stats", "sg_pt_walk", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
+    "sg_halfsweep", "sg_pt_stats", "sg_pt_walk", "sg_pt_visits", "sg_walk_tau_int", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
 ]
 
@@ -31,7 +31,7 @@ class SgShape(ctypes.Structure):
     _fields_ = [("L", ctypes.c_int32), ("n_samples", ctypes.c_int32), ("n_replicas", ctypes.c_int32),
                 ("n_temps", ctypes.c_int32), ("first_sample", ctypes.c_int32), ("first_replica", ctypes.c_int32),
                 ("n_replicas_total", ctypes.c_int32), ("reserved", ctypes.c_int32),
-                ("seed", ctypes.c_uint64)]
+                ("seed", ctypes.c_uint64), ("first_slot", ctypes.c_int32), ("n_temps_total", ctypes.c_int32)]
 
 
 class SgError(RuntimeError):
@@ -63,6 +63,11 @@ def load_library():
     L.sg_sweep_or.argtypes = [vp, i]; L.sg_sweep_or.restype = i
     L.sg_sweep_hb.argtypes = [vp, i]; L.sg_sweep_hb.restype = i
     L.sg_pt_swap.argtypes = [vp]; L.sg_pt_swap.restype = i
+    L.sg_pt_publish.argtypes = [vp, vp]; L.sg_pt_publish.restype = i
+    L.sg_pt_swap_gathered.argtypes = [vp, vp]; L.sg_pt_swap_gathered.restype = i
+    L.sg_energy_by_temp.argtypes = [vp, vp, vp]; L.sg_energy_by_temp.restype = i
+    L.sg_pt_visits.argtypes = [vp, vp]; L.sg_pt_visits.restype = i
+    L.sg_walk_tau_int.argtypes = [vp, ctypes.c_int64, d]; L.sg_walk_tau_int.restype = d
     L.sg_measure.argtypes = [vp, vp, vp, vp]; L.sg_measure.restype = i
     L.sg_run_units.argtypes = [vp, i, i]; L.sg_run_units.restype = i
     L.sg_measure_chiral.argtypes = [vp, vp, vp]; L.sg_measure_chiral.restype = i
@@ -105,8 +110,14 @@ def _ptr(a):
 
 
 def workspace_bytes(L, n_samples, n_replicas, n_temps, seed=0, first_sample=0):
-    shape = SgShape(L, n_samples, n_replicas, n_temps, first_sample, 0, 0, 0, seed)
+    shape = SgShape(L, n_samples, n_replicas, n_temps, first_sample, 0, 0, 0, seed, 0, 0)
     return int(load_library().sg_workspace_bytes(ctypes.byref(shape)))
+
+
+def walk_tau_int(series, window_c=0.0):
+    """integrated autocorrelation time (in PT sweeps) of a recorded walk in temperature (sg_walk_tau_int)."""
+    x = np.ascontiguousarray(series, dtype=np.int32)
+    return float(load_library().sg_walk_tau_int(_ptr(x), int(x.size), float(window_c)))
 
 
 def correlation_length(L, chi0, chik):
@@ -125,12 +136,14 @@ class SpinGlass:
     """One context of the C-ABI library on the current CUDA device and torch's current stream."""
 
     def __init__(self, L, n_samples, n_replicas, n_temps, betas, seed=1, first_sample=0, device=None, stream=None,
-                 first_replica=0, n_replicas_total=0):
+                 first_replica=0, n_replicas_total=0, first_slot=0, n_temps_total=0):
         import torch
         self._lib = load_library()
         self.L, self.S, self.R, self.T = int(L), int(n_samples), int(n_replicas), int(n_temps)
         self.N, self.C, self.P = self.L ** 3, self.R * self.T, self.R * (self.R - 1) // 2
-        self.shape = SgShape(self.L, self.S, self.R, self.T, int(first_sample), int(first_replica), int(n_replicas_total), 0, int(seed))
+        self.Tt = int(n_temps_total) if n_temps_total else self.T      # length of the PT chain (> T: temperature-slot sharding)
+        self.shape = SgShape(self.L, self.S, self.R, self.T, int(first_sample), int(first_replica), int(n_replicas_total), 0, int(seed),
+                             int(first_slot), int(n_temps_total))
         nbytes = int(self._lib.sg_workspace_bytes(ctypes.byref(self.shape)))
         if nbytes == 0:
             raise SgError(SG_EINVAL, "sg_workspace_bytes")
@@ -142,8 +155,8 @@ class SpinGlass:
         aligned = (base + 255) & ~255
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         betas = np.ascontiguousarray(betas, dtype=np.float64)
-        if betas.shape != (self.T,):
-            raise SgError(SG_EINVAL, "sg_create (betas must have n_temps entries)")
+        if betas.shape != (self.Tt,):
+            raise SgError(SG_EINVAL, "sg_create (betas must have n_temps (n_temps_total) entries)")
         self._ctx = ctypes.c_void_p()
         rc = self._lib.sg_create(ctypes.byref(self._ctx), ctypes.byref(self.shape), _ptr(betas), ctypes.c_void_p(aligned),
                                  nbytes, ctypes.c_void_p(self.stream.cuda_stream))
@@ -198,6 +211,28 @@ class SpinGlass:
     def pt_swap(self):
         self._check(self._lib.sg_pt_swap(self._ctx), "sg_pt_swap")
 
+    def pt_publish(self, out=None):
+        """Device tensor float64 [S][R][T]: the total energies of this context's slots (the send buffer of the all-gather of a
+        slot-sharded chain; asynchronous)."""
+        import torch
+        if out is None:
+            out = torch.empty((self.S, self.R, self.T), dtype=torch.float64, device=self.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float64 and out.numel() == self.S * self.C
+        self._check(self._lib.sg_pt_publish(self._ctx, ctypes.c_void_p(out.data_ptr())), "sg_pt_publish")
+        return out
+
+    def pt_swap_gathered(self, gathered):
+        """One PT sweep from the all-gathered energies, device tensor float64 [W][S][R][T], W = n_temps_total / n_temps."""
+        assert gathered.is_cuda and gathered.is_contiguous() and gathered.numel() == (self.Tt // self.T) * self.S * self.C
+        self._check(self._lib.sg_pt_swap_gathered(self._ctx, ctypes.c_void_p(gathered.data_ptr())), "sg_pt_swap_gathered")
+
+    def energy_by_temp(self, gathered):
+        """e [S][R][n_temps_total] = H/N of the copy of replica r at temperature t, from the all-gathered energies."""
+        assert gathered.is_cuda and gathered.is_contiguous() and gathered.numel() == (self.Tt // self.T) * self.S * self.C
+        e = np.empty((self.S, self.R, self.Tt))
+        self._check(self._lib.sg_energy_by_temp(self._ctx, ctypes.c_void_p(gathered.data_ptr()), _ptr(e)), "sg_energy_by_temp")
+        return e
+
     def measure(self):
         e = np.empty((self.S, self.R, self.T)); q0 = np.empty((self.S, self.P, self.T))
         qk = np.empty((self.S, self.P, self.T, 3, 2))
@@ -243,13 +278,13 @@ class SpinGlass:
         return out
 
     def get_perm(self, sample):
-        tos = np.empty((self.R, self.T), dtype=np.int32); sot = np.empty((self.R, self.T), dtype=np.int32)
+        tos = np.empty((self.R, self.Tt), dtype=np.int32); sot = np.empty((self.R, self.Tt), dtype=np.int32)
         self._check(self._lib.sg_get_perm(self._ctx, int(sample), _ptr(tos), _ptr(sot)), "sg_get_perm")
         return tos, sot
 
     def set_perm(self, sample, temp_of_slot):
         tos = np.ascontiguousarray(temp_of_slot, dtype=np.int32)
-        assert tos.shape == (self.R, self.T)
+        assert tos.shape == (self.R, self.Tt)
         self._check(self._lib.sg_set_perm(self._ctx, int(sample), _ptr(tos)), "sg_set_perm")
 
     def get_energies(self):
@@ -274,7 +309,7 @@ class SpinGlass:
         self._check(self._lib.sg_halfsweep(self._ctx, int(kind), int(colour)), "sg_halfsweep")
 
     def pt_stats(self):
-        n = max(self.T - 1, 1)
+        n = max(self.Tt - 1, 1)
         att = np.zeros((self.S, self.R, n), dtype=np.uint64); acc = np.zeros((self.S, self.R, n), dtype=np.uint64)
         self._check(self._lib.sg_pt_stats(self._ctx, _ptr(att), _ptr(acc)), "sg_pt_stats")
         return att, acc
@@ -293,21 +328,21 @@ class SpinGlass:
     def export_buffer(self):
         """Uninitialised device tensor of the shape export_replica / export_chirality fill (a receive buffer)."""
         import torch
-        return torch.empty((self.S, 3, self.N, self.T), dtype=torch.float32, device=self.device)
+        return torch.empty((self.S, 3, self.N, self.Tt), dtype=torch.float32, device=self.device)
 
     def export_replica(self, r, out=None):
         """Device tensor float32 [S][3][N][T]: the configurations of local replica r ordered by temperature (asynchronous)."""
         import torch
         if out is None:
-            out = torch.empty((self.S, 3, self.N, self.T), dtype=torch.float32, device=self.device)
-        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float32 and out.numel() == self.S * 3 * self.N * self.T
+            out = torch.empty((self.S, 3, self.N, self.Tt), dtype=torch.float32, device=self.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float32 and out.numel() == self.S * 3 * self.N * self.Tt
         self._check(self._lib.sg_export_replica(self._ctx, int(r), ctypes.c_void_p(out.data_ptr())), "sg_export_replica")
         return out
 
     def measure_cross(self, r, remote):
         """(q0 [S][T], qk [S][T][3][2]) between local replica r and a partner's export_replica tensor (on this device)."""
-        assert remote.is_cuda and remote.is_contiguous() and remote.numel() == self.S * 3 * self.N * self.T
-        q0 = np.empty((self.S, self.T)); qk = np.empty((self.S, self.T, 3, 2))
+        assert remote.is_cuda and remote.is_contiguous() and remote.numel() == self.S * 3 * self.N * self.Tt
+        q0 = np.empty((self.S, self.Tt)); qk = np.empty((self.S, self.Tt, 3, 2))
         self._check(self._lib.sg_measure_cross(self._ctx, int(r), ctypes.c_void_p(remote.data_ptr()), _ptr(q0), _ptr(qk)),
                     "sg_measure_cross")
         return q0, qk
@@ -316,8 +351,8 @@ class SpinGlass:
         """Device tensor float32 [S][3][N][T]: zeta_{x,mu} of local replica r ordered by temperature (asynchronous)."""
         import torch
         if out is None:
-            out = torch.empty((self.S, 3, self.N, self.T), dtype=torch.float32, device=self.device)
-        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float32 and out.numel() == self.S * 3 * self.N * self.T
+            out = torch.empty((self.S, 3, self.N, self.Tt), dtype=torch.float32, device=self.device)
+        assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float32 and out.numel() == self.S * 3 * self.N * self.Tt
         self._check(self._lib.sg_export_chirality(self._ctx, int(r), ctypes.c_void_p(out.data_ptr())), "sg_export_chirality")
         return out
 
@@ -332,9 +367,15 @@ class SpinGlass:
 
     def pt_walk(self):
         """(round_trips uint64 [S][R], label int32 [S][R][T]) of the random walk in temperature."""
-        trips = np.zeros((self.S, self.R), dtype=np.uint64); lab = np.zeros((self.S, self.R, self.T), dtype=np.int32)
+        trips = np.zeros((self.S, self.R), dtype=np.uint64); lab = np.zeros((self.S, self.R, self.Tt), dtype=np.int32)
         self._check(self._lib.sg_pt_walk(self._ctx, _ptr(trips), _ptr(lab)), "sg_pt_walk")
         return trips, lab
+
+    def pt_visits(self):
+        """visits uint64 [S][R][T][T]: PT sweeps configuration `slot` has spent at temperature index t."""
+        v = np.zeros((self.S, self.R, self.Tt, self.Tt), dtype=np.uint64)
+        self._check(self._lib.sg_pt_visits(self._ctx, _ptr(v)), "sg_pt_visits")
+        return v
 
     def tune(self, knob, value):
         self._check(self._lib.sg_tune(self._ctx, int(knob), int(value)), "sg_tune")

@@ -19,6 +19,8 @@ struct sg_ctx {
     sg_shape shape;
     int L, N, Nh, S, R, T, C, NG, Cp, P;
     int Rt, Cg;           // replicas / copies per sample of the whole job (replica sharding; = R, C otherwise)
+    int Tt, slot0;        // length of the PT chain and first slot held (temperature-slot sharding; = T, 0 otherwise); T = slots held
+    unsigned long long* visits;   // [S][R][Tt][Tt] histogram of the walk in temperature, nullptr when too large
     uint32_t g_first;     // global copy id of (local sample 0, local copy 0)
     cudaStream_t stream;
     // device arrays (carved from the caller's workspace)
@@ -54,6 +56,14 @@ struct sg_ctx {
     uint64_t hb_counter, pt_counter, launches;
     bool energies_fresh;
     int last_cuda;
+    // CUDA-graph replay of a unit (sg_run_units): while `capturing`, every launch whose parameter block carries the HB or
+    // PT counter notes its graph node, so that the counter can be patched before each replay
+    struct CounterNode { cudaGraphNode_t node; int which; size_t offset, size; };
+    bool capturing = false;
+    std::vector<CounterNode> counter_nodes;
+    cudaStream_t gstream = nullptr;      // capture / replay stream when the context's own stream is the legacy default stream
+    cudaEvent_t gevent = nullptr;
+    int graph_mode = 1;                  // SG_TUNE_GRAPH: 1 = sg_run_units replays a captured unit when it pays
 };
 
 namespace {
@@ -68,16 +78,21 @@ bool shape_ok(const sg_shape* s)
     if (s->reserved != 0 || s->first_replica < 0) return false;
     if (s->n_replicas_total != 0 && s->first_replica + s->n_replicas > s->n_replicas_total) return false;
     if (s->n_replicas_total == 0 && s->first_replica != 0) return false;
+    if (s->first_slot < 0 || s->n_temps_total < 0) return false;
+    if (s->n_temps_total == 0 && s->first_slot != 0) return false;
+    if (s->n_temps_total != 0 && (s->n_temps_total % s->n_temps != 0 || s->first_slot % s->n_temps != 0 ||
+                                  s->first_slot + s->n_temps > s->n_temps_total)) return false;
     const double N = (double)s->L * s->L * s->L;
     const double C = (double)s->n_replicas * s->n_temps;
-    if (N > 2.0e9 || C > 1.0e6) return false;
-    if (((double)s->first_sample + s->n_samples) * C > 4.0e9) return false;   // copy ids are 32-bit counters
+    const double Cjob = (double)(s->n_replicas_total ? s->n_replicas_total : s->n_replicas) * (s->n_temps_total ? s->n_temps_total : s->n_temps);
+    if (N > 2.0e9 || Cjob > 1.0e6) return false;
+    if (((double)s->first_sample + s->n_samples) * Cjob > 4.0e9) return false;   // copy ids are 32-bit counters
     if ((double)s->n_samples * std::ceil(C / 32.0) * N * 96.0 > 4.0e11) return false;
     return true;
 }
 
 struct Geometry {
-    int L, N, Nh, S, R, T, C, NG, Cp, P, tile_sites, ntiles, nchunk, chunk_sites, MS;
+    int L, N, Nh, S, R, T, Tt, C, NG, Cp, P, tile_sites, ntiles, nchunk, chunk_sites, MS;
     int mq_nchunk, mq_rows_per_cta, mq_Tw, mq_rows_t;
 };
 
@@ -86,6 +101,7 @@ Geometry geometry(const sg_shape* s)
     Geometry g;
     g.L = s->L; g.N = s->L * s->L * s->L; g.Nh = g.N / 2;
     g.S = s->n_samples; g.R = s->n_replicas; g.T = s->n_temps; g.C = g.R * g.T;
+    g.Tt = s->n_temps_total ? s->n_temps_total : s->n_temps;
     g.NG = (g.C + G - 1) / G; g.Cp = g.NG * G; g.P = g.R * (g.R - 1) / 2;
     // sweep tiles: 128 consecutive same-colour sites per CTA (4 passes of 32 site slots)
     g.tile_sites = 128;
@@ -109,13 +125,20 @@ Geometry geometry(const sg_shape* s)
     return g;
 }
 
+// histogram of the walk in temperature, [S][R][Tt][Tt] uint64: kept when it is at most 64 MiB
+size_t visits_bytes(const Geometry& g)
+{
+    const double b = (double)g.S * g.R * (double)g.Tt * g.Tt * sizeof(unsigned long long);
+    return (b <= 64.0 * 1024 * 1024) ? (size_t)b : 0;
+}
+
 struct Carve {
     size_t off = 0;
     size_t take(size_t bytes) { size_t o = off; off += align256(bytes); return o; }
 };
 
 struct Offsets {
-    size_t spins, Jg, Jt, Jp, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, logbin, xpart, total;
+    size_t spins, Jg, Jt, Jp, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, visits, logbin, xpart, total;
 };
 
 Offsets offsets(const Geometry& g)
@@ -129,7 +152,7 @@ Offsets offsets(const Geometry& g)
     size_t stg = (size_t)G * 3 * g.N * sizeof(float);
     o.staging = c.take(stg);
     o.beta_slot = c.take((size_t)g.S * g.Cp * sizeof(float));
-    o.betas = c.take((size_t)g.T * sizeof(double));
+    o.betas = c.take((size_t)g.Tt * sizeof(double));
     o.E = c.take((size_t)g.S * g.Cp * sizeof(double));
     o.Epart = c.take((size_t)g.S * g.NG * g.ntiles * G * sizeof(double));
     o.SDpart = c.take((size_t)g.S * g.NG * 2 * g.ntiles * G * 2 * sizeof(double));
@@ -139,14 +162,15 @@ Offsets offsets(const Geometry& g)
         const size_t a = (size_t)g.nchunk * 21, b = (size_t)g.mq_nchunk * 7;
         o.Mpart = c.take((size_t)g.S * items * (a > b ? a : b) * sizeof(double));
     }
-    o.result = c.take(((size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + (size_t)g.S * g.T * 21 + 1) * sizeof(double));
-    o.sot = c.take((size_t)g.S * g.R * g.T * sizeof(int));
-    o.tos = c.take((size_t)g.S * g.R * g.T * sizeof(int));
-    size_t st = (size_t)g.S * g.R * (g.T > 1 ? g.T - 1 : 1) * sizeof(unsigned long long);
+    o.result = c.take(((size_t)g.S * g.R * g.Tt + (size_t)g.S * g.P * g.Tt * 21 + (size_t)g.S * g.Tt * 21 + 1) * sizeof(double));
+    o.sot = c.take((size_t)g.S * g.R * g.Tt * sizeof(int));
+    o.tos = c.take((size_t)g.S * g.R * g.Tt * sizeof(int));
+    size_t st = (size_t)g.S * g.R * (g.Tt > 1 ? g.Tt - 1 : 1) * sizeof(unsigned long long);
     o.att = c.take(st);
     o.acc = c.take(st);
-    o.wlab = c.take((size_t)g.S * g.R * g.T * sizeof(int));
+    o.wlab = c.take((size_t)g.S * g.R * g.Tt * sizeof(int));
     o.trips = c.take((size_t)g.S * g.R * sizeof(unsigned long long));
+    o.visits = c.take(visits_bytes(g));
     o.logbin = c.take((size_t)SG_LOGBINS * g.S * g.T * SG_LOGBIN_OBS * sizeof(double));
     o.xpart = c.take((size_t)g.S * XCHUNKS * XTHREADS * 21 * sizeof(double));   // rows * T <= XTHREADS when T <= XTHREADS
     o.total = c.off;
@@ -171,6 +195,21 @@ int cuda_fail(sg_ctx* ctx, cudaError_t e)
         cudaError_t e__ = cudaGetLastError();                 \
         if (e__ != cudaSuccess) return cuda_fail((ctx), e__); \
     } while (0)
+
+// during the capture of a unit: remember the node of the launch just made if its parameter block holds a sweep counter
+// (which: 0 = HB counter, 1 = PT counter; offset / size: of the counter inside / of the parameter block)
+void note_counter_node(sg_ctx* ctx, cudaStream_t stream, int which, size_t offset, size_t size)
+{
+    if (!ctx->capturing) return;
+    cudaStreamCaptureStatus st;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t ndeps = 0;
+    if (cudaStreamGetCaptureInfo(stream, &st, nullptr, nullptr, &deps, &ndeps) != cudaSuccess || st != cudaStreamCaptureStatusActive || ndeps != 1) {
+        ctx->counter_nodes.push_back({ nullptr, -1, 0, 0 });     // marks the capture as unusable
+        return;
+    }
+    ctx->counter_nodes.push_back({ deps[0], which, offset, size });
+}
 
 int ilog2_exact(int L)
 {
@@ -327,7 +366,7 @@ int half_sweep_zm(sg_ctx* ctx, int kind, int colour, bool with_energy)
     p.colour = colour;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.hb_counter = (uint32_t)ctx->hb_counter;
-    p.g_first = ctx->g_first; p.Cg = ctx->Cg;
+    p.g_first = ctx->g_first; p.Cg = ctx->Cg; p.Tl = ctx->T; p.Tpad = ctx->Tt - ctx->T;
     const int nblk = p.ntx * p.nty * p.nzc;
     const dim3 grid(nblk * ctx->NG, ctx->S);
     int rc;
@@ -336,6 +375,7 @@ int half_sweep_zm(sg_ctx* ctx, int kind, int colour, bool with_energy)
     else rc = launch_zm<KIND_ENERGY, true>(ctx, p, grid);
     if (rc != SG_OK) return rc;
     SG_LAUNCHED(ctx);
+    if (kind == KIND_HB) note_counter_node(ctx, ctx->stream, 0, offsetof(ZmParams, hb_counter), sizeof(ZmParams));
     if (with_energy || kind == KIND_ENERGY) {
         k_reduce_energy<<<ctx->S * ctx->NG, 256, 0, ctx->stream>>>(ctx->Epart, ctx->E, nblk);
         SG_LAUNCHED(ctx);
@@ -356,7 +396,7 @@ int half_sweep(sg_ctx* ctx, int kind, int colour, bool with_energy)
     p.tile_sites = ctx->tile_sites; p.colour = colour; p.C = ctx->C;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.hb_counter = (uint32_t)ctx->hb_counter;
-    p.g_first = ctx->g_first; p.Cg = ctx->Cg;
+    p.g_first = ctx->g_first; p.Cg = ctx->Cg; p.Tl = ctx->T; p.Tpad = ctx->Tt - ctx->T;
     const dim3 grid(ctx->ntiles * ctx->NG, ctx->S);
     if (kind == KIND_OR) {
         if (with_energy) launch_sweep_l<KIND_OR, true>(ctx, p, grid);
@@ -368,6 +408,7 @@ int half_sweep(sg_ctx* ctx, int kind, int colour, bool with_energy)
         launch_sweep_l<KIND_ENERGY, true>(ctx, p, grid);
     }
     SG_LAUNCHED(ctx);
+    if (kind == KIND_HB) note_counter_node(ctx, ctx->stream, 0, offsetof(SweepParams, hb_counter), sizeof(SweepParams));
     if (with_energy || kind == KIND_ENERGY) {
         k_reduce_energy<<<ctx->S * ctx->NG, 256, 0, ctx->stream>>>(ctx->Epart, ctx->E, ctx->ntiles);
         SG_LAUNCHED(ctx);
@@ -407,7 +448,7 @@ int fill_beta_slot(sg_ctx* ctx)
 {
     const int n = ctx->S * ctx->Cp;
     k_fill_beta_slot<<<(n + 255) / 256, 256, 0, ctx->stream>>>(ctx->betas, ctx->temp_of_slot, ctx->beta_slot, ctx->S,
-                                                              ctx->R, ctx->T, ctx->Cp);
+                                                              ctx->R, ctx->Tt, ctx->T, ctx->slot0, ctx->Cp);
     SG_LAUNCHED(ctx);
     return SG_OK;
 }
@@ -472,9 +513,10 @@ int sweeps_resident(sg_ctx* ctx, int kind, int n_sweeps)
     p.n_sweeps = n_sweeps;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.hb_counter = (uint32_t)ctx->hb_counter;
-    p.g_first = ctx->g_first; p.Cg = ctx->Cg;
+    p.g_first = ctx->g_first; p.Cg = ctx->Cg; p.Tl = ctx->T; p.Tpad = ctx->Tt - ctx->T;
     if (int rc = (kind == KIND_HB) ? launch_res<1>(ctx, p) : launch_res<0>(ctx, p)) return rc;
     SG_LAUNCHED(ctx);
+    if (kind == KIND_HB) note_counter_node(ctx, ctx->stream, 0, offsetof(ResParams, hb_counter), sizeof(ResParams));
     if (kind == KIND_HB) ctx->hb_counter += (uint64_t)n_sweeps;
     ctx->energies_fresh = true;
     return SG_OK;
@@ -530,11 +572,12 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     *out = nullptr;
     if (!shape_ok(shape) || !betas || !dev_workspace) return SG_EINVAL;
     if (((uintptr_t)dev_workspace & 255) != 0) return SG_EINVAL;
-    for (int t = 0; t < shape->n_temps; ++t)
+    const int n_betas = shape->n_temps_total ? shape->n_temps_total : shape->n_temps;   // the whole chain
+    for (int t = 0; t < n_betas; ++t)
         if (!std::isfinite(betas[t])) return SG_EINVAL;
-    if (shape->n_temps > 1) {
+    if (n_betas > 1) {
         const bool up = betas[1] > betas[0];
-        for (int t = 1; t < shape->n_temps; ++t)
+        for (int t = 1; t < n_betas; ++t)
             if (up ? !(betas[t] > betas[t - 1]) : !(betas[t] < betas[t - 1])) return SG_EINVAL;
     }
     const Geometry g = geometry(shape);
@@ -546,8 +589,9 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->shape = *shape;
     ctx->L = g.L; ctx->N = g.N; ctx->Nh = g.Nh; ctx->S = g.S; ctx->R = g.R; ctx->T = g.T; ctx->C = g.C;
     ctx->NG = g.NG; ctx->Cp = g.Cp; ctx->P = g.P;
-    ctx->Rt = shape->n_replicas_total ? shape->n_replicas_total : g.R; ctx->Cg = ctx->Rt * g.T;
-    ctx->g_first = (uint32_t)shape->first_sample * (uint32_t)ctx->Cg + (uint32_t)shape->first_replica * (uint32_t)g.T;
+    ctx->Tt = g.Tt; ctx->slot0 = shape->first_slot;
+    ctx->Rt = shape->n_replicas_total ? shape->n_replicas_total : g.R; ctx->Cg = ctx->Rt * g.Tt;
+    ctx->g_first = (uint32_t)shape->first_sample * (uint32_t)ctx->Cg + (uint32_t)shape->first_replica * (uint32_t)g.Tt + (uint32_t)shape->first_slot;
     ctx->tile_sites = g.tile_sites; ctx->ntiles = g.ntiles; ctx->log2L = ilog2_exact(g.L);
     ctx->nchunk = g.nchunk; ctx->chunk_sites = g.chunk_sites; ctx->MS = g.MS;
     ctx->mq_nchunk = g.mq_nchunk; ctx->mq_rows_per_cta = g.mq_rows_per_cta; ctx->mq_Tw = g.mq_Tw; ctx->mq_rows_t = g.mq_rows_t;
@@ -559,7 +603,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->SDpart = (double*)(base + o.SDpart);
     ctx->phase = (double*)(base + o.phase); ctx->Mpart = (double*)(base + o.Mpart);
     ctx->result = (double*)(base + o.result);
-    ctx->result_doubles = (size_t)g.S * g.R * g.T + (size_t)g.S * g.P * g.T * 21 + (size_t)g.S * g.T * 21 + 1;
+    ctx->result_doubles = (size_t)g.S * g.R * g.Tt + (size_t)g.S * g.P * g.Tt * 21 + (size_t)g.S * g.Tt * 21 + 1;
     if (cudaHostAlloc((void**)&ctx->h_result, ctx->result_doubles * sizeof(double), cudaHostAllocDefault) != cudaSuccess) {
         ctx->h_result = nullptr;   // fall back to direct copies into the caller's arrays
         cudaGetLastError();
@@ -567,10 +611,11 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->slot_of_temp = (int*)(base + o.sot); ctx->temp_of_slot = (int*)(base + o.tos);
     ctx->attempts = (unsigned long long*)(base + o.att); ctx->accepts = (unsigned long long*)(base + o.acc);
     ctx->walk_label = (int*)(base + o.wlab); ctx->round_trips = (unsigned long long*)(base + o.trips);
+    ctx->visits = visits_bytes(g) ? (unsigned long long*)(base + o.visits) : nullptr;
     ctx->logbin = (double*)(base + o.logbin); ctx->n_acc = 0;
     ctx->Xpart = (double*)(base + o.xpart);
     for (int b = 0; b < SG_LOGBINS; ++b) ctx->n_acc_cg[b] = 0;
-    ctx->h_betas.assign(betas, betas + g.T);
+    ctx->h_betas.assign(betas, betas + g.Tt);
     ctx->inited.assign(g.S, 0);
     ctx->bimodal_D.assign(g.S, std::nan("")); ctx->packed_on = 0;
     ctx->hb_counter = ctx->pt_counter = ctx->launches = 0;
@@ -587,16 +632,17 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
         phase[2 * x] = std::cos(2.0 * kPi * (double)x / (double)g.L);
         phase[2 * x + 1] = std::sin(2.0 * kPi * (double)x / (double)g.L);
     }
-    std::vector<int> ident((size_t)g.S * g.R * g.T);
-    for (size_t k = 0; k < ident.size(); ++k) ident[k] = (int)(k % g.T);
-    cudaError_t e = cudaMemcpyAsync(ctx->betas, betas, g.T * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
+    std::vector<int> ident((size_t)g.S * g.R * g.Tt);
+    for (size_t k = 0; k < ident.size(); ++k) ident[k] = (int)(k % g.Tt);
+    cudaError_t e = cudaMemcpyAsync(ctx->betas, betas, g.Tt * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->phase, phase.data(), phase.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->slot_of_temp, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->temp_of_slot, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
-    const size_t st = (size_t)g.S * g.R * (g.T > 1 ? g.T - 1 : 1) * sizeof(unsigned long long);
+    const size_t st = (size_t)g.S * g.R * (g.Tt > 1 ? g.Tt - 1 : 1) * sizeof(unsigned long long);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->attempts, 0, st, ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->accepts, 0, st, ctx->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->walk_label, 0, (size_t)g.S * g.R * g.T * sizeof(int), ctx->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->walk_label, 0, (size_t)g.S * g.R * g.Tt * sizeof(int), ctx->stream);
+    if (e == cudaSuccess && ctx->visits) e = cudaMemsetAsync(ctx->visits, 0, visits_bytes(g), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->round_trips, 0, (size_t)g.S * g.R * sizeof(unsigned long long), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->logbin, 0, (size_t)SG_LOGBINS * g.S * g.T * SG_LOGBIN_OBS * sizeof(double), ctx->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->E, 0, (size_t)g.S * g.Cp * sizeof(double), ctx->stream);
@@ -612,6 +658,8 @@ int sg_destroy(sg_ctx* ctx)
 {
     if (!ctx) return SG_EINVAL;
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->gstream) { cudaStreamSynchronize(ctx->gstream); cudaStreamDestroy(ctx->gstream); }
+    if (ctx->gevent) cudaEventDestroy(ctx->gevent);
     if (ctx->h_result) cudaFreeHost(ctx->h_result);
     delete ctx;
     return SG_OK;
@@ -678,14 +726,14 @@ int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const 
         const size_t nthr = (size_t)ctx->NG * ctx->N * 8;
         const uint32_t g_sample = ctx->g_first + (uint32_t)sample * (uint32_t)ctx->Cg;
         k_init_spins<<<(unsigned)((nthr + 255) / 256), 256, 0, ctx->stream>>>(
-            ctx->spins + (size_t)sample * ctx->NG * ctx->N * SITE_FLOATS, ctx->L, ctx->N, ctx->NG, ctx->C, g_sample,
+            ctx->spins + (size_t)sample * ctx->NG * ctx->N * SITE_FLOATS, ctx->L, ctx->N, ctx->NG, ctx->C, g_sample, ctx->T, ctx->Tt - ctx->T,
             (uint32_t)(ctx->shape.seed & 0xffffffffu), (uint32_t)(ctx->shape.seed >> 32));
         SG_LAUNCHED(ctx);
     }
     // identity temperature assignment for this sample
-    std::vector<int> ident((size_t)ctx->R * ctx->T);
-    for (size_t k = 0; k < ident.size(); ++k) ident[k] = (int)(k % ctx->T);
-    const size_t off = (size_t)sample * ctx->R * ctx->T;
+    std::vector<int> ident((size_t)ctx->R * ctx->Tt);
+    for (size_t k = 0; k < ident.size(); ++k) ident[k] = (int)(k % ctx->Tt);
+    const size_t off = (size_t)sample * ctx->R * ctx->Tt;
     SG_CUDA(ctx, cudaMemcpyAsync(ctx->slot_of_temp + off, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
     SG_CUDA(ctx, cudaMemcpyAsync(ctx->temp_of_slot + off, ident.data(), ident.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -756,40 +804,169 @@ int sg_halfsweep(sg_ctx* ctx, int kind, int colour)
     return half_sweep(ctx, kind, colour, false);
 }
 
-int sg_pt_swap(sg_ctx* ctx)
+// one PT sweep of every chain from the energies E: local (E_wstride unused) or all-gathered [W][S][R][T] (slot sharding)
+static int pt_launch(sg_ctx* ctx, const double* E, long long E_sstride, long long E_wstride)
 {
-    if (!ctx) return SG_EINVAL;
-    if (int rc = all_inited(ctx)) return rc;
-    if (int rc = ensure_energies(ctx)) return rc;
     PtParams p;
-    p.betas = ctx->betas; p.E = ctx->E; p.slot_of_temp = ctx->slot_of_temp; p.temp_of_slot = ctx->temp_of_slot;
+    p.betas = ctx->betas; p.E = E; p.slot_of_temp = ctx->slot_of_temp; p.temp_of_slot = ctx->temp_of_slot;
     p.beta_slot = ctx->beta_slot; p.attempts = ctx->attempts; p.accepts = ctx->accepts;
-    p.walk_label = ctx->walk_label; p.round_trips = ctx->round_trips;
-    p.S = ctx->S; p.R = ctx->R; p.T = ctx->T; p.Cp = ctx->Cp;
+    p.walk_label = ctx->walk_label; p.round_trips = ctx->round_trips; p.visits = ctx->visits;
+    p.S = ctx->S; p.R = ctx->R; p.T = ctx->Tt; p.Cp = ctx->Cp;
+    p.Tl = ctx->T; p.slot0 = ctx->slot0; p.E_sstride = E_sstride; p.E_wstride = E_wstride;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.pt_counter = (uint32_t)ctx->pt_counter;
     p.chain_first = (uint32_t)ctx->shape.first_sample * (uint32_t)ctx->Rt + (uint32_t)ctx->shape.first_replica; p.Rt = ctx->Rt;
     const int chains = ctx->S * ctx->R;
-    k_pt_swap<<<(chains + 63) / 64, 64, 0, ctx->stream>>>(p);
+    const size_t smem = (size_t)ctx->Tt * PT_SMEM_PER_TEMP;
+    if (smem <= 40 * 1024) k_pt_swap<<<chains, 32, smem, ctx->stream>>>(p);             // a warp per chain, the chain in shared memory
+    else k_pt_swap_serial<<<(chains + 63) / 64, 64, 0, ctx->stream>>>(p);
     SG_LAUNCHED(ctx);
+    note_counter_node(ctx, ctx->stream, 1, offsetof(PtParams, pt_counter), sizeof(PtParams));
     ctx->pt_counter += 1;
     return SG_OK;
 }
 
+int sg_pt_swap(sg_ctx* ctx)
+{
+    if (!ctx || ctx->Tt != ctx->T) return SG_EINVAL;     // a slot-sharded chain needs the other shards' energies: sg_pt_swap_gathered
+    if (int rc = all_inited(ctx)) return rc;
+    if (int rc = ensure_energies(ctx)) return rc;
+    return pt_launch(ctx, ctx->E, ctx->Cp, 0);
+}
+
+int sg_pt_publish(sg_ctx* ctx, void* dev_out)
+{
+    if (!ctx || !dev_out) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    if (int rc = ensure_energies(ctx)) return rc;
+    SG_CUDA(ctx, cudaMemcpy2DAsync(dev_out, (size_t)ctx->C * sizeof(double), ctx->E, (size_t)ctx->Cp * sizeof(double),
+                                   (size_t)ctx->C * sizeof(double), ctx->S, cudaMemcpyDeviceToDevice, ctx->stream));
+    return SG_OK;
+}
+
+int sg_pt_swap_gathered(sg_ctx* ctx, const void* dev_all)
+{
+    if (!ctx || !dev_all) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    return pt_launch(ctx, (const double*)dev_all, (long long)ctx->R * ctx->T, (long long)ctx->S * ctx->R * ctx->T);
+}
+
+int sg_energy_by_temp(sg_ctx* ctx, const void* dev_all, double* e)
+{
+    if (!ctx || !dev_all || !e) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    const int n = ctx->S * ctx->R * ctx->Tt;
+    k_energy_by_temp<<<(n + 127) / 128, 128, 0, ctx->stream>>>((const double*)dev_all, ctx->slot_of_temp, ctx->result, ctx->S, ctx->R, ctx->Tt,
+                                                            ctx->T, ctx->N);
+    SG_LAUNCHED(ctx);
+    SG_CUDA(ctx, cudaMemcpyAsync(e, ctx->result, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+static int one_unit(sg_ctx* ctx, int n_or)
+{
+    if (int rc = sg_sweep_hb(ctx, 1)) return rc;
+    if (int rc = sg_sweep_or(ctx, n_or)) return rc;
+    return sg_pt_swap(ctx);
+}
+
+// Units u0 .. n_units-1 as replays of ONE captured unit ("CUDA-graph capture of a unit").  The launches
+// of a unit are the same from unit to unit except for the HB and PT sweep counters inside two or three parameter blocks; those
+// nodes are noted during the capture (note_counter_node) and patched before every replay.  Returns SG_OK with *done = false
+// when the capture is not possible (the caller then issues the units one by one).
+static int replay_units(sg_ctx* ctx, int n_units, int n_or, bool* done)
+{
+    *done = false;
+    cudaStream_t user = ctx->stream, cap = ctx->stream;
+    if (user == nullptr || user == cudaStreamLegacy || user == cudaStreamPerThread) {
+        // the legacy default stream cannot be captured: replay on a stream of our own, ordered after / before the caller's by events
+        if (!ctx->gstream) {
+            if (cudaStreamCreateWithFlags(&ctx->gstream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); ctx->gstream = nullptr; return SG_OK; }
+            if (cudaEventCreateWithFlags(&ctx->gevent, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); cudaStreamDestroy(ctx->gstream); ctx->gstream = nullptr; return SG_OK; }
+        }
+        cap = ctx->gstream;
+        SG_CUDA(ctx, cudaEventRecord(ctx->gevent, user));
+        SG_CUDA(ctx, cudaStreamWaitEvent(cap, ctx->gevent, 0));
+    }
+    const uint64_t hb0 = ctx->hb_counter, pt0 = ctx->pt_counter, launches0 = ctx->launches;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    ctx->counter_nodes.clear();
+    if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return SG_OK; }
+    ctx->stream = cap; ctx->capturing = true;
+    const int rc_cap = one_unit(ctx, n_or);
+    ctx->capturing = false; ctx->stream = user;
+    const cudaError_t e_end = cudaStreamEndCapture(cap, &graph);
+    const uint64_t per_unit = ctx->launches - launches0;
+    ctx->hb_counter = hb0; ctx->pt_counter = pt0; ctx->launches = launches0;      // nothing ran
+    bool ok = rc_cap == SG_OK && e_end == cudaSuccess && graph != nullptr;
+    for (const auto& cn : ctx->counter_nodes) ok = ok && cn.node != nullptr;
+    if (ok && cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) ok = false;
+    struct Patch { cudaKernelNodeParams np; std::vector<unsigned char> block; void* args[1]; int which; size_t offset; uint32_t base; };
+    std::vector<Patch> patches(ok ? ctx->counter_nodes.size() : 0);
+    for (size_t k = 0; ok && k < patches.size(); ++k) {
+        const auto& cn = ctx->counter_nodes[k];
+        Patch& pa = patches[k];
+        if (cudaGraphKernelNodeGetParams(cn.node, &pa.np) != cudaSuccess || !pa.np.kernelParams) { ok = false; break; }
+        pa.block.assign((const unsigned char*)pa.np.kernelParams[0], (const unsigned char*)pa.np.kernelParams[0] + cn.size);
+        pa.which = cn.which; pa.offset = cn.offset;
+        std::memcpy(&pa.base, pa.block.data() + cn.offset, sizeof(uint32_t));     // the counter the capture saw
+    }
+    int rc = SG_OK;
+    if (ok) {
+        for (int u = 0; u < n_units && rc == SG_OK; ++u) {
+            for (Patch& pa : patches) {
+                const uint32_t v = pa.base + (uint32_t)u;     // both counters advance by one per unit
+                std::memcpy(pa.block.data() + pa.offset, &v, sizeof(uint32_t));
+                pa.args[0] = pa.block.data();
+                pa.np.kernelParams = pa.args; pa.np.extra = nullptr;
+                cudaGraphNode_t node = ctx->counter_nodes[&pa - patches.data()].node;
+                if (cudaGraphExecKernelNodeSetParams(exec, node, &pa.np) != cudaSuccess) { rc = cuda_fail(ctx, cudaGetLastError()); break; }
+            }
+            if (rc != SG_OK) break;
+            const cudaError_t e = cudaGraphLaunch(exec, cap);
+            if (e != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
+            ctx->hb_counter += 1; ctx->pt_counter += 1; ctx->launches += per_unit;
+        }
+        ctx->energies_fresh = true;
+        *done = (rc == SG_OK);
+    } else {
+        cudaGetLastError();
+    }
+    if (exec) cudaGraphExecDestroy(exec);
+    if (graph) cudaGraphDestroy(graph);
+    ctx->counter_nodes.clear();
+    if (cap != user) {
+        cudaEventRecord(ctx->gevent, cap);
+        cudaStreamWaitEvent(user, ctx->gevent, 0);
+    }
+    return rc;
+}
+
 int sg_run_units(sg_ctx* ctx, int n_units, int n_or)
 {
-    if (!ctx || n_units < 0 || n_or < 0) return SG_EINVAL;
-    for (int u = 0; u < n_units; ++u) {
-        if (int rc = sg_sweep_hb(ctx, 1)) return rc;
-        if (int rc = sg_sweep_or(ctx, n_or)) return rc;
-        if (int rc = sg_pt_swap(ctx)) return rc;
+    if (!ctx || n_units < 0 || n_or < 0 || ctx->Tt != ctx->T) return SG_EINVAL;
+    if (int rc = all_inited(ctx)) return rc;
+    int u = 0;
+    // Replaying a captured unit pays when a unit is a handful of short launches (the resident kernel: L <= 12) and there are
+    // enough units to amortise the capture; the first unit always runs directly (it sets the kernels' attributes).
+    if (ctx->graph_mode && n_units >= 8 && use_resident(ctx)) {
+        if (int rc = one_unit(ctx, n_or)) return rc;
+        u = 1;
+        bool done = false;
+        if (int rc = replay_units(ctx, n_units - 1, n_or, &done)) return rc;
+        if (done) return SG_OK;
     }
+    for (; u < n_units; ++u)
+        if (int rc = one_unit(ctx, n_or)) return rc;
     return SG_OK;
 }
 
 // S3 + S5 into ctx->result = [ e | q0 | qk ] (asynchronous); with_q = false skips the overlap pass
 static int launch_measure(sg_ctx* ctx, bool with_q)
 {
+    if (ctx->Tt != ctx->T) return SG_EINVAL;      // slot-sharded: sg_energy_by_temp, sg_export_replica / sg_measure_cross
     if (int rc = all_inited(ctx)) return rc;
     if (int rc = ensure_energies(ctx)) return rc;
     const int PT = ctx->P * ctx->T;
@@ -910,7 +1087,7 @@ static int launch_measure_chiral(sg_ctx* ctx)
 
 int sg_measure_chiral(sg_ctx* ctx, double* qc0, double* qck)
 {
-    if (!ctx) return SG_EINVAL;
+    if (!ctx || ctx->Tt != ctx->T) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     const int PT = ctx->P * ctx->T;
     const int nQ = ctx->S * PT;
@@ -935,27 +1112,27 @@ int sg_export_replica(sg_ctx* ctx, int r, void* dev_out)
 {
     if (!ctx || !dev_out || r < 0 || r >= ctx->R) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
-    const size_t n = (size_t)ctx->N * ctx->T;
+    const size_t n = (size_t)ctx->N * ctx->Tt;
     k_export_by_temp<<<dim3((unsigned)((n + 255) / 256), ctx->S), 256, 0, ctx->stream>>>(ctx->spins, ctx->slot_of_temp, (float*)dev_out, ctx->L,
-                                                                                      ctx->N, ctx->NG, ctx->R, ctx->T, r);
+                                                                                      ctx->N, ctx->NG, ctx->R, ctx->Tt, ctx->T, ctx->slot0, r);
     SG_LAUNCHED(ctx);
     return SG_OK;
 }
 
 int sg_measure_cross(sg_ctx* ctx, int r, const void* dev_remote, double* q0, double* qk)
 {
-    if (!ctx || !dev_remote || r < 0 || r >= ctx->R || ctx->T > XTHREADS) return SG_EINVAL;
+    if (!ctx || !dev_remote || r < 0 || r >= ctx->R || ctx->Tt > XTHREADS) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     CrossParams p;
     p.spins = ctx->spins; p.slot_of_temp = ctx->slot_of_temp; p.remote = (const float*)dev_remote; p.phase = ctx->phase; p.Xpart = ctx->Xpart;
-    p.L = ctx->L; p.N = ctx->N; p.NG = ctx->NG; p.R = ctx->R; p.T = ctx->T; p.r = r;
-    const int rows = XTHREADS / ctx->T;
+    p.L = ctx->L; p.N = ctx->N; p.NG = ctx->NG; p.R = ctx->R; p.T = ctx->Tt; p.r = r; p.Tl = ctx->T; p.slot0 = ctx->slot0;
+    const int rows = XTHREADS / ctx->Tt;
     k_overlap_cross<<<dim3(XCHUNKS, ctx->S), XTHREADS, 0, ctx->stream>>>(p);
     SG_LAUNCHED(ctx);
-    const int total = ctx->S * ctx->T * 7;
-    k_reduce_cross<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->Xpart, ctx->result, ctx->S, ctx->T, XCHUNKS * rows, ctx->N);
+    const int total = ctx->S * ctx->Tt * 7;
+    k_reduce_cross<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->Xpart, ctx->result, ctx->S, ctx->Tt, XCHUNKS * rows, ctx->N);
     SG_LAUNCHED(ctx);
-    const size_t nQ = (size_t)ctx->S * ctx->T;
+    const size_t nQ = (size_t)ctx->S * ctx->Tt;
     if (q0) SG_CUDA(ctx, cudaMemcpyAsync(q0, ctx->result, nQ * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     if (qk) SG_CUDA(ctx, cudaMemcpyAsync(qk, ctx->result + nQ, nQ * 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -964,7 +1141,7 @@ int sg_measure_cross(sg_ctx* ctx, int r, const void* dev_remote, double* q0, dou
 
 int sg_export_chirality(sg_ctx* ctx, int r, void* dev_out)
 {
-    if (!ctx || !dev_out || r < 0 || r >= ctx->R) return SG_EINVAL;
+    if (!ctx || !dev_out || r < 0 || r >= ctx->R || ctx->Tt != ctx->T) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     const size_t n = (size_t)ctx->N * ctx->T;
     k_export_zeta_by_temp<<<dim3((unsigned)((n + 255) / 256), ctx->S), 256, 0, ctx->stream>>>(ctx->spins, ctx->slot_of_temp, (float*)dev_out,
@@ -992,7 +1169,7 @@ int sg_chiral_cross(sg_ctx* ctx, const void* dev_a, const void* dev_b, double* q
 
 int sg_schwinger_dyson(sg_ctx* ctx, double* sd)
 {
-    if (!ctx || !sd) return SG_EINVAL;
+    if (!ctx || !sd || ctx->Tt != ctx->T) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     SdParams p;
     p.spins = ctx->spins; p.Jg = ctx->Jg; p.SDpart = ctx->SDpart;
@@ -1031,7 +1208,7 @@ int sg_get_couplings(sg_ctx* ctx, int sample, float* out)
 int sg_get_perm(sg_ctx* ctx, int sample, int32_t* temp_of_slot, int32_t* slot_of_temp)
 {
     if (!ctx || sample < 0 || sample >= ctx->S) return SG_EINVAL;
-    const size_t n = (size_t)ctx->R * ctx->T, off = (size_t)sample * n;
+    const size_t n = (size_t)ctx->R * ctx->Tt, off = (size_t)sample * n;
     if (temp_of_slot) SG_CUDA(ctx, cudaMemcpyAsync(temp_of_slot, ctx->temp_of_slot + off, n * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     if (slot_of_temp) SG_CUDA(ctx, cudaMemcpyAsync(slot_of_temp, ctx->slot_of_temp + off, n * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -1041,7 +1218,7 @@ int sg_get_perm(sg_ctx* ctx, int sample, int32_t* temp_of_slot, int32_t* slot_of
 int sg_set_perm(sg_ctx* ctx, int sample, const int32_t* temp_of_slot)
 {
     if (!ctx || !temp_of_slot || sample < 0 || sample >= ctx->S) return SG_EINVAL;
-    const int R = ctx->R, T = ctx->T;
+    const int R = ctx->R, T = ctx->Tt;
     std::vector<int> tos(temp_of_slot, temp_of_slot + (size_t)R * T), sot((size_t)R * T, -1);
     for (int r = 0; r < R; ++r)
         for (int s = 0; s < T; ++s) {
@@ -1096,8 +1273,8 @@ int sg_set_counters(sg_ctx* ctx, uint64_t hb_counter, uint64_t pt_counter)
 int sg_pt_stats(sg_ctx* ctx, uint64_t* attempts, uint64_t* accepts)
 {
     if (!ctx) return SG_EINVAL;
-    if (ctx->T < 2) return SG_OK;
-    const size_t n = (size_t)ctx->S * ctx->R * (ctx->T - 1) * sizeof(unsigned long long);
+    if (ctx->Tt < 2) return SG_OK;
+    const size_t n = (size_t)ctx->S * ctx->R * (ctx->Tt - 1) * sizeof(unsigned long long);
     if (attempts) SG_CUDA(ctx, cudaMemcpyAsync(attempts, ctx->attempts, n, cudaMemcpyDeviceToHost, ctx->stream));
     if (accepts) SG_CUDA(ctx, cudaMemcpyAsync(accepts, ctx->accepts, n, cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -1108,9 +1285,41 @@ int sg_pt_walk(sg_ctx* ctx, uint64_t* round_trips, int32_t* label)
 {
     if (!ctx) return SG_EINVAL;
     if (round_trips) SG_CUDA(ctx, cudaMemcpyAsync(round_trips, ctx->round_trips, (size_t)ctx->S * ctx->R * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
-    if (label) SG_CUDA(ctx, cudaMemcpyAsync(label, ctx->walk_label, (size_t)ctx->S * ctx->R * ctx->T * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    if (label) SG_CUDA(ctx, cudaMemcpyAsync(label, ctx->walk_label, (size_t)ctx->S * ctx->R * ctx->Tt * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return SG_OK;
+}
+
+int sg_pt_visits(sg_ctx* ctx, uint64_t* visits)
+{
+    if (!ctx || !visits || !ctx->visits) return SG_EINVAL;
+    SG_CUDA(ctx, cudaMemcpyAsync(visits, ctx->visits, (size_t)ctx->S * ctx->R * ctx->Tt * ctx->Tt * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return SG_OK;
+}
+
+// Integrated autocorrelation time of a recorded walk in temperature: tau = 1/2 + sum_{k=1..W} rho(k), with the
+// self-consistent window W >= c tau(W) (Madras-Sokal; Ref. 31 of the paper is a textbook treatment of the same estimator)
+double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c)
+{
+    if (!series || n < 4) return std::nan("");
+    const double c = window_c > 0.0 ? window_c : 6.0;
+    double m = 0.0;
+    for (int64_t i = 0; i < n; ++i) m += (double)series[i];
+    m /= (double)n;
+    double c0 = 0.0;
+    for (int64_t i = 0; i < n; ++i) { const double d = (double)series[i] - m; c0 += d * d; }
+    c0 /= (double)n;
+    if (!(c0 > 0.0)) return std::nan("");
+    double tau = 0.5;
+    for (int64_t k = 1; k <= n / 2; ++k) {
+        double ck = 0.0;
+        for (int64_t i = 0; i + k < n; ++i) ck += ((double)series[i] - m) * ((double)series[i + k] - m);
+        ck /= (double)(n - k);
+        tau += ck / c0;
+        if ((double)k >= c * tau) break;
+    }
+    return tau;
 }
 
 int sg_tune(sg_ctx* ctx, int knob, int value)
@@ -1136,6 +1345,10 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
     case SG_TUNE_MEASURE_IMPL:
         if (value != SG_MEASURE_AUTO && value != SG_MEASURE_STAGED) return SG_EINVAL;
         ctx->measure_impl = value;
+        return SG_OK;
+    case SG_TUNE_GRAPH:
+        if (value != 0 && value != 1) return SG_EINVAL;
+        ctx->graph_mode = value;
         return SG_OK;
     case SG_TUNE_ZCHUNK:
         if (value < 0) return SG_EINVAL;

@@ -49,6 +49,14 @@ __host__ __device__ inline void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+// Global copy id of local copy c of a sample (it enters the Philox counters of the heat bath and of the initial spins):
+// gbase = id of the sample's local copy 0; a context that holds only Tl of the chain's slots per replica (temperature-slot
+// sharding, sg_shape.first_slot / n_temps_total) skips Tpad = n_temps_total - Tl ids between its replicas.
+__device__ __forceinline__ uint32_t copy_gid(uint32_t gbase, int c, int Tl, int Tpad)
+{
+    return gbase + (uint32_t)c + (Tpad ? (uint32_t)((c / Tl) * Tpad) : 0u);
+}
+
 // r = ((w >> 9) + 1/2) 2^-23: exact in fp32
 __device__ __forceinline__ float uniform23(uint32_t w) { return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f); }
 

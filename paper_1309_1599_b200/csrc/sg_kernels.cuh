@@ -27,6 +27,7 @@ struct SweepParams {
     int colour;
     int C;                   // copies per sample (R*T); Cp = NG*G
     int Cg;                  // copies per sample of the whole job (all replicas, sg_shape.n_replicas_total): stride of the global copy id
+    int Tl, Tpad;            // slots per replica held here, n_temps_total - Tl (copy_gid)
     uint32_t key0, key1, hb_counter;
     uint32_t g_first;        // global copy id of (local sample 0, copy 0) = first_sample*C
 };
@@ -110,11 +111,11 @@ __global__ void __launch_bounds__(SWEEP_THREADS) k_sweep(const SweepParams p)
             }
         } else if (KIND == KIND_HB) {
             const float bt[4] = { beta4.x, beta4.y, beta4.z, beta4.w };
-            const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.Cg + (uint32_t)(grp * G + q * 4);
+            const uint32_t gbase = p.g_first + (uint32_t)sample * (uint32_t)p.Cg;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 uint32_t w[4];
-                philox4x32_10((uint32_t)i, g0 + j, p.hb_counter, STREAM_HB, p.key0, p.key1, w);
+                philox4x32_10((uint32_t)i, copy_gid(gbase, grp * G + q * 4 + j, p.Tl, p.Tpad), p.hb_counter, STREAM_HB, p.key0, p.key1, w);
                 hb_update(hf[0][j], hf[1][j], hf[2][j], bt[j], uniform23(w[0]), uniform23(w[1]),
                           s[0][j], s[1][j], s[2][j]);
                 if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
@@ -168,7 +169,7 @@ __global__ void k_reduce_energy(const double* __restrict__ Epart, double* __rest
 // S0: initial spins uniform on S^2, Philox stream 3, counter (i, g, 0, 3)
 // ------------------------------------------------------------------------------------------------
 __global__ void k_init_spins(float* __restrict__ spins_sample /* [NG][2][Nh][3][G] of one sample */, int L, int N, int NG,
-                             int C, uint32_t g_sample, uint32_t key0, uint32_t key1)
+                             int C, uint32_t g_sample, int Tl, int Tpad, uint32_t key0, uint32_t key1)
 {
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;   // over NG*N*8 (site, quad)
     if (t >= (size_t)NG * N * 8) return;
@@ -180,7 +181,7 @@ __global__ void k_init_spins(float* __restrict__ spins_sample /* [NG][2][Nh][3][
     for (int j = 0; j < 4; ++j) {
         const int c = grp * G + q * 4 + j;
         uint32_t w[4];
-        philox4x32_10((uint32_t)i, g_sample + (uint32_t)c, 0u, STREAM_SPINS, key0, key1, w);
+        philox4x32_10((uint32_t)i, copy_gid(g_sample, c, Tl, Tpad), 0u, STREAM_SPINS, key0, key1, w);
         const float zc = 1.0f - 2.0f * uniform23(w[0]);
         const float rho = sqrtf(fmaxf(1.0f - zc * zc, 0.0f));
         float sn, cs;
@@ -260,47 +261,127 @@ __global__ void k_gather_couplings(const float* __restrict__ M, float* __restric
 }
 
 // ------------------------------------------------------------------------------------------------
-// S4: parallel tempering.  One thread per chain (sample, replica); pairs in order.
+// S4: parallel tempering.  The pairs of a chain (sample, replica) are taken in order on the updated
+// assignment, so a chain is sequential; everything around that dependence is not.  k_pt_swap gives a warp to a chain:
+// the lanes stage the chain's assignment, energies, beta differences and uniforms (one Philox block per pair) in shared
+// memory, lane 0 walks the T-1 pairs there (fp64 exp, no global round trips), the lanes write the new assignment, the
+// betas of the slots, the statistics and the random-walk labels back.  k_pt_swap_serial (one thread per chain, straight
+// from global memory) is the same arithmetic for chains too long for shared memory.
+// Temperature-slot sharding (sg_shape.first_slot / n_temps_total): every context of the chain runs the
+// SAME kernel on the all-gathered energies (E + w*E_wstride: the block of the context with slot window w) and keeps the
+// whole assignment; only beta_slot is restricted to the slots [slot0, slot0 + Tl) it holds.
 // ------------------------------------------------------------------------------------------------
 struct PtParams {
     const double* betas;   // [T]
-    const double* E;       // [S][Cp]
+    const double* E;       // local: [S][Cp], copy r*T + slot; gathered: [W][S][R][Tl]
     int* slot_of_temp;     // [S][R][T]
     int* temp_of_slot;     // [S][R][T]
-    float* beta_slot;      // [S][Cp]
+    float* beta_slot;      // [S][Cp], local copy r*Tl + (slot - slot0)
     unsigned long long* attempts;  // [S][R][T-1]
     unsigned long long* accepts;
     int* walk_label;                 // [S][R][T]: 0 = no end touched yet, 1 = last touched index 0, 2 = last touched index T-1
     unsigned long long* round_trips; // [S][R]: completed walks 0 -> T-1 -> 0, summed over the chain's configurations
-    int S, R, T, Cp, Rt;   // Rt: replicas of the whole job (sg_shape.n_replicas_total)
+    unsigned long long* visits;      // [S][R][T][T]: PT sweeps configuration `slot` has spent at temperature index t (after the sweep)
+    int S, R, T, Cp, Rt;   // T: length of the chain (n_temps_total); Rt: replicas of the whole job (sg_shape.n_replicas_total)
+    int Tl, slot0;         // slots per replica held by this context and the first of them (Tl = T, slot0 = 0 unless slot-sharded)
+    long long E_sstride, E_wstride;   // E of (sample, r, slot) = E[(slot / Tl) * E_wstride + sample * E_sstride + r * Tl + slot % Tl]
     uint32_t key0, key1, pt_counter, chain_first;   // chain id of (local sample 0, r = 0) = first_sample*Rt + first_replica
 };
 
-__global__ void k_pt_swap(const PtParams p)
+__device__ __forceinline__ double pt_energy(const PtParams& p, int sample, int r, int slot)
+{
+    return p.E[(long long)(slot / p.Tl) * p.E_wstride + (long long)sample * p.E_sstride + r * p.Tl + slot % p.Tl];
+}
+
+__device__ __forceinline__ double pt_uniform(const PtParams& p, int sample, int r, int t)
+{
+    uint32_t w[4];
+    philox4x32_10((uint32_t)t, p.chain_first + (uint32_t)(sample * p.Rt + r), p.pt_counter, STREAM_PT, p.key0, p.key1, w);
+    return ((double)(w[0] >> 9) + 0.5) * (1.0 / 8388608.0);
+}
+
+constexpr int PT_SMEM_PER_TEMP = 2 * sizeof(double) + 2 * sizeof(int) + 2 * sizeof(double);   // E, sot, tos, rr, dbeta (+ slack)
+
+__global__ void __launch_bounds__(32) k_pt_swap(const PtParams p)
+{
+    extern __shared__ __align__(16) unsigned char pt_sm[];
+    const int chain = blockIdx.x, lane = threadIdx.x, T = p.T;
+    const int sample = chain / p.R, r = chain % p.R;
+    double* const Es = reinterpret_cast<double*>(pt_sm);          // [T] energy of configuration `slot`
+    double* const rr = Es + T;                                    // [T] uniform of pair t
+    double* const db = rr + T;                                    // [T] beta_t - beta_{t+1}
+    int* const sot = reinterpret_cast<int*>(db + T);              // [T]
+    unsigned char* const acc = reinterpret_cast<unsigned char*>(sot + T);   // [T] pair t accepted
+    int* const sot_g = p.slot_of_temp + (size_t)chain * T;
+    int* const tos_g = p.temp_of_slot + (size_t)chain * T;
+    for (int t = lane; t < T; t += 32) {
+        Es[t] = pt_energy(p, sample, r, t);
+        sot[t] = sot_g[t];
+        if (t + 1 < T) { rr[t] = pt_uniform(p, sample, r, t); db[t] = p.betas[t] - p.betas[t + 1]; }
+    }
+    __syncwarp();
+    if (lane == 0) {
+        int i = sot[0];                    // the configuration now at temperature index t
+        double Ei = Es[i];
+        for (int t = 0; t + 1 < T; ++t) {
+            const int j = sot[t + 1];
+            const double Ej = Es[j];
+            const double delta = db[t] * (Ei - Ej);
+            const bool accept = (delta >= 0.0) || (rr[t] < exp(delta));
+            acc[t] = accept ? 1 : 0;
+            if (accept) { sot[t] = j; sot[t + 1] = i; }     // i moves on to index t + 1
+            else { i = j; Ei = Ej; }
+        }
+    }
+    __syncwarp();
+    float* const bs = p.beta_slot + (size_t)sample * p.Cp + r * p.Tl;
+    int* const lab = p.walk_label + (size_t)chain * T;
+    unsigned long long trips = 0ull;
+    for (int t = lane; t < T; t += 32) {
+        const int slot = sot[t];
+        sot_g[t] = slot;
+        tos_g[slot] = t;
+        if (slot >= p.slot0 && slot < p.slot0 + p.Tl) bs[slot - p.slot0] = (float)p.betas[t];
+        if (t + 1 < T) {
+            p.attempts[(size_t)chain * (T - 1) + t] += 1ull;
+            if (acc[t]) p.accepts[(size_t)chain * (T - 1) + t] += 1ull;
+        }
+        // random walk in temperature of every configuration of the chain
+        if (t == 0) {
+            if (lab[slot] == 2) trips += 1ull;
+            lab[slot] = 1;
+        } else if (t == T - 1 && lab[slot] == 1) {
+            lab[slot] = 2;
+        }
+        if (p.visits) p.visits[((size_t)chain * T + slot) * T + t] += 1ull;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) trips += __shfl_xor_sync(0xffffffffu, trips, o);
+    if (lane == 0) p.round_trips[chain] += trips;
+}
+
+__global__ void k_pt_swap_serial(const PtParams p)
 {
     const int chain = blockIdx.x * blockDim.x + threadIdx.x;
     if (chain >= p.S * p.R) return;
     const int sample = chain / p.R, r = chain % p.R;
     int* sot = p.slot_of_temp + (size_t)chain * p.T;
     int* tos = p.temp_of_slot + (size_t)chain * p.T;
-    const double* E = p.E + (size_t)sample * p.Cp + r * p.T;
-    float* bs = p.beta_slot + (size_t)sample * p.Cp + r * p.T;
+    float* bs = p.beta_slot + (size_t)sample * p.Cp + r * p.Tl;
     for (int t = 0; t + 1 < p.T; ++t) {
         const int i = sot[t], j = sot[t + 1];
-        const double delta = (p.betas[t] - p.betas[t + 1]) * (E[i] - E[j]);
-        uint32_t w[4];
-        philox4x32_10((uint32_t)t, p.chain_first + (uint32_t)(sample * p.Rt + r), p.pt_counter, STREAM_PT, p.key0, p.key1, w);
-        const double rr = ((double)(w[0] >> 9) + 0.5) * (1.0 / 8388608.0);
+        const double delta = (p.betas[t] - p.betas[t + 1]) * (pt_energy(p, sample, r, i) - pt_energy(p, sample, r, j));
+        const double rr = pt_uniform(p, sample, r, t);
         const bool accept = (delta >= 0.0) || (rr < exp(delta));
         p.attempts[(size_t)chain * (p.T - 1) + t] += 1ull;
         if (accept) {
             sot[t] = j; sot[t + 1] = i;
             tos[j] = t; tos[i] = t + 1;
-            bs[j] = (float)p.betas[t]; bs[i] = (float)p.betas[t + 1];
+            if (j >= p.slot0 && j < p.slot0 + p.Tl) bs[j - p.slot0] = (float)p.betas[t];
+            if (i >= p.slot0 && i < p.slot0 + p.Tl) bs[i - p.slot0] = (float)p.betas[t + 1];
             p.accepts[(size_t)chain * (p.T - 1) + t] += 1ull;
         }
     }
-    // random walk in temperature of every configuration of the chain
     int* lab = p.walk_label + (size_t)chain * p.T;
     unsigned long long trips = 0ull;
     for (int slot = 0; slot < p.T; ++slot) {
@@ -311,19 +392,32 @@ __global__ void k_pt_swap(const PtParams p)
         } else if (t == p.T - 1 && lab[slot] == 1) {
             lab[slot] = 2;
         }
+        if (p.visits) p.visits[((size_t)chain * p.T + slot) * p.T + t] += 1ull;
     }
     p.round_trips[chain] += trips;
 }
 
-// beta_slot[sample][r*T + slot] = beta[temp_of_slot], for all chains (after init / set_perm)
+// e[sample][r][t] = E(configuration of replica r at temperature index t) / N from the all-gathered energies [W][S][R][Tl]
+__global__ void k_energy_by_temp(const double* __restrict__ Eall, const int* __restrict__ slot_of_temp, double* __restrict__ out,
+                                 int S, int R, int T, int Tl, int N)
+{
+    const int u = blockIdx.x * blockDim.x + threadIdx.x;
+    if (u >= S * R * T) return;
+    const int sample = u / (R * T), r = (u / T) % R;
+    const int slot = slot_of_temp[u];
+    out[u] = Eall[(size_t)(slot / Tl) * S * R * Tl + ((size_t)sample * R + r) * Tl + slot % Tl] / (double)N;
+}
+
+// beta_slot[sample][r*Tl + s] = beta[temp_of_slot[sample][r][slot0 + s]], for all chains (after init / set_perm);
+// T = length of the chain, Tl = slots per replica held by this context
 __global__ void k_fill_beta_slot(const double* __restrict__ betas, const int* __restrict__ temp_of_slot,
-                                 float* __restrict__ beta_slot, int S, int R, int T, int Cp)
+                                 float* __restrict__ beta_slot, int S, int R, int T, int Tl, int slot0, int Cp)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= S * Cp) return;
     const int sample = t / Cp, c = t % Cp;
     float b = 0.f;
-    if (c < R * T) b = (float)betas[temp_of_slot[(size_t)sample * R * T + c]];
+    if (c < R * Tl) b = (float)betas[temp_of_slot[((size_t)sample * R + c / Tl) * T + slot0 + c % Tl]];
     beta_slot[t] = b;
 }
 
@@ -426,17 +520,22 @@ __global__ void k_reduce_measure(const double* __restrict__ Mpart, const double*
 // buffer.  Thread = (site row, temperature): private fp64 sums, partials reduced in a fixed order by k_reduce_cross.
 // ------------------------------------------------------------------------------------------------
 __global__ void k_export_by_temp(const float* __restrict__ spins, const int* __restrict__ slot_of_temp, float* __restrict__ out,
-                                 int L, int N, int NG, int R, int T, int r)
+                                 int L, int N, int NG, int R, int T, int Tl, int slot0, int r)
 {
+    // T: length of the chain; the context holds the slots [slot0, slot0 + Tl) (all of them unless slot-sharded).
+    // A temperature whose configuration lives elsewhere is written as zeros, so that the sum of the shards' buffers
+    // is the whole replica.
     const int sample = blockIdx.y;
     const size_t f = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // (site, temperature), temperature fastest
     if (f >= (size_t)N * T) return;
     const int i = (int)(f / T), t = (int)(f - (size_t)i * T);
-    const int c = r * T + slot_of_temp[((size_t)sample * R + r) * T + t];
+    const int slot = slot_of_temp[((size_t)sample * R + r) * T + t] - slot0;
+    const bool here = slot >= 0 && slot < Tl;
+    const int c = r * Tl + (here ? slot : 0);
     const float* src = spins + (((size_t)sample * NG + c / G) * N + site_slot(i, L, N >> 1)) * SITE_FLOATS + (c % G);
     float* dst = out + (size_t)sample * 3 * N * T + f;
 #pragma unroll
-    for (int a = 0; a < 3; ++a) dst[(size_t)a * N * T] = src[a * G];
+    for (int a = 0; a < 3; ++a) dst[(size_t)a * N * T] = here ? src[a * G] : 0.f;
 }
 
 constexpr int XCHUNKS = 128, XTHREADS = 256;     // k_overlap_cross: site chunks per sample, threads per CTA
@@ -448,6 +547,7 @@ struct CrossParams {
     const double* phase;       // [L][2]
     double* Xpart;             // [S][XCHUNKS * rows][T][7]
     int L, N, NG, R, T, r;
+    int Tl, slot0;             // slots per replica held here and the first of them (T, 0 unless slot-sharded)
 };
 
 __global__ void __launch_bounds__(XTHREADS) k_overlap_cross(const CrossParams p)
@@ -462,10 +562,12 @@ __global__ void __launch_bounds__(XTHREADS) k_overlap_cross(const CrossParams p)
     const float* rem = p.remote + (size_t)sample * 3 * p.N * p.T;
     const size_t plane = (size_t)p.N * p.T;
     for (int t = tx; t < p.T; t += Tw) {
-        const int c = p.r * p.T + p.slot_of_temp[((size_t)sample * p.R + p.r) * p.T + t];
+        const int slot = p.slot_of_temp[((size_t)sample * p.R + p.r) * p.T + t] - p.slot0;
+        const bool here = slot >= 0 && slot < p.Tl;      // else the configuration at t lives in another shard: sums stay 0
+        const int c = p.r * p.Tl + (here ? slot : 0);
         const float* loc = base + (size_t)(c / G) * p.N * SITE_FLOATS + (c % G);
         double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };
-        for (int i = i_begin + row; i < i_end; i += rows) {
+        for (int i = i_begin + row; here && i < i_end; i += rows) {
             const float* s = loc + site_slot(i, p.L, p.N >> 1) * SITE_FLOATS;
             const size_t f = (size_t)i * p.T + t;
             const float qf = fmaf(s[0], rem[f], fmaf(s[G], rem[plane + f], s[2 * G] * rem[2 * plane + f]));

@@ -25,6 +25,7 @@ struct ResParams {
     const float* beta_slot;  // [S][Cp]
     double* E;               // [S][Cp]: total H of every slot, written by the last half-sweep
     int L, N, Nh, NG, C, Cp, Cg;   // Cg: copies per sample of the whole job (stride of the global copy id)
+    int Tl, Tpad;                  // slots per replica held here, n_temps_total - Tl (copy_gid)
     int n_sweeps;
     uint32_t key0, key1, hb_counter, g_first;
 };
@@ -54,7 +55,9 @@ __global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
     float* const sp = lat + q * 4;
     float4 beta4 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (KIND_ == 1) beta4 = ldg4(p.beta_slot + (size_t)sample * p.Cp + c_first + q * 4);
-    const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.Cg + (uint32_t)(c_first + q * 4);
+    uint32_t gid[4];                                  // global ids of this thread's four copies
+#pragma unroll
+    for (int j = 0; j < 4; ++j) gid[j] = copy_gid(p.g_first + (uint32_t)sample * (uint32_t)p.Cg, c_first + q * 4 + j, p.Tl, p.Tpad);
     float eacc[4] = { 0.f, 0.f, 0.f, 0.f };
 
     for (int sw = 0; sw < p.n_sweeps; ++sw) {
@@ -114,7 +117,7 @@ __global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         uint32_t w[4];
-                        philox4x32_10((uint32_t)i, g0 + j, p.hb_counter + (uint32_t)sw, STREAM_HB, p.key0, p.key1, w);
+                        philox4x32_10((uint32_t)i, gid[j], p.hb_counter + (uint32_t)sw, STREAM_HB, p.key0, p.key1, w);
                         hb_update(hf[0][j], hf[1][j], hf[2][j], bt[j], uniform23(w[0]), uniform23(w[1]), s[0][j], s[1][j], s[2][j]);
                         if (last) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
                     }

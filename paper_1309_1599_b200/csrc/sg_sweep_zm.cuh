@@ -101,6 +101,7 @@ struct ZmParams {
     const float* beta_slot;  // [S][Cp]
     double* Epart;           // [S][NG][nblk][G]
     int L, N, Nh, NG, C, Cg; // Cg: copies per sample of the whole job (stride of the global copy id)
+    int Tl, Tpad;            // slots per replica held here, n_temps_total - Tl (copy_gid)
     int ntx, nty, nzc, ZC;   // tiles along x1, x2; chunks along x3 of ZC planes each
     int colour;
     uint32_t key0, key1, hb_counter, g_first;
@@ -109,7 +110,7 @@ struct ZmParams {
 // the single-site update of 4 copies held by one thread (shared by the update kinds)
 template <int KIND, bool WITH_E>
 __device__ __forceinline__ void zm_update(const float (&hf)[3][4], float (&s)[3][4], float (&eacc)[4], const float4& beta4,
-                                          uint32_t i, uint32_t g0, const ZmParams& p)
+                                          uint32_t i, const uint32_t (&gid)[4], const ZmParams& p)
 {
     if (KIND == KIND_OR) {
 #pragma unroll
@@ -123,7 +124,7 @@ __device__ __forceinline__ void zm_update(const float (&hf)[3][4], float (&s)[3]
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             uint32_t w[4];
-            philox4x32_10(i, g0 + j, p.hb_counter, STREAM_HB, p.key0, p.key1, w);
+            philox4x32_10(i, gid[j], p.hb_counter, STREAM_HB, p.key0, p.key1, w);
             hb_update(hf[0][j], hf[1][j], hf[2][j], bt[j], uniform23(w[0]), uniform23(w[1]), s[0][j], s[1][j], s[2][j]);
             if (WITH_E) eacc[j] += fmaf(hf[0][j], s[0][j], fmaf(hf[1][j], s[1][j], hf[2][j] * s[2][j]));
         }
@@ -286,7 +287,11 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
     const int Y = Y0 + ky;
     float4 beta4 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (KIND == KIND_HB) beta4 = ldg4(p.beta_slot + (size_t)sample * p.NG * G + grp * G + q * 4);
-    const uint32_t g0 = p.g_first + (uint32_t)sample * (uint32_t)p.Cg + (uint32_t)(grp * G + q * 4);
+    uint32_t gid[4] = { 0u, 0u, 0u, 0u };             // global ids of this thread's four copies (heat bath only)
+    if (KIND == KIND_HB) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) gid[j] = copy_gid(p.g_first + (uint32_t)sample * (uint32_t)p.Cg, grp * G + q * 4 + j, p.Tl, p.Tpad);
+    }
     float eacc[4] = { 0.f, 0.f, 0.f, 0.f };
 
     // Own spin of step k: site (X0 + 2 kx + off, Y, z0 + k), off = (ky + z + colour) & 1.  In the colour-split
@@ -371,7 +376,7 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
             // the own spin is needed only now (s.h and the reflection): take it from the prefetch registers ...
 #pragma unroll
             for (int a = 0; a < 3; ++a) { s[a][0] = pre[d][a].x; s[a][1] = pre[d][a].y; s[a][2] = pre[d][a].z; s[a][3] = pre[d][a].w; }
-            zm_update<KIND, WITH_E>(hf, s, eacc, beta4, i, g0, p);
+            zm_update<KIND, WITH_E>(hf, s, eacc, beta4, i, gid, p);
             if (KIND != KIND_ENERGY) {
 #pragma unroll
                 for (int a = 0; a < 3; ++a) st4(own + a * G, make_float4(s[a][0], s[a][1], s[a][2], s[a][3]));

@@ -1,7 +1,8 @@
-"""Multi-process plumbing of the weak-scaling run: one process per GPU, disorder
-samples sharded across ranks, no data-path collective (samples are independent).
-torch.distributed carries only the barrier and the max / sum of a few host scalars; the functions
-work with any backend (nccl on the GPU box, gloo in the CPU tests)."""
+"""Multi-process plumbing: one process per GPU.  Disorder samples sharded across ranks need no
+data-path collective (samples are independent); one sample can be sharded by replica (whole PT chains per
+rank, no exchange inside the Monte Carlo) or by temperature slot (the paper's mode: one all-gather of
+the energies per PT step).  Orchestration only: every number is computed by the library's kernels; the functions work with
+any torch.distributed backend (nccl on the GPU box, gloo in the CPU tests)."""
 import os
 
 
@@ -111,6 +112,85 @@ def measure_all_pairs(gpu, rank, world_size, n_local, chirality=False):
 
         out = out + _pairs_from_blocks(tuple(gpu.measure_chiral()), rank, world_size, n_local, gpu.export_chirality, cross, alloc, stream)
     return out
+
+
+def slot_window_of_rank(rank, world_size, n_temps_total):
+    """(first_slot, n_temps) of rank `rank` when the configurations (slots) of every PT chain are sharded over the ranks
+    (sg_shape.first_slot / n_temps_total; the paper's multi-GPU mode, where N_GPU = N_T and a GPU holds
+    the two replicas of one slot).  Contiguous, disjoint windows of equal length; world_size must divide n_temps_total."""
+    if world_size <= 0 or not 0 <= rank < world_size:
+        raise ValueError("0 <= rank < world_size required")
+    if n_temps_total % world_size != 0:
+        raise ValueError("world_size must divide n_temps_total")
+    n = n_temps_total // world_size
+    return rank * n, n
+
+
+def _on_stream(gpu):
+    import contextlib
+    import torch
+    stream = getattr(gpu, "stream", None)
+    return torch.cuda.stream(stream) if isinstance(stream, torch.cuda.Stream) else contextlib.nullcontext()
+
+
+def pt_step_sharded(gpu, world_size, gathered=None):
+    """The PT sweep of slot-sharded chains: every rank publishes the energies of its slots (S*R*n_temps doubles, a device
+    buffer), ONE all-gather carries them to all ranks (the paper's "exchange with the master of a double precision
+    number"; 8*C bytes per sample in all), and every rank runs the same swap kernel on the gathered vector:
+    identical Philox counters, identical decisions, so the temperature assignment stays replicated with no second
+    exchange.  `gathered`: reusable device tensor [world_size][S][R][n_temps] float64.  Returns it."""
+    import torch
+    import torch.distributed as dist
+    with _on_stream(gpu):
+        mine = gpu.pt_publish()
+        if gathered is None:
+            gathered = torch.empty((world_size,) + tuple(mine.shape), dtype=mine.dtype, device=mine.device)
+        if world_size > 1:
+            dist.all_gather(list(gathered.unbind(0)), mine)
+        else:
+            gathered[0].copy_(mine)
+        gpu.pt_swap_gathered(gathered)
+    return gathered
+
+
+def unit_sharded(gpu, n_or, world_size, gathered=None):
+    """One MCS of slot-sharded chains: the sweeps touch only the rank's own lattices, the PT step is pt_step_sharded."""
+    gpu.sweep_hb(1)
+    gpu.sweep_or(n_or)
+    return pt_step_sharded(gpu, world_size, gathered)
+
+
+def overlaps_sharded(gpu, world_size, pairs=None):
+    """Overlaps of slot-sharded chains.  The two configurations at temperature t of a replica pair (a, b) may live on
+    different ranks.  Per replica b: every rank exports the temperatures whose configuration it holds (zeros elsewhere,
+    sg_export_replica), an all-reduce (sum) assembles the replica ordered by temperature on every rank, every rank forms the
+    overlap with its part of replica a (sg_measure_cross: zero where it does not hold the configuration), and a last
+    all-reduce (sum) of the few numbers completes every temperature.  Returns (q0 [S][P][T], qk [S][P][T][3][2]) on every
+    rank, pairs a < b in the order of sg_measure (or the given list).  At measurement time only."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    R = gpu.R
+    if pairs is None:
+        pairs = [(a, b) for a in range(R) for b in range(a + 1, R)]
+    q0s, qks = {}, {}
+    with _on_stream(gpu):
+        for b in sorted({b for _, b in pairs}):
+            full = gpu.export_replica(b)
+            if world_size > 1:
+                dist.all_reduce(full, op=dist.ReduceOp.SUM)
+            for a in [a for a, bb in pairs if bb == b]:
+                q0s[(a, b)], qks[(a, b)] = gpu.measure_cross(a, full)
+    q0 = np.stack([q0s[pr] for pr in pairs], axis=1)
+    qk = np.stack([qks[pr] for pr in pairs], axis=1)
+    if world_size > 1:
+        t0, tk = torch.from_numpy(q0), torch.from_numpy(qk)
+        dev = getattr(gpu, "device", "cpu") if dist.get_backend() == "nccl" else "cpu"
+        t0, tk = t0.to(dev), tk.to(dev)
+        dist.all_reduce(t0, op=dist.ReduceOp.SUM)
+        dist.all_reduce(tk, op=dist.ReduceOp.SUM)
+        q0, qk = t0.cpu().numpy(), tk.cpu().numpy()
+    return q0, qk
 
 
 def init_process_group(backend, world_size):

@@ -474,21 +474,35 @@ def test_resident_kernel_is_bit_identical_to_the_per_half_sweep_kernels(sg, L, S
             assert np.array_equal(spins, ref), (impl, cpc)
 
 
-def test_run_units_equals_the_three_calls(sg):
-    """sg_run_units(n, n_or) = n x (sg_sweep_hb(1); sg_sweep_or(n_or); sg_pt_swap()), bit for bit."""
-    L, S, R, T = 6, 2, 2, 6
+@pytest.mark.parametrize("L,S,R,T,n_units,own_stream", [(6, 2, 2, 6, 7, False), (6, 2, 2, 6, 25, False), (8, 3, 4, 16, 30, True), (4, 1, 2, 4, 40, True),
+                                                    (16, 1, 2, 8, 12, True)])
+def test_run_units_equals_the_three_calls(sg, L, S, R, T, n_units, own_stream):
+    """sg_run_units(n, n_or) = n x (sg_sweep_hb(1); sg_sweep_or(n_or); sg_pt_swap()), bit for bit -- issued one by one
+    (n < 8, L = 16, SG_TUNE_GRAPH = 0) or as replays of one captured unit with patched sweep counters (CUDA graph; on the
+    caller's stream, or on the library's own when the caller's is the legacy default stream)."""
+    import torch
     betas = np.linspace(0.5, 1.8, T)
-    a = sg.SpinGlass(L, S, R, T, betas, seed=4); b = sg.SpinGlass(L, S, R, T, betas, seed=4)
-    for g in (a, b):
+    stream = torch.cuda.Stream() if own_stream else None
+    a = sg.SpinGlass(L, S, R, T, betas, seed=4, stream=stream); b = sg.SpinGlass(L, S, R, T, betas, seed=4, stream=stream)
+    c = sg.SpinGlass(L, S, R, T, betas, seed=4, stream=stream)
+    c.tune(sg.TUNE_GRAPH, 0)
+    for g in (a, b, c):
         for s in range(S):
             g.init_sample(s)
-    for _ in range(7):
+    for _ in range(n_units):
         a.unit(3)
-    b.run_units(7, 3)
-    for s in range(S):
-        assert np.array_equal(a.get_spins(s), b.get_spins(s))
-        assert np.array_equal(a.get_perm(s)[0], b.get_perm(s)[0])
-    assert np.array_equal(a.get_energies(), b.get_energies()) and a.get_counters() == b.get_counters() == (7, 7)
+    b.run_units(n_units, 3)
+    c.run_units(n_units, 3)
+    b.run_units(9, 0); c.run_units(9, 0)          # a second capture on the same context, n_or = 0
+    for _ in range(9):
+        a.unit(0)
+    assert b.kernel_launches() == c.kernel_launches()      # replays count the launches of the captured unit
+    for g in (b, c):
+        for s in range(S):
+            assert np.array_equal(a.get_spins(s), g.get_spins(s))
+            assert np.array_equal(a.get_perm(s)[0], g.get_perm(s)[0])
+        assert np.array_equal(a.get_energies(), g.get_energies()) and a.get_counters() == g.get_counters() == (n_units + 9, n_units + 9)
+        assert np.array_equal(a.pt_stats()[1], g.pt_stats()[1]) and np.array_equal(a.pt_visits(), g.pt_visits())
 
 
 @pytest.mark.parametrize("L,S,T,impl", [(8, 2, 5, 2), (6, 1, 7, 1), (4, 2, 4, 0), (16, 1, 20, 0)])
@@ -550,3 +564,102 @@ def test_checkpoint_resume_is_bit_exact(sg, L, S, R, T, impl):
         assert np.array_equal(a.get_spins(s), b.get_spins(s))
         assert np.array_equal(a.get_perm(s)[0], b.get_perm(s)[0]) and np.array_equal(a.get_perm(s)[1], b.get_perm(s)[1])
     assert np.array_equal(a.get_energies(), b.get_energies())
+
+
+@pytest.mark.parametrize("L,S,R,T,W,impl", [(8, 2, 2, 8, 2, 2), (6, 1, 3, 6, 3, 1), (4, 2, 2, 4, 4, 0), (8, 1, 4, 12, 2, 0)])
+def test_temperature_slot_shards_reproduce_the_single_context(sg, L, S, R, T, W, impl):
+    """sg_shape.first_slot / n_temps_total (the paper's multi-GPU mode): W contexts on one GPU, each
+    holding T/W consecutive slots of every chain, against one context holding whole chains, over 50 units: initial spins,
+    spins, the whole temperature assignment, energies, PT statistics, round trips and the visit histogram identical bit for
+    bit (heat bath keyed by global copy id; the PT kernel runs on the all-gathered energies with the same counters on every
+    shard), and the overlaps assembled across the shards equal the single context's sg_measure."""
+    import torch
+    from paper_1309_1599_b200 import multi
+    betas = np.linspace(0.5, 1.6, T)
+    Tl, n_or, units = T // W, 2, 50
+    whole = sg.SpinGlass(L, S, R, T, betas, seed=91, first_sample=2)
+    shards = [sg.SpinGlass(L, S, R, Tl, betas, seed=91, first_sample=2, first_slot=w * Tl, n_temps_total=T) for w in range(W)]
+    for g in [whole] + shards:
+        g.tune(sg.TUNE_SWEEP_IMPL, impl)
+        for s in range(S):
+            g.init_sample(s, sg.GEN_OFFDIAG_SYM, 1.0)
+    def shard_spins(s):
+        parts = [g.get_spins(s).reshape(R, Tl, 3, -1) for g in shards]
+        return np.concatenate(parts, axis=1).reshape(R * T, 3, -1)
+    for s in range(S):
+        assert np.array_equal(whole.get_spins(s), shard_spins(s)), "initial spins"
+    gathered = torch.empty((W, S, R, Tl), dtype=torch.float64, device="cuda")
+    for u in range(units):
+        whole.unit(n_or)
+        for w, g in enumerate(shards):
+            g.sweep_hb(1); g.sweep_or(n_or)
+            g.pt_publish(out=gathered[w])
+        torch.cuda.synchronize()
+        for g in shards:
+            g.pt_swap_gathered(gathered)
+    E = whole.get_energies().reshape(S, R, T)
+    for s in range(S):
+        assert np.array_equal(whole.get_spins(s), shard_spins(s)), "spins"
+        for g in shards:
+            assert np.array_equal(whole.get_perm(s)[0], g.get_perm(s)[0]) and np.array_equal(whole.get_perm(s)[1], g.get_perm(s)[1])
+    for w, g in enumerate(shards):
+        assert np.array_equal(E[:, :, w * Tl:(w + 1) * Tl], g.get_energies().reshape(S, R, Tl))
+        assert np.array_equal(whole.pt_stats()[0], g.pt_stats()[0]) and np.array_equal(whole.pt_stats()[1], g.pt_stats()[1])
+        assert np.array_equal(whole.pt_walk()[0], g.pt_walk()[0]) and np.array_equal(whole.pt_walk()[1], g.pt_walk()[1])
+        assert np.array_equal(whole.pt_visits(), g.pt_visits())
+        with pytest.raises(sg.SgError):
+            g.pt_swap()
+        with pytest.raises(sg.SgError):
+            g.measure()
+    assert whole.pt_stats()[1].sum() > 0 and whole.pt_visits().sum() == S * R * T * units
+    # measurement across the shards: e by temperature from the gathered energies, overlaps by export / sum / cross / sum
+    whole.tune(sg.TUNE_MEASURE_IMPL, sg.MEASURE_STAGED)      # fp64 sums per site, as sg_measure_cross forms them
+    e, q0, qk = whole.measure()
+    for w, g in enumerate(shards):
+        g.pt_publish(out=gathered[w])
+    torch.cuda.synchronize()
+    assert np.array_equal(shards[0].energy_by_temp(gathered), e)
+    pairs = [(a, b) for a in range(R) for b in range(a + 1, R)]
+    for p, (a, b) in enumerate(pairs):
+        full = sum(g.export_replica(b) for g in shards)
+        parts = [g.measure_cross(a, full) for g in shards]
+        q0_x = sum(pp[0] for pp in parts); qk_x = sum(pp[1] for pp in parts)
+        assert np.abs(q0_x - q0[:, p]).max() <= 1e-12 and np.abs(qk_x - qk[:, p]).max() <= 1e-12
+        # every temperature is held by exactly one shard: the other shards contribute exact zeros
+        assert all(((pp[0] == 0) | (pp[0] == q0_x)).all() for pp in parts)
+    # one shard alone through the orchestration (world size 1 path of multi.pt_step_sharded on a whole-chain context)
+    solo = sg.SpinGlass(L, S, R, T, betas, seed=91, first_sample=2)
+    solo.tune(sg.TUNE_SWEEP_IMPL, impl)
+    ref = sg.SpinGlass(L, S, R, T, betas, seed=91, first_sample=2)
+    ref.tune(sg.TUNE_SWEEP_IMPL, impl)
+    for g in (solo, ref):
+        for s in range(S):
+            g.init_sample(s, sg.GEN_OFFDIAG_SYM, 1.0)
+    for _ in range(3):
+        multi.unit_sharded(solo, n_or, 1)
+        ref.unit(n_or)
+    for s in range(S):
+        assert np.array_equal(solo.get_spins(s), ref.get_spins(s)) and np.array_equal(solo.get_perm(s)[0], ref.get_perm(s)[0])
+    for g in [whole, solo, ref] + shards:
+        g.close()
+
+
+def test_pt_visit_histogram_and_tau_int_match_oracle(sg, oracle):
+    """sg_pt_visits is the oracle's visit histogram bit for bit (fed the oracle's energies), and sg_walk_tau_int of a
+    recorded walk in temperature equals the oracle's estimator."""
+    L, S, R, T = 4, 2, 2, 6
+    betas = np.linspace(0.4, 1.2, T)
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas, seed=12)
+    series = []
+    for _ in range(300):
+        sim.sweep_hb(1)
+        E = sim.energies()
+        gpu.set_energies(E)
+        sim.pt_swap(energies=E)
+        gpu.pt_swap()
+        series.append(gpu.get_perm(0)[0][0, 0])
+    assert np.array_equal(gpu.pt_visits(), sim.visits) and sim.visits.sum() == S * R * T * 300
+    assert np.array_equal(gpu.pt_walk()[0], sim.round_trips[..., 0])
+    for c in (6.0, 3.0):
+        assert sg.walk_tau_int(series, c) == pytest.approx(oracle.walk_tau_int(series, c), rel=1e-12)
+    assert len(set(series)) > 2

@@ -109,3 +109,79 @@ def test_single_process_passthrough():
     for bad in ((0, 4, 4), (0, 3, 4), (2, 2, 4)):               # one replica per rank, not a divisor, rank out of range
         with pytest.raises(ValueError):
             multi.replica_window_of_rank(*bad)
+
+
+class _FakeSlotShard:
+    """Stands in for a slot-sharded SpinGlass (no GPU): it 'holds' n_temps slots of every chain, its energies are
+    100 * rank + slot, its exported replica carries the rank in the columns it owns, a cross overlap counts what it saw."""
+    S, R, N = 2, 2, 4
+
+    def __init__(self, rank, world, n_temps_total):
+        self.rank, self.W, self.Tt = rank, world, n_temps_total
+        self.first_slot, self.T = multi.slot_window_of_rank(rank, world, n_temps_total)
+        self.swapped_with = None
+        self.calls = []
+
+    def sweep_hb(self, n):
+        self.calls.append("hb")
+
+    def sweep_or(self, n):
+        self.calls.append("or%d" % n)
+
+    def pt_publish(self):
+        import torch
+        self.calls.append("publish")
+        return torch.full((self.S, self.R, self.T), 100.0 * self.rank, dtype=torch.float64) + torch.arange(self.T, dtype=torch.float64)
+
+    def pt_swap_gathered(self, gathered):
+        self.calls.append("swap")
+        self.swapped_with = gathered.clone()
+
+    def export_replica(self, b):
+        import torch
+        out = torch.zeros((self.S, 3, self.N, self.Tt))
+        out[..., self.first_slot:self.first_slot + self.T] = 1.0 + b          # the temperatures this shard holds (identity assignment)
+        return out
+
+    def measure_cross(self, a, full):
+        q0 = np.zeros((self.S, self.Tt)); qk = np.zeros((self.S, self.Tt, 3, 2))
+        own = slice(self.first_slot, self.first_slot + self.T)
+        q0[:, own] = 10.0 * a + full[0, 0, 0, own].numpy()                    # 10 a + (1 + b) where the whole replica b arrived
+        qk[:, own] = q0[:, own, None, None]
+        return q0, qk
+
+
+def _slot_worker(rank, world, port, out):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    assert multi.init_process_group("gloo", world)
+    shard = _FakeSlotShard(rank, world, 6)
+    gathered = multi.unit_sharded(shard, 3, world)
+    q0, qk = multi.overlaps_sharded(shard, world)
+    out.put((rank, shard.calls, gathered.tolist(), shard.swapped_with.tolist(), q0.tolist(), qk.shape))
+    multi.barrier()
+    import torch.distributed as dist
+    dist.destroy_process_group()
+
+
+def test_two_rank_gloo_temperature_slot_sharding():
+    """The PT step of slot-sharded chains: sweeps, publish, ONE all-gather, the same swap call on every
+    rank with the same gathered energies in rank order; overlaps: export, sum, cross, sum -- every temperature complete on
+    every rank."""
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_slot_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted(out.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    expect = [[[[100.0 * w + t for t in range(3)]] * 2] * 2 for w in range(2)]        # [W][S][R][Tl]
+    for g in got:
+        assert g[1] == ["hb", "or3", "publish", "swap"]
+        assert g[2] == expect and g[3] == expect                 # identical gathered energies on both ranks
+        assert g[4] == [[[0.0 + 2.0] * 6]] * 2 and g[5] == (2, 1, 6, 3, 2)   # pair (0, 1): 10*0 + (1 + 1) at all six temperatures
+    assert multi.slot_window_of_rank(1, 3, 12) == (4, 4)
+    with pytest.raises(ValueError):
+        multi.slot_window_of_rank(0, 4, 6)
