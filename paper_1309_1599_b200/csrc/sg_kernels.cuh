@@ -405,7 +405,7 @@ __global__ void k_energy_by_temp(const double* __restrict__ Eall, const int* __r
     if (u >= S * R * T) return;
     const int sample = u / (R * T), r = (u / T) % R;
     const int slot = slot_of_temp[u];
-    out[u] = Eall[(size_t)(slot / Tl) * S * R * Tl + ((size_t)sample * R + r) * Tl + slot % Tl] / (double)N;
+    out[u] = Eall[(size_t)(slot / Tl) * S * R * Tl + ((size_t)sample * R + r) * Tl + slot % Tl] * (1.0 / (double)N);   // as k_reduce_measure
 }
 
 // beta_slot[sample][r*Tl + s] = beta[temp_of_slot[sample][r][slot0 + s]], for all chains (after init / set_perm);
