@@ -267,6 +267,10 @@ double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c);
  *   SG_SWEEP_RESIDENT all n sweeps of an sg_sweep_or / sg_sweep_hb call in ONE launch, the lattice of a (sample, group of
  *                     32 copies) held in shared memory; SG_EINVAL unless the lattice of 4 copies fits (N * 48 B <= 200 KB).
  *                     sg_halfsweep and the stand-alone energy pass keep using the z-marching / tiled kernel.
+ *   SG_SWEEP_FUSED    sg_sweep_or only: both colours of a sweep in ONE pass of the colour-fused z-marching kernel (SURVEY.md
+ *                     section 8(f1): every spin read once and written once per sweep; the new colour-0 values of the one-site
+ *                     ring around a CTA's column are recomputed, the sweep runs out of place between two state buffers);
+ *                     heat bath, sg_halfsweep and the energy pass as SG_SWEEP_ZMARCH.  SG_EINVAL unless L is a multiple of 8.
  * All kernels perform the same arithmetic in the same order: the spins do not depend on the choice.
  * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else even, >= 4 and a divisor of L.
  * SG_TUNE_RES_COPIES: copies per CTA of the resident kernel: 0 = automatic, else 4, 8, 16 or 32 (SG_EINVAL if the lattice
@@ -284,7 +288,7 @@ double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c);
  *   one by one.  Same launches, same results. */
 enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2, SG_TUNE_PACKED = 3, SG_TUNE_MEASURE_IMPL = 4, SG_TUNE_GRAPH = 5 };
 enum { SG_MEASURE_AUTO = 0, SG_MEASURE_STAGED = 1 };
-enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2, SG_SWEEP_RESIDENT = 3 };
+enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2, SG_SWEEP_RESIDENT = 3, SG_SWEEP_FUSED = 4 };
 int sg_tune(sg_ctx* ctx, int knob, int value);
 
 /* ---- utilities ---- */

@@ -12,6 +12,7 @@
 #include "sg_kernels.cuh"
 #include "sg_measure.cuh"
 #include "sg_sweep_res.cuh"
+#include "sg_sweep_fz.cuh"
 
 using namespace sg;
 
@@ -24,7 +25,7 @@ struct sg_ctx {
     uint32_t g_first;     // global copy id of (local sample 0, local copy 0)
     cudaStream_t stream;
     // device arrays (carved from the caller's workspace)
-    float* spins; float* Jg; float* Jt; unsigned char* Jp; float* Mraw; float* staging; float* beta_slot;
+    float* spins; float* spins2; float* Jr; float* Jg; float* Jt; unsigned char* Jp; float* Mraw; float* staging; float* beta_slot;
     double* betas; double* E; double* Epart; double* SDpart; double* phase; double* Mpart; double* result;
     double* h_result = nullptr;   // pinned host mirror of `result`: one device-to-host copy per measurement call
     size_t result_doubles = 0;
@@ -42,7 +43,9 @@ struct sg_ctx {
     int res_cpc, res_cpc_req;   // copies per CTA of the resident kernel (4, 8, 16, 32); requested, 0 = automatic
     int zm_zc_req;    // requested planes per chunk, 0 = automatic
     int zm_ok, zm_ZC, zm_nzc;
-    uint32_t zm_attr_set = 0;   // template instances of k_sweep_zm whose shared-memory attribute this context has set on its device
+    uint32_t zm_attr_set = 0;
+    uint32_t fz_attr_set = 0;   // the same for k_sweep_fz
+    int fz_ZC, fz_nzc;          // chunking of the colour-fused sweep   // template instances of k_sweep_zm whose shared-memory attribute this context has set on its device
     // measure geometry
     int nchunk, chunk_sites, MS;
     int mq_nchunk, mq_rows_per_cta, mq_Tw, mq_rows_t;   // k_measure_rows: row chunks per sample, rows per CTA, temperatures and rows per CTA pass
@@ -138,13 +141,16 @@ struct Carve {
 };
 
 struct Offsets {
-    size_t spins, Jg, Jt, Jp, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, visits, logbin, xpart, total;
+    size_t spins, spins2, Jr, Jg, Jt, Jp, Mraw, staging, beta_slot, betas, E, Epart, SDpart, phase, Mpart, result, sot, tos, att, acc, wlab, trips, visits, logbin, xpart, total;
 };
 
 Offsets offsets(const Geometry& g)
 {
     Carve c; Offsets o;
     o.spins = c.take((size_t)g.S * g.NG * g.N * SITE_FLOATS * sizeof(float));
+    // the colour-fused sweep (L a multiple of 8) is out of place: a second state buffer, and the couplings of the ring sites
+    o.spins2 = c.take((g.L % 8 == 0) ? (size_t)g.S * g.NG * g.N * SITE_FLOATS * sizeof(float) : 0);
+    o.Jr = c.take((g.L % 8 == 0) ? (size_t)g.S * (g.N / 4) * JG * sizeof(float) : 0);
     o.Jg = c.take((size_t)g.S * 2 * g.Nh * JG * sizeof(float));
     o.Jt = c.take((g.L % 8 == 0) ? (size_t)g.S * 2 * g.Nh * JG * sizeof(float) : 0);
     o.Jp = c.take((g.L % 8 == 0) ? (size_t)g.S * g.N * 8 : 0);
@@ -386,6 +392,60 @@ int half_sweep_zm(sg_ctx* ctx, int kind, int colour, bool with_energy)
     return SG_OK;
 }
 
+// ---- colour-fused overrelaxation sweep (sg_sweep_fz.cuh): one pass per sweep, out of place ----
+constexpr int FZ_NSO = 4, FZ_NSN = 3, FZ_NJ = 2;
+
+void fz_plan(sg_ctx* ctx)
+{
+    const int L = ctx->L;
+    ctx->fz_ZC = 0; ctx->fz_nzc = 0;
+    if (L % 8 != 0) return;
+    int ZC = 0;
+    if (ctx->zm_zc_req > 0) {
+        ZC = ctx->zm_zc_req;
+    } else {
+        // the longest chunk (a chunk recomputes 2 colour-0 planes per ZC) that still gives every SM a few CTAs in turn (1 per SM resident)
+        const long per_chunk = (long)ctx->S * ctx->NG * (L / 8) * (L / 8);
+        for (int cand = L; cand >= 4; --cand) {
+            if ((cand & 1) || L % cand != 0) continue;
+            ZC = cand;
+            if (per_chunk * (L / cand) >= 4 * 148) break;
+        }
+    }
+    if (ZC < 2 || (ZC & 1) || L % ZC != 0) return;
+    ctx->fz_ZC = ZC; ctx->fz_nzc = L / ZC;
+}
+
+int sweep_fused(sg_ctx* ctx, bool with_energy)
+{
+    FzParams p;
+    p.src = ctx->spins; p.dst = ctx->spins2; p.Jt = ctx->Jt; p.Jr = ctx->Jr; p.Epart = ctx->Epart;
+    p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG;
+    p.ntx = ctx->L / 8; p.nty = ctx->L / 8; p.nzc = ctx->fz_nzc; p.ZC = ctx->fz_ZC;
+    const int nblk = p.ntx * p.nty * p.nzc;
+    const dim3 grid(nblk * ctx->NG, ctx->S);
+    constexpr size_t smem = fz_smem_bytes<FZ_NSO, FZ_NSN, FZ_NJ>();
+    auto k0 = k_sweep_fz<false, FZ_NSO, FZ_NSN, FZ_NJ>;
+    auto k1 = k_sweep_fz<true, FZ_NSO, FZ_NSN, FZ_NJ>;
+    const uint32_t bit = with_energy ? 2u : 1u;
+    if (!(ctx->fz_attr_set & bit)) {
+        SG_CUDA(ctx, cudaFuncSetAttribute(with_energy ? k1 : k0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ctx->fz_attr_set |= bit;
+    }
+    if (with_energy) k1<<<grid, FzGeom::THREADS, smem, ctx->stream>>>(p);
+    else k0<<<grid, FzGeom::THREADS, smem, ctx->stream>>>(p);
+    SG_LAUNCHED(ctx);
+    float* t = ctx->spins; ctx->spins = ctx->spins2; ctx->spins2 = t;      // the new state
+    if (with_energy) {
+        k_reduce_energy<<<ctx->S * ctx->NG, 256, 0, ctx->stream>>>(ctx->Epart, ctx->E, nblk);
+        SG_LAUNCHED(ctx);
+        ctx->energies_fresh = true;
+    } else {
+        ctx->energies_fresh = false;
+    }
+    return SG_OK;
+}
+
 // one half-sweep of every copy; with_energy also reduces E (valid because a whole colour is swept)
 int half_sweep(sg_ctx* ctx, int kind, int colour, bool with_energy)
 {
@@ -527,6 +587,11 @@ int sweeps(sg_ctx* ctx, int kind, int n_sweeps)
     if (!ctx || n_sweeps < 0) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     if (n_sweeps > 0 && use_resident(ctx)) return sweeps_resident(ctx, kind, n_sweeps);
+    if (kind == KIND_OR && ctx->sweep_impl == SG_SWEEP_FUSED && ctx->fz_ZC > 0 && !use_packed(ctx)) {
+        for (int k = 0; k < n_sweeps; ++k)
+            if (int rc = sweep_fused(ctx, k == n_sweeps - 1)) return rc;
+        return SG_OK;
+    }
     for (int k = 0; k < n_sweeps; ++k) {
         if (int rc = half_sweep(ctx, kind, 0, false)) return rc;
         if (int rc = half_sweep(ctx, kind, 1, k == n_sweeps - 1)) return rc;
@@ -597,6 +662,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->mq_nchunk = g.mq_nchunk; ctx->mq_rows_per_cta = g.mq_rows_per_cta; ctx->mq_Tw = g.mq_Tw; ctx->mq_rows_t = g.mq_rows_t;
     ctx->stream = (cudaStream_t)cuda_stream;
     char* base = (char*)dev_workspace;
+    ctx->spins2 = (g.L % 8 == 0) ? (float*)(base + o.spins2) : nullptr; ctx->Jr = (g.L % 8 == 0) ? (float*)(base + o.Jr) : nullptr;
     ctx->spins = (float*)(base + o.spins); ctx->Jg = (float*)(base + o.Jg); ctx->Jt = (g.L % 8 == 0) ? (float*)(base + o.Jt) : nullptr; ctx->Jp = (g.L % 8 == 0) ? (unsigned char*)(base + o.Jp) : nullptr; ctx->Mraw = (float*)(base + o.Mraw);
     ctx->staging = (float*)(base + o.staging); ctx->beta_slot = (float*)(base + o.beta_slot);
     ctx->betas = (double*)(base + o.betas); ctx->E = (double*)(base + o.E); ctx->Epart = (double*)(base + o.Epart);
@@ -623,6 +689,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->res_cpc_req = 0;
     res_plan(ctx);
     zm_plan(ctx);
+    fz_plan(ctx);
     ctx->energies_fresh = false;
     ctx->last_cuda = 0;
 
@@ -719,6 +786,12 @@ int sg_init_sample(sg_ctx* ctx, int sample, int gen_mode, double sigma_D, const 
     k_gather_couplings<<<(ctx->N + 127) / 128, 128, 0, ctx->stream>>>(Mdev, ctx->Jg + (size_t)sample * 2 * ctx->Nh * JG,
                                                                            ctx->Jt ? ctx->Jt + (size_t)sample * 2 * ctx->Nh * JG : nullptr, ctx->L);
     SG_LAUNCHED(ctx);
+    if (ctx->Jr) {
+        const size_t n = (size_t)(ctx->N / 4);
+        k_gather_ring_couplings<<<(unsigned)((n + 127) / 128), 128, 0, ctx->stream>>>(ctx->Jg + (size_t)sample * 2 * ctx->Nh * JG,
+                                                                                   ctx->Jr + (size_t)sample * n * JG, ctx->L);
+        SG_LAUNCHED(ctx);
+    }
 
     if (spins) {
         if (int rc = sg_set_spins(ctx, sample, spins)) return rc;
@@ -1327,8 +1400,8 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
     if (!ctx) return SG_EINVAL;
     switch (knob) {
     case SG_TUNE_SWEEP_IMPL:
-        if (value != SG_SWEEP_AUTO && value != SG_SWEEP_TILED && value != SG_SWEEP_ZMARCH && value != SG_SWEEP_RESIDENT) return SG_EINVAL;
-        if (value == SG_SWEEP_ZMARCH && ctx->L % 8 != 0) return SG_EINVAL;
+        if (value != SG_SWEEP_AUTO && value != SG_SWEEP_TILED && value != SG_SWEEP_ZMARCH && value != SG_SWEEP_RESIDENT && value != SG_SWEEP_FUSED) return SG_EINVAL;
+        if ((value == SG_SWEEP_ZMARCH || value == SG_SWEEP_FUSED) && ctx->L % 8 != 0) return SG_EINVAL;
         if (value == SG_SWEEP_RESIDENT && !ctx->res_ok) return SG_EINVAL;
         ctx->sweep_impl = value;
         return SG_OK;
@@ -1355,6 +1428,7 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
         if (value > 0 && (ctx->L % 8 != 0 || value < 4 || (value & 1) || ctx->L % value != 0)) return SG_EINVAL;
         ctx->zm_zc_req = value;
         zm_plan(ctx);
+        fz_plan(ctx);
         return SG_OK;
     default:
         return SG_EINVAL;

@@ -663,3 +663,35 @@ def test_pt_visit_histogram_and_tau_int_match_oracle(sg, oracle):
     for c in (6.0, 3.0):
         assert sg.walk_tau_int(series, c) == pytest.approx(oracle.walk_tau_int(series, c), rel=1e-12)
     assert len(set(series)) > 2
+
+
+@pytest.mark.parametrize("L,S,R,T,zc", [(8, 2, 2, 5, 0), (8, 1, 1, 3, 4), (16, 2, 4, 12, 0), (16, 1, 2, 20, 8), (24, 1, 2, 16, 0), (24, 1, 1, 7, 6),
+                                        (32, 1, 2, 24, 0), (32, 1, 1, 32, 32), (40, 1, 1, 8, 0)])
+def test_fused_sweep_is_bit_identical_to_two_half_sweeps(sg, L, S, R, T, zc):
+    """SG_SWEEP_FUSED: the colour-fused, out-of-place overrelaxation sweep (colour 0 of plane k and
+    colour 1 of plane k-1 in one pass, ring values recomputed) gives the spins of the two half-sweeps of the z-marching
+    kernel bit for bit -- for every chunk length, tiles that wrap in x1 / x2 (L = 8), several groups, padded groups, odd
+    numbers of sweeps (the state ends in the second buffer) -- and the same energies; heat bath, PT and measurement
+    run unchanged on whichever buffer holds the state."""
+    betas = np.linspace(0.5, 1.9, T)
+    a = sg.SpinGlass(L, S, R, T, betas, seed=23); b = sg.SpinGlass(L, S, R, T, betas, seed=23)
+    a.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_ZMARCH); b.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_FUSED)
+    if zc:
+        b.tune(sg.TUNE_ZCHUNK, zc)
+    for g in (a, b):
+        for s in range(S):
+            g.init_sample(s, sg.GEN_GENERAL9 if s % 2 else sg.GEN_OFFDIAG_SYM, 1.0)
+    for n_or in (1, 2, 3):
+        for g in (a, b):
+            g.sweep_or(n_or)
+        for s in range(S):
+            assert np.array_equal(a.get_spins(s), b.get_spins(s)), (n_or, s)
+        Ea, Eb = a.get_energies(), b.get_energies()
+        assert np.abs(Ea - Eb).max() <= 1e-7 * L ** 3          # fp32 partial sums per thread over a chunk: the chunkings differ
+    for g in (a, b):
+        g.sweep_hb(1); g.sweep_or(3); g.pt_swap(); g.sweep_or(1)
+    for s in range(S):
+        assert np.array_equal(a.get_spins(s), b.get_spins(s)) and np.array_equal(a.get_perm(s)[0], b.get_perm(s)[0])
+    if R > 1:
+        assert np.abs(a.measure()[1] - b.measure()[1]).max() <= 1e-12
+    a.close(); b.close()
