@@ -52,7 +52,9 @@ typedef struct {
                                   (initial spins, heat bath, PT) a single context holding all n_replicas_total would: the PT chains
                                   of a sample are per replica, so its replicas can live on different GPUs with no
                                   exchange inside the Monte Carlo; overlaps are measured between the replicas a context holds */
-    int32_t reserved;          /* must be 0 */
+    int32_t flags;             /* 0, or SG_SHAPE_FUSED_BUFFER: the workspace also holds the second state buffer and the ring
+                                  couplings of the colour-fused sweep (SG_SWEEP_FUSED; L a multiple of 8, else SG_EINVAL):
+                                  sg_workspace_bytes grows by the size of the spins plus N/4 * 224 bytes per sample */
     uint64_t seed;             /* Philox key */
     int32_t first_slot;        /* temperature-slot sharding of one chain (App. A.3: "each GPU updates only 2
                                   lattices ... N_GPU = N_T"): the context holds the configurations (slots) [first_slot, first_slot +
@@ -85,6 +87,7 @@ enum {
 };
 
 enum { SG_KIND_OR = 0, SG_KIND_HB = 1 };
+enum { SG_SHAPE_FUSED_BUFFER = 1 };   /* sg_shape.flags */
 
 /* Device bytes the caller must provide for `shape`; 0 if the shape is invalid. */
 size_t sg_workspace_bytes(const sg_shape* shape);
@@ -270,7 +273,9 @@ double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c);
  *   SG_SWEEP_FUSED    sg_sweep_or only: both colours of a sweep in ONE pass of the colour-fused z-marching kernel (SURVEY.md
  *                     section 8(f1): every spin read once and written once per sweep; the new colour-0 values of the one-site
  *                     ring around a CTA's column are recomputed, the sweep runs out of place between two state buffers);
- *                     heat bath, sg_halfsweep and the energy pass as SG_SWEEP_ZMARCH.  SG_EINVAL unless L is a multiple of 8.
+ *                     heat bath, sg_halfsweep and the energy pass as SG_SWEEP_ZMARCH.  SG_EINVAL unless the context was created
+ *                     with sg_shape.flags = SG_SHAPE_FUSED_BUFFER.  Measured SLOWER than SG_SWEEP_ZMARCH (DESIGN.md section 10:
+ *                     28.7 instead of 38.5 bytes per update from HBM, but 4.9 instead of 3.1 instructions): opt-in.
  * All kernels perform the same arithmetic in the same order: the spins do not depend on the choice.
  * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else even, >= 4 and a divisor of L.
  * SG_TUNE_RES_COPIES: copies per CTA of the resident kernel: 0 = automatic, else 4, 8, 16 or 32 (SG_EINVAL if the lattice

@@ -11,6 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libsg_b200.so")
 
 GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2, 3, 4
 KIND_OR, KIND_HB = 0, 1
+SHAPE_FUSED_BUFFER = 1
 SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
 TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES, TUNE_PACKED, TUNE_MEASURE_IMPL, TUNE_GRAPH = 0, 1, 2, 3, 4, 5
 MEASURE_AUTO, MEASURE_STAGED = 0, 1
@@ -30,7 +31,7 @@ DECLARED_SYMBOLS = [
 class SgShape(ctypes.Structure):
     _fields_ = [("L", ctypes.c_int32), ("n_samples", ctypes.c_int32), ("n_replicas", ctypes.c_int32),
                 ("n_temps", ctypes.c_int32), ("first_sample", ctypes.c_int32), ("first_replica", ctypes.c_int32),
-                ("n_replicas_total", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("n_replicas_total", ctypes.c_int32), ("flags", ctypes.c_int32),
                 ("seed", ctypes.c_uint64), ("first_slot", ctypes.c_int32), ("n_temps_total", ctypes.c_int32)]
 
 
@@ -136,13 +137,13 @@ class SpinGlass:
     """One context of the C-ABI library on the current CUDA device and torch's current stream."""
 
     def __init__(self, L, n_samples, n_replicas, n_temps, betas, seed=1, first_sample=0, device=None, stream=None,
-                 first_replica=0, n_replicas_total=0, first_slot=0, n_temps_total=0):
+                 first_replica=0, n_replicas_total=0, first_slot=0, n_temps_total=0, fused_buffer=False):
         import torch
         self._lib = load_library()
         self.L, self.S, self.R, self.T = int(L), int(n_samples), int(n_replicas), int(n_temps)
         self.N, self.C, self.P = self.L ** 3, self.R * self.T, self.R * (self.R - 1) // 2
         self.Tt = int(n_temps_total) if n_temps_total else self.T      # length of the PT chain (> T: temperature-slot sharding)
-        self.shape = SgShape(self.L, self.S, self.R, self.T, int(first_sample), int(first_replica), int(n_replicas_total), 0, int(seed),
+        self.shape = SgShape(self.L, self.S, self.R, self.T, int(first_sample), int(first_replica), int(n_replicas_total), SHAPE_FUSED_BUFFER if fused_buffer else 0, int(seed),
                              int(first_slot), int(n_temps_total))
         nbytes = int(self._lib.sg_workspace_bytes(ctypes.byref(self.shape)))
         if nbytes == 0:

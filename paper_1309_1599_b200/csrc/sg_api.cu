@@ -78,7 +78,8 @@ bool shape_ok(const sg_shape* s)
     if (!s) return false;
     if (s->L < 2 || (s->L & 1) || s->L > 1024) return false;
     if (s->n_samples <= 0 || s->n_replicas <= 0 || s->n_temps <= 0 || s->first_sample < 0) return false;
-    if (s->reserved != 0 || s->first_replica < 0) return false;
+    if ((s->flags & ~SG_SHAPE_FUSED_BUFFER) != 0 || s->first_replica < 0) return false;
+    if ((s->flags & SG_SHAPE_FUSED_BUFFER) && s->L % 8 != 0) return false;
     if (s->n_replicas_total != 0 && s->first_replica + s->n_replicas > s->n_replicas_total) return false;
     if (s->n_replicas_total == 0 && s->first_replica != 0) return false;
     if (s->first_slot < 0 || s->n_temps_total < 0) return false;
@@ -97,6 +98,7 @@ bool shape_ok(const sg_shape* s)
 struct Geometry {
     int L, N, Nh, S, R, T, Tt, C, NG, Cp, P, tile_sites, ntiles, nchunk, chunk_sites, MS;
     int mq_nchunk, mq_rows_per_cta, mq_Tw, mq_rows_t;
+    bool fused;     // SG_SHAPE_FUSED_BUFFER
 };
 
 Geometry geometry(const sg_shape* s)
@@ -105,6 +107,7 @@ Geometry geometry(const sg_shape* s)
     g.L = s->L; g.N = s->L * s->L * s->L; g.Nh = g.N / 2;
     g.S = s->n_samples; g.R = s->n_replicas; g.T = s->n_temps; g.C = g.R * g.T;
     g.Tt = s->n_temps_total ? s->n_temps_total : s->n_temps;
+    g.fused = (s->flags & SG_SHAPE_FUSED_BUFFER) != 0;
     g.NG = (g.C + G - 1) / G; g.Cp = g.NG * G; g.P = g.R * (g.R - 1) / 2;
     // sweep tiles: 128 consecutive same-colour sites per CTA (4 passes of 32 site slots)
     g.tile_sites = 128;
@@ -149,8 +152,8 @@ Offsets offsets(const Geometry& g)
     Carve c; Offsets o;
     o.spins = c.take((size_t)g.S * g.NG * g.N * SITE_FLOATS * sizeof(float));
     // the colour-fused sweep (L a multiple of 8) is out of place: a second state buffer, and the couplings of the ring sites
-    o.spins2 = c.take((g.L % 8 == 0) ? (size_t)g.S * g.NG * g.N * SITE_FLOATS * sizeof(float) : 0);
-    o.Jr = c.take((g.L % 8 == 0) ? (size_t)g.S * (g.N / 4) * JG * sizeof(float) : 0);
+    o.spins2 = c.take(g.fused ? (size_t)g.S * g.NG * g.N * SITE_FLOATS * sizeof(float) : 0);
+    o.Jr = c.take(g.fused ? (size_t)g.S * (g.N / 4) * JG * sizeof(float) : 0);
     o.Jg = c.take((size_t)g.S * 2 * g.Nh * JG * sizeof(float));
     o.Jt = c.take((g.L % 8 == 0) ? (size_t)g.S * 2 * g.Nh * JG * sizeof(float) : 0);
     o.Jp = c.take((g.L % 8 == 0) ? (size_t)g.S * g.N * 8 : 0);
@@ -393,13 +396,13 @@ int half_sweep_zm(sg_ctx* ctx, int kind, int colour, bool with_energy)
 }
 
 // ---- colour-fused overrelaxation sweep (sg_sweep_fz.cuh): one pass per sweep, out of place ----
-constexpr int FZ_NSO = 4, FZ_NSN = 3, FZ_NJ = 2;
+constexpr int FZ_NSO = 4, FZ_NSN = 3, FZ_NJ = 3;
 
 void fz_plan(sg_ctx* ctx)
 {
     const int L = ctx->L;
     ctx->fz_ZC = 0; ctx->fz_nzc = 0;
-    if (L % 8 != 0) return;
+    if (L % 8 != 0 || !ctx->spins2) return;
     int ZC = 0;
     if (ctx->zm_zc_req > 0) {
         ZC = ctx->zm_zc_req;
@@ -662,7 +665,7 @@ int sg_create(sg_ctx** out, const sg_shape* shape, const double* betas, void* de
     ctx->mq_nchunk = g.mq_nchunk; ctx->mq_rows_per_cta = g.mq_rows_per_cta; ctx->mq_Tw = g.mq_Tw; ctx->mq_rows_t = g.mq_rows_t;
     ctx->stream = (cudaStream_t)cuda_stream;
     char* base = (char*)dev_workspace;
-    ctx->spins2 = (g.L % 8 == 0) ? (float*)(base + o.spins2) : nullptr; ctx->Jr = (g.L % 8 == 0) ? (float*)(base + o.Jr) : nullptr;
+    ctx->spins2 = g.fused ? (float*)(base + o.spins2) : nullptr; ctx->Jr = g.fused ? (float*)(base + o.Jr) : nullptr;
     ctx->spins = (float*)(base + o.spins); ctx->Jg = (float*)(base + o.Jg); ctx->Jt = (g.L % 8 == 0) ? (float*)(base + o.Jt) : nullptr; ctx->Jp = (g.L % 8 == 0) ? (unsigned char*)(base + o.Jp) : nullptr; ctx->Mraw = (float*)(base + o.Mraw);
     ctx->staging = (float*)(base + o.staging); ctx->beta_slot = (float*)(base + o.beta_slot);
     ctx->betas = (double*)(base + o.betas); ctx->E = (double*)(base + o.E); ctx->Epart = (double*)(base + o.Epart);
@@ -1402,6 +1405,7 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
     case SG_TUNE_SWEEP_IMPL:
         if (value != SG_SWEEP_AUTO && value != SG_SWEEP_TILED && value != SG_SWEEP_ZMARCH && value != SG_SWEEP_RESIDENT && value != SG_SWEEP_FUSED) return SG_EINVAL;
         if ((value == SG_SWEEP_ZMARCH || value == SG_SWEEP_FUSED) && ctx->L % 8 != 0) return SG_EINVAL;
+        if (value == SG_SWEEP_FUSED && !ctx->spins2) return SG_EINVAL;
         if (value == SG_SWEEP_RESIDENT && !ctx->res_ok) return SG_EINVAL;
         ctx->sweep_impl = value;
         return SG_OK;

@@ -42,7 +42,8 @@ struct FzGeom {
     static constexpr int JSTAGE = JA + JR + JB;                    // 17920: A interior | A ring | B
     static constexpr int WARPS_I = 8, WARPS_R = 4;                 // interior (A + B) and ring (A only) consumer warps
     static constexpr int CONSUMERS = (WARPS_I + WARPS_R) * 32;     // 384
-    static constexpr int THREADS = CONSUMERS + 32;                 // + one producer warp
+    static constexpr int THREADS = CONSUMERS;                      // no producer warp: the first ring warp issues the bulk copies
+                                                                   // (384 threads leave 168 registers per thread; 416 would cap them at 128)
 };
 
 template <int NSO, int NSN, int NJ>
@@ -179,60 +180,61 @@ __global__ void __launch_bounds__(FzGeom::THREADS, 1) k_sweep_fz(const FzParams 
     float* const dst_grp = p.dst + grp_off;
     auto wrapz = [&](int z) { return (z < 0) ? z + L : ((z >= L) ? z - L : z); };
 
-    if (tid >= Gm::CONSUMERS) {
-        // ---------------- producer warp ----------------
-        const int lane = tid - Gm::CONSUMERS;
-        const uint64_t pol_last = policy_evict_last();
-        const float* const c1 = src_grp + (size_t)p.Nh * SITE_FLOATS;          // old colour-1 sites
-        const size_t tile_lin = (size_t)TYI * p.ntx + TXI;
-        const unsigned char* const Jt0 = reinterpret_cast<const unsigned char*>(p.Jt) + (((size_t)(sample * 2 + 0) * ntile + tile_lin) * L) * Gm::JA;
-        const unsigned char* const Jt1 = reinterpret_cast<const unsigned char*>(p.Jt) + (((size_t)(sample * 2 + 1) * ntile + tile_lin) * L) * Gm::JB;
-        const unsigned char* const Jr0 = reinterpret_cast<const unsigned char*>(p.Jr) + (((size_t)sample * ntile + tile_lin) * L) * Gm::JR;
-        for (int m = 0; m < ZC + 4; ++m) {
-            {   // old colour-1 plane m of the chunk: x3 = z0 - 2 + m
-                const int st = m % NSO;
-                if (m >= NSO) mbar_wait(empty_o(st), ((m / NSO) - 1) & 1);
-                if (lane == 0) mbar_expect_tx(full_o(st), Gm::OLOADED);
-                __syncwarp();
-                const int z = wrapz(z0 - 2 + m);
-                if (lane < Gm::OROWS) {
-                    const int yy = lane - 2;
-                    int y = Y0 + yy; y = (y < 0) ? y + L : ((y >= L) ? y - L : y);
-                    // slots [sa, sb] of the row hold colour-1 sites: h = X0/2 - 1 + slot (periodic)
-                    int sa, sb;
-                    if (yy >= 0 && yy < 8) { sa = 0; sb = 5; }
-                    else if (yy == -1 || yy == 8) { sa = ((yy + z) & 1) ? 1 : 0; sb = sa + 4; }
-                    else { sa = 1; sb = 4; }
-                    const size_t rowh = (size_t)Lh * (y + (size_t)L * z);
-                    const uint32_t dst = smem_u32(oring + (size_t)st * Gm::OSTAGE) + lane * Gm::OROW * Gm::SITE_BYTES;
-                    const int hb = (X0 >> 1) - 1;
-                    if (sa == 0 && X0 == 0) {                                       // the first site wraps
-                        bulk_g2s_hint(dst, c1 + (rowh + (Lh - 1)) * SITE_FLOATS, Gm::SITE_BYTES, full_o(st), pol_last);
-                        sa = 1;
-                    }
-                    if (sb == 5 && X0 + 8 == L) {                                   // the last site wraps
-                        bulk_g2s_hint(dst + 5 * Gm::SITE_BYTES, c1 + rowh * SITE_FLOATS, Gm::SITE_BYTES, full_o(st), pol_last);
-                        sb = 4;
-                    }
-                    bulk_g2s_hint(dst + sa * Gm::SITE_BYTES, c1 + (rowh + (hb + sa)) * SITE_FLOATS, (sb - sa + 1) * Gm::SITE_BYTES, full_o(st), pol_last);
-                }
+    // ---------------- producer duty (first ring warp, at the start of every step) ----------------
+    const int lane = tid & 31;
+    const uint64_t pol_last = policy_evict_last();
+    const float* const c1 = src_grp + (size_t)p.Nh * SITE_FLOATS;          // old colour-1 sites
+    const size_t tile_lin = (size_t)TYI * p.ntx + TXI;
+    const unsigned char* const Jt0 = reinterpret_cast<const unsigned char*>(p.Jt) + (((size_t)(sample * 2 + 0) * ntile + tile_lin) * L) * Gm::JA;
+    const unsigned char* const Jt1 = reinterpret_cast<const unsigned char*>(p.Jt) + (((size_t)(sample * 2 + 1) * ntile + tile_lin) * L) * Gm::JB;
+    const unsigned char* const Jr0 = reinterpret_cast<const unsigned char*>(p.Jr) + (((size_t)sample * ntile + tile_lin) * L) * Gm::JR;
+    // old colour-1 plane m of the chunk (x3 = z0 - 2 + m) into stage m % NSO: one row of the diamond per lane
+    auto load_o = [&](int m) {
+        const int st = m % NSO;
+        if (m >= NSO) mbar_wait(empty_o(st), ((m / NSO) - 1) & 1);
+        if (lane == 0) mbar_expect_tx(full_o(st), Gm::OLOADED);
+        __syncwarp();
+        const int z = wrapz(z0 - 2 + m);
+        if (lane < Gm::OROWS) {
+            const int yy = lane - 2;
+            int y = Y0 + yy; y = (y < 0) ? y + L : ((y >= L) ? y - L : y);
+            // slots [sa, sb] of the row hold colour-1 sites: h = X0/2 - 1 + slot (periodic)
+            int sa, sb;
+            if (yy >= 0 && yy < 8) { sa = 0; sb = 5; }
+            else if (yy == -1 || yy == 8) { sa = ((yy + z) & 1) ? 1 : 0; sb = sa + 4; }
+            else { sa = 1; sb = 4; }
+            const size_t rowh = (size_t)Lh * (y + (size_t)L * z);
+            const uint32_t dst = smem_u32(oring + (size_t)st * Gm::OSTAGE) + lane * Gm::OROW * Gm::SITE_BYTES;
+            const int hb = (X0 >> 1) - 1;
+            if (sa == 0 && X0 == 0) {                                       // the first site wraps
+                bulk_g2s_hint(dst, c1 + (rowh + (Lh - 1)) * SITE_FLOATS, Gm::SITE_BYTES, full_o(st), pol_last);
+                sa = 1;
             }
-            const int n = m - 2;                      // couplings of step n: colour 0 of plane pz (tile, ring), colour 1 of plane pz - 1
-            if (n >= 0) {
-                const int st = n % NJ;
-                if (n >= NJ) mbar_wait(empty_j(st), ((n / NJ) - 1) & 1);
-                if (lane == 0) {
-                    const int pz = wrapz(z0 - 1 + n), pzm = wrapz(z0 - 2 + n);
-                    const uint32_t dst = smem_u32(jring + (size_t)st * Gm::JSTAGE);
-                    mbar_expect_tx(full_j(st), Gm::JSTAGE);
-                    bulk_g2s_hint(dst, Jt0 + (size_t)pz * Gm::JA, Gm::JA, full_j(st), pol_last);
-                    bulk_g2s_hint(dst + Gm::JA, Jr0 + (size_t)pz * Gm::JR, Gm::JR, full_j(st), pol_last);
-                    bulk_g2s_hint(dst + Gm::JA + Gm::JR, Jt1 + (size_t)pzm * Gm::JB, Gm::JB, full_j(st), pol_last);
-                }
-                __syncwarp();
+            if (sb == 5 && X0 + 8 == L) {                                   // the last site wraps
+                bulk_g2s_hint(dst + 5 * Gm::SITE_BYTES, c1 + rowh * SITE_FLOATS, Gm::SITE_BYTES, full_o(st), pol_last);
+                sb = 4;
             }
+            bulk_g2s_hint(dst + sa * Gm::SITE_BYTES, c1 + (rowh + (hb + sa)) * SITE_FLOATS, (sb - sa + 1) * Gm::SITE_BYTES, full_o(st), pol_last);
         }
-        return;
+    };
+    // couplings of step n: colour 0 of plane pz (tile, ring), colour 1 of plane pz - 1
+    auto load_j = [&](int n) {
+        const int st = n % NJ;
+        if (n >= NJ) mbar_wait(empty_j(st), ((n / NJ) - 1) & 1);
+        if (lane == 0) {
+            const int pz = wrapz(z0 - 1 + n), pzm = wrapz(z0 - 2 + n);
+            const uint32_t dst = smem_u32(jring + (size_t)st * Gm::JSTAGE);
+            mbar_expect_tx(full_j(st), Gm::JSTAGE);
+            bulk_g2s_hint(dst, Jt0 + (size_t)pz * Gm::JA, Gm::JA, full_j(st), pol_last);
+            bulk_g2s_hint(dst + Gm::JA, Jr0 + (size_t)pz * Gm::JR, Gm::JR, full_j(st), pol_last);
+            bulk_g2s_hint(dst + Gm::JA + Gm::JR, Jt1 + (size_t)pzm * Gm::JB, Gm::JB, full_j(st), pol_last);
+        }
+        __syncwarp();
+    };
+    const bool duty = (tid >> 5) == Gm::WARPS_I;
+    if (duty) {
+        for (int m = 0; m < NSO; ++m) load_o(m);
+        for (int n = 0; n < NJ - 1; ++n) load_j(n);
     }
 
     const int q = tid & 7;
@@ -288,8 +290,9 @@ __global__ void __launch_bounds__(FzGeom::THREADS, 1) k_sweep_fz(const FzParams 
     __syncwarp();
     if ((tid & 31) == 0) mbar_arrive(empty_o(0));          // plane z0 - 2 serves nothing else
 
-    float own[3][4];            // old colour 0 of the column in plane pz, fetched one step ahead
-    fz_ldg_spin(src_grp + gpos(0, gx[0], gy[0], wrapz(z0 - 1)), own);
+    float own[2][3][4];         // old colour 0 of the column in plane pz, fetched two steps ahead
+    fz_ldg_spin(src_grp + gpos(0, gx[0], gy[0], wrapz(z0 - 1)), own[0]);
+    fz_ldg_spin(src_grp + gpos(0, gx[1], gy[1], wrapz(z0)), own[1]);
 
     for (int n2 = 0; n2 < ZC + 2; n2 += 2) {
 #pragma unroll
@@ -297,6 +300,10 @@ __global__ void __launch_bounds__(FzGeom::THREADS, 1) k_sweep_fz(const FzParams 
             const int n = n2 + d;
             const int pz = wrapz(z0 - 1 + n);
             const int so_cur = (n + 1) % NSO, so_up = (n + 2) % NSO, sj = n % NJ, sn = n % NSN;
+            if (duty) {                   // the planes and couplings of the steps to come, into the stages the last steps freed
+                if (n + NSO < ZC + 4) load_o(n + NSO);
+                if (n + NJ - 1 < ZC + 2) load_j(n + NJ - 1);
+            }
             mbar_wait(full_o(so_up), ((n + 2) / NSO) & 1);
             mbar_wait(full_j(sj), (n / NJ) & 1);
             const unsigned char* const Oc = oring + (size_t)so_cur * Gm::OSTAGE;
@@ -308,9 +315,9 @@ __global__ void __launch_bounds__(FzGeom::THREADS, 1) k_sweep_fz(const FzParams 
 #pragma unroll
             for (int a = 0; a < 3; ++a)
 #pragma unroll
-                for (int j = 0; j < 4; ++j) { hf[a][j] = 0.f; s0[a][j] = own[a][j]; }
-            // the own spin of the next step: still a whole step ahead of its use
-            fz_ldg_spin(src_grp + gpos(0, gx[d ^ 1], gy[d ^ 1], wrapz(z0 + n)), own);
+                for (int j = 0; j < 4; ++j) { hf[a][j] = 0.f; s0[a][j] = own[d][a][j]; }
+            // the own spin of step n + 2 (same column): two steps ahead of its use
+            fz_ldg_spin(src_grp + gpos(0, gx[d], gy[d], wrapz(wrapz(z0 + 1 + n))), own[d]);
             fz_lds_J(Jst + jA, J);
 #pragma unroll
             for (int k = 0; k < 4; ++k) { fz_lds_spin(Oc + oA[d][k], nb); fz_acc(J, k, nb, hf); }

@@ -73,8 +73,18 @@ def test_create_rejects_bad_arguments_without_a_device(lib):
     assert call(binding.SgShape(4, 1, 2, 4, 0, 3, 4, 0, 1), bp(betas), fake, big) == binding.SG_EINVAL
     assert call(binding.SgShape(4, 1, 2, 4, 0, 1, 0, 0, 1), bp(betas), fake, big) == binding.SG_EINVAL
     assert call(binding.SgShape(4, 1, 2, 4, 0, -1, 4, 0, 1), bp(betas), fake, big) == binding.SG_EINVAL
-    assert call(binding.SgShape(4, 1, 2, 4, 0, 0, 0, 7, 1), bp(betas), fake, big) == binding.SG_EINVAL   # reserved != 0
+    assert call(binding.SgShape(4, 1, 2, 4, 0, 0, 0, 7, 1), bp(betas), fake, big) == binding.SG_EINVAL   # unknown flag bits
+    assert call(binding.SgShape(4, 1, 2, 4, 0, 0, 0, 1, 1), bp(betas), fake, big) == binding.SG_EINVAL   # fused buffer: L % 8 != 0
+    # temperature-slot sharding: n_temps_total a multiple of n_temps, first_slot a multiple of n_temps inside it
+    assert call(binding.SgShape(4, 1, 2, 4, 0, 0, 0, 0, 1, 0, 6), bp(betas), fake, big) == binding.SG_EINVAL
+    assert call(binding.SgShape(4, 1, 2, 4, 0, 0, 0, 0, 1, 2, 8), bp(betas), fake, big) == binding.SG_EINVAL
+    assert call(binding.SgShape(4, 1, 2, 4, 0, 0, 0, 0, 1, 8, 8), bp(betas), fake, big) == binding.SG_EINVAL
+    assert call(binding.SgShape(4, 1, 2, 4, 0, 0, 0, 0, 1, 4, 0), bp(betas), fake, big) == binding.SG_EINVAL
     assert ctx.value is None
+    for fn in (lib.sg_pt_publish, lib.sg_pt_swap_gathered):
+        assert fn(None, None) == binding.SG_EINVAL
+    assert lib.sg_energy_by_temp(None, None, None) == binding.SG_EINVAL and lib.sg_pt_visits(None, None) == binding.SG_EINVAL
+    assert np.isnan(lib.sg_walk_tau_int(None, 10, 0.0))
     for fn in (lib.sg_sweep_or, lib.sg_sweep_hb):
         assert fn(None, 1) == binding.SG_EINVAL
     assert lib.sg_pt_swap(None) == binding.SG_EINVAL

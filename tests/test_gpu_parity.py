@@ -674,7 +674,9 @@ def test_fused_sweep_is_bit_identical_to_two_half_sweeps(sg, L, S, R, T, zc):
     numbers of sweeps (the state ends in the second buffer) -- and the same energies; heat bath, PT and measurement
     run unchanged on whichever buffer holds the state."""
     betas = np.linspace(0.5, 1.9, T)
-    a = sg.SpinGlass(L, S, R, T, betas, seed=23); b = sg.SpinGlass(L, S, R, T, betas, seed=23)
+    a = sg.SpinGlass(L, S, R, T, betas, seed=23); b = sg.SpinGlass(L, S, R, T, betas, seed=23, fused_buffer=True)
+    with pytest.raises(sg.SgError):
+        a.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_FUSED)            # no second state buffer in this context's workspace
     a.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_ZMARCH); b.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_FUSED)
     if zc:
         b.tune(sg.TUNE_ZCHUNK, zc)
