@@ -16,7 +16,7 @@ SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
 TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES, TUNE_PACKED, TUNE_MEASURE_IMPL, TUNE_GRAPH = 0, 1, 2, 3, 4, 5
 MEASURE_AUTO, MEASURE_STAGED = 0, 1
 LOGBINS, LOGBIN_OBS = 32, 6
-SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT, SWEEP_FUSED = 0, 1, 2, 3, 4
+SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT, SWEEP_FUSED, SWEEP_CLUSTER = 0, 1, 2, 3, 4, 5
 
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [

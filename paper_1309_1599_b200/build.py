@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsg_b200.so")
 SOURCES = [os.path.join(CSRC, "sg_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("sg_device.cuh", "sg_kernels.cuh", "sg_sweep_zm.cuh", "sg_sweep_res.cuh", "sg_measure.cuh", "sg_sweep_fz.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("sg_device.cuh", "sg_kernels.cuh", "sg_sweep_zm.cuh", "sg_sweep_res.cuh", "sg_measure.cuh", "sg_sweep_fz.cuh", "sg_sweep_cres.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "sg_b200.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -13,6 +13,7 @@
 #include "sg_measure.cuh"
 #include "sg_sweep_res.cuh"
 #include "sg_sweep_fz.cuh"
+#include "sg_sweep_cres.cuh"
 
 using namespace sg;
 
@@ -45,6 +46,7 @@ struct sg_ctx {
     int zm_ok, zm_ZC, zm_nzc;
     uint32_t zm_attr_set = 0;
     uint32_t fz_attr_set = 0;   // the same for k_sweep_fz
+    uint32_t cres_attr_set = 0; // and for k_sweep_cres
     int fz_ZC, fz_nzc;          // chunking of the colour-fused sweep   // template instances of k_sweep_zm whose shared-memory attribute this context has set on its device
     // measure geometry
     int nchunk, chunk_sites, MS;
@@ -585,11 +587,58 @@ int sweeps_resident(sg_ctx* ctx, int kind, int n_sweeps)
     return SG_OK;
 }
 
+// ---- cluster-resident multi-sweep kernel (sg_sweep_cres.cuh): L = 16, the lattice of a copy group in the shared memory of 8 CTAs ----
+bool use_cluster(const sg_ctx* ctx)
+{
+    return ctx->L == CresGeom::L && ctx->sweep_impl == SG_SWEEP_CLUSTER;
+}
+
+template <int KIND>
+int launch_cres(sg_ctx* ctx, const CresParams& p)
+{
+    auto kern = k_sweep_cres<KIND>;
+    const uint32_t bit = 1u << KIND;
+    if (!(ctx->cres_attr_set & bit)) {
+        SG_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CresGeom::SMEM));
+        ctx->cres_attr_set |= bit;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(CresGeom::CS * ctx->NG, ctx->S);
+    cfg.blockDim = dim3(CresGeom::THREADS);
+    cfg.dynamicSmemBytes = CresGeom::SMEM;
+    cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CresGeom::CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    SG_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, p));
+    return SG_OK;
+}
+
+int sweeps_cluster(sg_ctx* ctx, int kind, int n_sweeps)
+{
+    CresParams p;
+    p.spins = ctx->spins; p.Jg = ctx->Jg; p.beta_slot = ctx->beta_slot; p.Epart = ctx->Epart;
+    p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.Cp = ctx->Cp; p.Cg = ctx->Cg; p.Tl = ctx->T; p.Tpad = ctx->Tt - ctx->T;
+    p.n_sweeps = n_sweeps;
+    p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
+    p.hb_counter = (uint32_t)ctx->hb_counter; p.g_first = ctx->g_first;
+    if (int rc = (kind == KIND_HB) ? launch_cres<KIND_HB>(ctx, p) : launch_cres<KIND_OR>(ctx, p)) return rc;
+    SG_LAUNCHED(ctx);
+    if (kind == KIND_HB) note_counter_node(ctx, ctx->stream, 0, offsetof(CresParams, hb_counter), sizeof(CresParams));
+    k_reduce_energy<<<ctx->S * ctx->NG, 256, 0, ctx->stream>>>(ctx->Epart, ctx->E, CresGeom::CS);
+    SG_LAUNCHED(ctx);
+    if (kind == KIND_HB) ctx->hb_counter += (uint64_t)n_sweeps;
+    ctx->energies_fresh = true;
+    return SG_OK;
+}
+
 int sweeps(sg_ctx* ctx, int kind, int n_sweeps)
 {
     if (!ctx || n_sweeps < 0) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     if (n_sweeps > 0 && use_resident(ctx)) return sweeps_resident(ctx, kind, n_sweeps);
+    if (n_sweeps > 0 && use_cluster(ctx)) return sweeps_cluster(ctx, kind, n_sweeps);
     if (kind == KIND_OR && ctx->sweep_impl == SG_SWEEP_FUSED && ctx->fz_ZC > 0 && !use_packed(ctx)) {
         for (int k = 0; k < n_sweeps; ++k)
             if (int rc = sweep_fused(ctx, k == n_sweeps - 1)) return rc;
@@ -1403,9 +1452,10 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
     if (!ctx) return SG_EINVAL;
     switch (knob) {
     case SG_TUNE_SWEEP_IMPL:
-        if (value != SG_SWEEP_AUTO && value != SG_SWEEP_TILED && value != SG_SWEEP_ZMARCH && value != SG_SWEEP_RESIDENT && value != SG_SWEEP_FUSED) return SG_EINVAL;
+        if (value != SG_SWEEP_AUTO && value != SG_SWEEP_TILED && value != SG_SWEEP_ZMARCH && value != SG_SWEEP_RESIDENT && value != SG_SWEEP_FUSED && value != SG_SWEEP_CLUSTER) return SG_EINVAL;
         if ((value == SG_SWEEP_ZMARCH || value == SG_SWEEP_FUSED) && ctx->L % 8 != 0) return SG_EINVAL;
         if (value == SG_SWEEP_FUSED && !ctx->spins2) return SG_EINVAL;
+        if (value == SG_SWEEP_CLUSTER && ctx->L != CresGeom::L) return SG_EINVAL;
         if (value == SG_SWEEP_RESIDENT && !ctx->res_ok) return SG_EINVAL;
         ctx->sweep_impl = value;
         return SG_OK;

@@ -16,7 +16,7 @@ import numpy as np
 
 sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 
-IMPLS = {"auto": 0, "tiled": 1, "zmarch": 2, "resident": 3, "fused": 4}
+IMPLS = {"auto": 0, "tiled": 1, "zmarch": 2, "resident": 3, "fused": 4, "cluster": 5}
 
 
 def _context(sg, W, args, stream=None):

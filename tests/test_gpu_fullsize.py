@@ -148,3 +148,27 @@ def test_pt_and_measure_at_full_size(full, oracle):
         assert np.abs(qk[s, p, t].reshape(-1) - o[1:]).max() <= 1e-6
     for s, r, t in [(0, 0, 0), (3, 3, 47), (1, 2, 20)]:
         assert abs(e[s, r, t] - E[s, r * T + sot[s, r, t]] / N) <= 1e-12 * abs(E).max()
+
+
+def test_fused_and_cluster_kernels_stay_bit_identical_over_many_sweeps():
+    """The opt-in sweep kernels of SURVEY.md section 8(f1) against the z-marching half-sweeps at full size and over many
+    sweeps (a rare race would show here, not in a three-sweep test): the colour-fused sweep at cfg 4's lattice (one
+    sample, 192 copies, 40 sweeps) and the cluster-resident kernel at cfg 2's shape (8 samples, 48 sweeps): every spin
+    of every copy bit for bit."""
+    import paper_1309_1599_b200 as sg
+    for cfg, impl, S, sweeps in ((W.CONFIGS[4], sg.SWEEP_FUSED, 1, 40), (W.CONFIGS[2], sg.SWEEP_CLUSTER, 8, 48)):
+        ctxs = []
+        for k in (sg.SWEEP_ZMARCH, impl):
+            g = sg.SpinGlass(cfg.L, S, cfg.n_replicas, cfg.n_temps, cfg.betas, seed=3, fused_buffer=(k == sg.SWEEP_FUSED))
+            g.tune(sg.TUNE_SWEEP_IMPL, k)
+            for s in range(S):
+                g.init_sample(s, sg.GEN_OFFDIAG_SYM, cfg.sigma_D)
+            ctxs.append(g)
+        for _ in range(sweeps // 8):
+            for g in ctxs:
+                g.sweep_or(8)
+        for s in range(S):
+            assert np.array_equal(ctxs[0].get_spins(s), ctxs[1].get_spins(s)), (cfg.name, s)
+        assert np.abs(ctxs[0].get_energies() - ctxs[1].get_energies()).max() <= 1e-7 * cfg.n_sites
+        for g in ctxs:
+            g.close()

@@ -697,3 +697,41 @@ def test_fused_sweep_is_bit_identical_to_two_half_sweeps(sg, L, S, R, T, zc):
     if R > 1:
         assert np.abs(a.measure()[1] - b.measure()[1]).max() <= 1e-12
     a.close(); b.close()
+
+
+@pytest.mark.parametrize("S,R,T", [(1, 1, 5), (2, 2, 16), (3, 4, 24), (1, 2, 40)])
+def test_cluster_resident_kernel_is_bit_identical_at_L16(sg, S, R, T):
+    """SG_SWEEP_CLUSTER: the L = 16 lattice of a copy group in the shared memory of a cluster of
+    8 CTAs, all sweeps of a call in one launch, x3 neighbours across the cuts through distributed shared memory -- spins and
+    temperature assignment bit-identical to the z-marching kernel for OR and heat bath, one or several sweeps per call,
+    one to three (padded) copy groups; energies to summation order; also through sg_run_units."""
+    L = 16
+    betas = np.linspace(0.5, 2.2, T)
+    a = sg.SpinGlass(L, S, R, T, betas, seed=31, first_sample=1); b = sg.SpinGlass(L, S, R, T, betas, seed=31, first_sample=1)
+    a.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_ZMARCH); b.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_CLUSTER)
+    for g in (a, b):
+        for s in range(S):
+            g.init_sample(s, sg.GEN_GENERAL9 if s % 2 else sg.GEN_OFFDIAG_SYM, 1.0)
+    for n in (1, 2, 3):
+        for g in (a, b):
+            g.sweep_or(n)
+        for s in range(S):
+            assert np.array_equal(a.get_spins(s), b.get_spins(s)), ("or", n, s)
+        assert np.abs(a.get_energies() - b.get_energies()).max() <= 1e-7 * L ** 3
+        for g in (a, b):
+            g.sweep_hb(n)
+        for s in range(S):
+            assert np.array_equal(a.get_spins(s), b.get_spins(s)), ("hb", n, s)
+        assert np.abs(a.get_energies() - b.get_energies()).max() <= 1e-7 * L ** 3
+    E = a.get_energies()
+    for g in (a, b):
+        g.set_energies(E)                         # identical energies: identical PT decisions
+        g.pt_swap()
+        g.sweep_hb(1); g.sweep_or(4)
+    for s in range(S):
+        assert np.array_equal(a.get_spins(s), b.get_spins(s)) and np.array_equal(a.get_perm(s)[0], b.get_perm(s)[0])
+    assert a.get_counters() == b.get_counters()
+    with pytest.raises(sg.SgError):
+        sg.SpinGlass(8, 1, 1, 2, [0.5, 1.0]).tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_CLUSTER)
+    a.close(); b.close()
+
