@@ -264,7 +264,8 @@ double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c);
 /* ---- tuning (results do not depend on it beyond floating-point summation order) ----
  * SG_TUNE_SWEEP_IMPL: which half-sweep kernel serves sg_sweep_or / sg_sweep_hb / the energy pass.
  *   SG_SWEEP_AUTO     the resident kernel when the lattice of 8 copies fits in shared memory (N * 96 B <= 200 KB: L <= 12), else the
- *                     z-marching kernel when L is a multiple of 8, else the tiled kernel (default)
+ *                     z-marching kernel when L is a multiple of 8, else the tiled kernel (default); at L = 16 with at least 15
+ *                     (sample, copy group) pairs the overrelaxation sweeps go to the cluster-resident kernel (SG_SWEEP_CLUSTER)
  *   SG_SWEEP_TILED    the tiled kernel (any even L)
  *   SG_SWEEP_ZMARCH   the z-marching kernel; SG_EINVAL unless L is a multiple of 8
  *   SG_SWEEP_RESIDENT all n sweeps of an sg_sweep_or / sg_sweep_hb call in ONE launch, the lattice of a (sample, group of

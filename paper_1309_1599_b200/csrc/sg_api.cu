@@ -588,9 +588,13 @@ int sweeps_resident(sg_ctx* ctx, int kind, int n_sweeps)
 }
 
 // ---- cluster-resident multi-sweep kernel (sg_sweep_cres.cuh): L = 16, the lattice of a copy group in the shared memory of 8 CTAs ----
-bool use_cluster(const sg_ctx* ctx)
+// explicit request: both sweep kinds; automatic choice: overrelaxation only (measured at cfg 2: 96 against 101 us per OR sweep,
+// 241 against 164 us per heat-bath sweep -- 15 clusters = 120 of the 148 SMs run at once), and only when the clusters fill the GPU
+bool use_cluster(const sg_ctx* ctx, int kind)
 {
-    return ctx->L == CresGeom::L && ctx->sweep_impl == SG_SWEEP_CLUSTER;
+    if (ctx->L != CresGeom::L) return false;
+    if (ctx->sweep_impl == SG_SWEEP_CLUSTER) return true;
+    return ctx->sweep_impl == SG_SWEEP_AUTO && kind == KIND_OR && (long)ctx->S * ctx->NG >= 15;
 }
 
 template <int KIND>
@@ -638,7 +642,7 @@ int sweeps(sg_ctx* ctx, int kind, int n_sweeps)
     if (!ctx || n_sweeps < 0) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     if (n_sweeps > 0 && use_resident(ctx)) return sweeps_resident(ctx, kind, n_sweeps);
-    if (n_sweeps > 0 && use_cluster(ctx)) return sweeps_cluster(ctx, kind, n_sweeps);
+    if (n_sweeps > 0 && use_cluster(ctx, kind)) return sweeps_cluster(ctx, kind, n_sweeps);
     if (kind == KIND_OR && ctx->sweep_impl == SG_SWEEP_FUSED && ctx->fz_ZC > 0 && !use_packed(ctx)) {
         for (int k = 0; k < n_sweeps; ++k)
             if (int rc = sweep_fused(ctx, k == n_sweeps - 1)) return rc;

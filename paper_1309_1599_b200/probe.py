@@ -4,6 +4,7 @@ measurements and as the short command line `ncu` wraps (profiles/*.md name these
     python -m paper_1309_1599_b200.probe sweep --cfg 4 --impl fused --sweeps 32        # us per OR sweep, CUDA events
     python -m paper_1309_1599_b200.probe sweep --cfg 4 --impl zmarch --samples 2 --reps 1 --sweeps 6   # a short run for ncu
     python -m paper_1309_1599_b200.probe units --cfg 1 --graph 1                       # us per MCS through sg_run_units
+    python -m paper_1309_1599_b200.probe exercise --shape 8,2,2,6 --impl zmarch        # every entry point once (compute-sanitizer)
 
 Prints one JSON line per measurement.  Timing is on the device (CUDA events on the context's stream), best and median
 of `--reps` repetitions after a warm-up; nothing here is a bench value (bench.py is)."""
@@ -79,9 +80,37 @@ def units(args):
     print(json.dumps(out), flush=True)
 
 
+def exercise(args):
+    """Every kernel family once on a small shape: what compute-sanitizer (memcheck / racecheck) is pointed at."""
+    import paper_1309_1599_b200 as sg
+    L, S, R, T = [int(v) for v in args.shape.split(",")]
+    betas = np.linspace(0.5, 1.8, T)
+    g = sg.SpinGlass(L, S, R, T, betas, seed=7, fused_buffer=(args.impl == "fused"))
+    g.tune(sg.TUNE_SWEEP_IMPL, IMPLS[args.impl])
+    for s in range(S):
+        g.init_sample(s, sg.GEN_OFFDIAG_SYM, 1.0)
+    g.run_units(9, 2)
+    g.unit(1)
+    g.halfsweep(sg.KIND_OR, 0); g.halfsweep(sg.KIND_HB, 1)
+    e, q0, qk = g.measure()
+    out = dict(probe="exercise", shape=[L, S, R, T], impl=args.impl, e_mean=float(e.mean()), launches=0)
+    if R > 1:
+        g.measure_chiral(); g.accumulate(True); g.get_logbins()
+        buf = g.export_replica(1)
+        q0x, _ = g.measure_cross(0, buf)
+        out["cross_minus_measure"] = float(np.abs(q0x - q0[:, 0]).max())
+    g.schwinger_dyson(); g.pt_walk(); g.pt_visits(); g.pt_stats()
+    spins = g.get_spins(0)
+    out["norm_err"] = float(np.abs(np.sqrt((spins.astype(np.float64) ** 2).sum(axis=1)) - 1.0).max())
+    out["launches"] = g.kernel_launches()
+    g.close()
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
-    ap.add_argument("what", choices=["sweep", "units"])
+    ap.add_argument("what", choices=["sweep", "units", "exercise"])
+    ap.add_argument("--shape", default="8,2,2,6", help="exercise: L,S,R,T")
     ap.add_argument("--cfg", type=int, default=4, help="index into BASELINE.json configs (sg_workloads.CONFIGS)")
     ap.add_argument("--impl", choices=sorted(IMPLS), default="auto", help="SG_TUNE_SWEEP_IMPL")
     ap.add_argument("--kind", choices=["or", "hb"], default="or")
@@ -92,7 +121,7 @@ def main():
     ap.add_argument("--graph", type=int, default=1, help="SG_TUNE_GRAPH")
     ap.add_argument("--reps", type=int, default=5)
     args = ap.parse_args()
-    {"sweep": sweep, "units": units}[args.what](args)
+    {"sweep": sweep, "units": units, "exercise": exercise}[args.what](args)
 
 
 if __name__ == "__main__":
