@@ -66,6 +66,12 @@ struct sg_ctx {
     struct CounterNode { cudaGraphNode_t node; int which; size_t offset, size; };
     bool capturing = false;
     std::vector<CounterNode> counter_nodes;
+    // sg_set_spins: a group is uploaded in UP_CHUNKS site chunks on a copy stream of the library's own, each transposed on the
+    // context's stream as soon as it has landed (events), so the PCIe link does not wait for the transposition kernels
+    static constexpr int UP_CHUNKS = 4;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_copied[UP_CHUNKS] = {}, ev_done[UP_CHUNKS] = {}, ev_start = nullptr;
+    int upload_state = 0;                // 0 = not tried, 1 = pipelined upload available, -1 = not available (plain path)
     cudaStream_t gstream = nullptr;      // capture / replay stream when the context's own stream is the legacy default stream
     cudaEvent_t gevent = nullptr;
     int graph_mode = 1;                  // SG_TUNE_GRAPH: 1 = sg_run_units replays a captured unit when it pays
@@ -783,14 +789,69 @@ int sg_destroy(sg_ctx* ctx)
     cudaStreamSynchronize(ctx->stream);
     if (ctx->gstream) { cudaStreamSynchronize(ctx->gstream); cudaStreamDestroy(ctx->gstream); }
     if (ctx->gevent) cudaEventDestroy(ctx->gevent);
+    if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
+    if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
+    for (int k = 0; k < sg_ctx::UP_CHUNKS; ++k) {
+        if (ctx->ev_copied[k]) cudaEventDestroy(ctx->ev_copied[k]);
+        if (ctx->ev_done[k]) cudaEventDestroy(ctx->ev_done[k]);
+    }
     if (ctx->h_result) cudaFreeHost(ctx->h_result);
     delete ctx;
+    return SG_OK;
+}
+
+// the streams and events of the pipelined upload, created on first use
+static bool upload_ready(sg_ctx* ctx)
+{
+    if (ctx->upload_state != 0) return ctx->upload_state > 0;
+    ctx->upload_state = -1;
+    if (cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); ctx->copy_stream = nullptr; return false; }
+    bool ok = cudaEventCreateWithFlags(&ctx->ev_start, cudaEventDisableTiming) == cudaSuccess;
+    for (int k = 0; ok && k < sg_ctx::UP_CHUNKS; ++k)
+        ok = cudaEventCreateWithFlags(&ctx->ev_copied[k], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&ctx->ev_done[k], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); return false; }
+    ctx->upload_state = 1;
+    return true;
+}
+
+// large lattices: chunks of sites, copy of chunk k+1 (copy stream) under the transposition of chunk k (context's stream)
+static int set_spins_pipelined(sg_ctx* ctx, int sample, const float* in)
+{
+    constexpr int K = sg_ctx::UP_CHUNKS;
+    const int N = ctx->N, nchunk_sites = (N + K - 1) / K;
+    const size_t copy_floats = (size_t)3 * N;
+    SG_CUDA(ctx, cudaEventRecord(ctx->ev_start, ctx->stream));             // the staging buffer may still be in use by earlier work
+    SG_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_start, 0));
+    bool used[K] = {};
+    for (int grp = 0; grp < ctx->NG; ++grp) {
+        const int c0 = grp * G, nc = (ctx->C - c0 < G) ? ctx->C - c0 : G;
+        float* dev = ctx->spins + ((size_t)(sample * ctx->NG + grp) * N) * SITE_FLOATS;
+        for (int k = 0; k < K; ++k) {
+            const int i_first = k * nchunk_sites, n = (N - i_first < nchunk_sites) ? N - i_first : nchunk_sites;
+            if (n <= 0) break;
+            float* stg = ctx->staging + (size_t)G * 3 * i_first;           // region of chunk k: [c][3][n]
+            if (used[k]) SG_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_done[k], 0));
+            if (nc < G) SG_CUDA(ctx, cudaMemsetAsync(stg, 0, (size_t)G * 3 * n * sizeof(float), ctx->copy_stream));
+            SG_CUDA(ctx, cudaMemcpy2DAsync(stg, (size_t)n * sizeof(float), in + (size_t)c0 * copy_floats + i_first, (size_t)N * sizeof(float),
+                                           (size_t)n * sizeof(float), (size_t)nc * 3, cudaMemcpyHostToDevice, ctx->copy_stream));
+            SG_CUDA(ctx, cudaEventRecord(ctx->ev_copied[k], ctx->copy_stream));
+            SG_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_copied[k], 0));
+            k_spins_from_staging_chunk<<<dim3((n + 31) / 32, 3), dim3(32, 8), 0, ctx->stream>>>(stg, dev, N, ctx->L, i_first, n);
+            SG_LAUNCHED(ctx);
+            SG_CUDA(ctx, cudaEventRecord(ctx->ev_done[k], ctx->stream));
+            used[k] = true;
+        }
+    }
+    SG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->energies_fresh = false;
     return SG_OK;
 }
 
 int sg_set_spins(sg_ctx* ctx, int sample, const float* in)
 {
     if (!ctx || !in || sample < 0 || sample >= ctx->S) return SG_EINVAL;
+    if (ctx->N >= 32768 && upload_ready(ctx)) return set_spins_pipelined(ctx, sample, in);
     const size_t copy_floats = (size_t)3 * ctx->N;
     for (int grp = 0; grp < ctx->NG; ++grp) {
         const int c0 = grp * G, nc = (ctx->C - c0 < G) ? ctx->C - c0 : G;

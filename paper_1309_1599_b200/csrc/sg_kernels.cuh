@@ -214,6 +214,24 @@ __global__ void k_spins_from_staging(const float* __restrict__ stg, float* __res
     }
 }
 
+// the same for the sites [i_first, i_first + n) only, staged as [c][3][n] (sg_set_spins uploads a group in site chunks so that
+// the host-to-device copy of one chunk overlaps the transposition of the previous one)
+__global__ void k_spins_from_staging_chunk(const float* __restrict__ stg, float* __restrict__ dev, int N, int L, int i_first, int n)
+{
+    __shared__ float tile[32][33];
+    const int comp = blockIdx.y;
+    const int j0 = blockIdx.x * 32;
+    for (int c = threadIdx.y; c < 32; c += 8) {
+        const int j = j0 + threadIdx.x;
+        tile[c][threadIdx.x] = (j < n) ? stg[((size_t)c * 3 + comp) * n + j] : 0.f;
+    }
+    __syncthreads();
+    for (int r = threadIdx.y; r < 32; r += 8) {
+        const int j = j0 + r;
+        if (j < n) dev[site_slot(i_first + j, L, N >> 1) * SITE_FLOATS + comp * G + threadIdx.x] = tile[threadIdx.x][r];
+    }
+}
+
 __global__ void k_spins_to_staging(const float* __restrict__ dev, float* __restrict__ stg, int N, int L)
 {
     __shared__ float tile[32][33];
