@@ -47,6 +47,7 @@ struct sg_ctx {
     uint32_t zm_attr_set = 0;
     uint32_t fz_attr_set = 0;   // the same for k_sweep_fz
     uint32_t cres_attr_set = 0; // and for k_sweep_cres
+    bool cres_unavailable = false;   // a cluster launch failed on this device: the automatic choice stops using it
     int fz_ZC, fz_nzc;          // chunking of the colour-fused sweep   // template instances of k_sweep_zm whose shared-memory attribute this context has set on its device
     // measure geometry
     int nchunk, chunk_sites, MS;
@@ -530,10 +531,16 @@ constexpr size_t RES_SMEM_MAX = 200 * 1024;   // + 8.4 KB static reduction scrat
 template <int KIND, int CPC>
 int launch_res_c(sg_ctx* ctx, const ResParams& p)
 {
-    const size_t smem = res_smem_bytes(ctx->N, CPC);
+    // the couplings ride along in shared memory when they fit beside the lattice (L <= 8: no global load left in the sweep loop)
+    const bool jsmem = res_smem_bytes(ctx->N, CPC) + res_jsmem_bytes(ctx->N) <= RES_SMEM_MAX;
+    const size_t smem = res_smem_bytes(ctx->N, CPC) + (jsmem ? res_jsmem_bytes(ctx->N) : 0);
     const dim3 grid(ctx->NG * (G / CPC), ctx->S);
 #define SG_RES_CASE(LG)                                                                                              \
-    {                                                                                                                \
+    if (jsmem) {                                                                                                     \
+        auto kern = k_sweep_res<KIND, LG, CPC, true>;                                                                \
+        SG_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES_SMEM_MAX));    \
+        kern<<<grid, RES_THREADS, smem, ctx->stream>>>(p);                                                           \
+    } else {                                                                                                         \
         auto kern = k_sweep_res<KIND, LG, CPC>;                                                                      \
         SG_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RES_SMEM_MAX));    \
         kern<<<grid, RES_THREADS, smem, ctx->stream>>>(p);                                                           \
@@ -581,7 +588,7 @@ int sweeps_resident(sg_ctx* ctx, int kind, int n_sweeps)
     ResParams p;
     p.spins = ctx->spins; p.Jg = ctx->Jg; p.beta_slot = ctx->beta_slot; p.E = ctx->E;
     p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.C = ctx->C; p.Cp = ctx->Cp;
-    p.n_sweeps = n_sweeps;
+    p.n_sweeps = n_sweeps; p.n_hb = 0;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.hb_counter = (uint32_t)ctx->hb_counter;
     p.g_first = ctx->g_first; p.Cg = ctx->Cg; p.Tl = ctx->T; p.Tpad = ctx->Tt - ctx->T;
@@ -593,6 +600,24 @@ int sweeps_resident(sg_ctx* ctx, int kind, int n_sweeps)
     return SG_OK;
 }
 
+// the sweeps of a whole unit -- n_hb heat-bath sweeps, then n_or overrelaxation sweeps -- in ONE launch of the resident kernel
+int sweeps_resident_unit(sg_ctx* ctx, int n_hb, int n_or)
+{
+    ResParams p;
+    p.spins = ctx->spins; p.Jg = ctx->Jg; p.beta_slot = ctx->beta_slot; p.E = ctx->E;
+    p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.C = ctx->C; p.Cp = ctx->Cp;
+    p.n_sweeps = n_or; p.n_hb = n_hb;
+    p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
+    p.hb_counter = (uint32_t)ctx->hb_counter;
+    p.g_first = ctx->g_first; p.Cg = ctx->Cg; p.Tl = ctx->T; p.Tpad = ctx->Tt - ctx->T;
+    if (int rc = launch_res<2>(ctx, p)) return rc;
+    SG_LAUNCHED(ctx);
+    note_counter_node(ctx, ctx->stream, 0, offsetof(ResParams, hb_counter), sizeof(ResParams));
+    ctx->hb_counter += (uint64_t)n_hb;
+    ctx->energies_fresh = true;
+    return SG_OK;
+}
+
 // ---- cluster-resident multi-sweep kernel (sg_sweep_cres.cuh): L = 16, the lattice of a copy group in the shared memory of 8 CTAs ----
 // explicit request: both sweep kinds; automatic choice: overrelaxation only (measured at cfg 2: 96 against 101 us per OR sweep,
 // 241 against 164 us per heat-bath sweep -- 15 clusters = 120 of the 148 SMs run at once), and only when the clusters fill the GPU
@@ -600,7 +625,7 @@ bool use_cluster(const sg_ctx* ctx, int kind)
 {
     if (ctx->L != CresGeom::L) return false;
     if (ctx->sweep_impl == SG_SWEEP_CLUSTER) return true;
-    return ctx->sweep_impl == SG_SWEEP_AUTO && kind == KIND_OR && (long)ctx->S * ctx->NG >= 15;
+    return ctx->sweep_impl == SG_SWEEP_AUTO && !ctx->cres_unavailable && kind == KIND_OR && (long)ctx->S * ctx->NG >= 15;
 }
 
 template <int KIND>
@@ -648,7 +673,14 @@ int sweeps(sg_ctx* ctx, int kind, int n_sweeps)
     if (!ctx || n_sweeps < 0) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     if (n_sweeps > 0 && use_resident(ctx)) return sweeps_resident(ctx, kind, n_sweeps);
-    if (n_sweeps > 0 && use_cluster(ctx, kind)) return sweeps_cluster(ctx, kind, n_sweeps);
+    if (n_sweeps > 0 && use_cluster(ctx, kind)) {
+        const int rc = sweeps_cluster(ctx, kind, n_sweeps);
+        // the automatic choice falls back to the z-marching kernel where 8-CTA clusters of 192 KB cannot be launched
+        // (the launch call itself fails: nothing ran); an explicit request reports the error
+        if (rc == SG_OK || ctx->sweep_impl == SG_SWEEP_CLUSTER || ctx->capturing) return rc;
+        cudaGetLastError();
+        ctx->cres_unavailable = true;
+    }
     if (kind == KIND_OR && ctx->sweep_impl == SG_SWEEP_FUSED && ctx->fz_ZC > 0 && !use_packed(ctx)) {
         for (int k = 0; k < n_sweeps; ++k)
             if (int rc = sweep_fused(ctx, k == n_sweeps - 1)) return rc;
@@ -1056,6 +1088,11 @@ int sg_energy_by_temp(sg_ctx* ctx, const void* dev_all, double* e)
 
 static int one_unit(sg_ctx* ctx, int n_or)
 {
+    if (n_or > 0 && use_resident(ctx)) {              // small lattices: the unit's sweeps in one launch
+        if (int rc = all_inited(ctx)) return rc;
+        if (int rc = sweeps_resident_unit(ctx, 1, n_or)) return rc;
+        return sg_pt_swap(ctx);
+    }
     if (int rc = sg_sweep_hb(ctx, 1)) return rc;
     if (int rc = sg_sweep_or(ctx, n_or)) return rc;
     return sg_pt_swap(ctx);

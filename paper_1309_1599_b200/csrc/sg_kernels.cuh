@@ -318,7 +318,7 @@ __device__ __forceinline__ double pt_uniform(const PtParams& p, int sample, int 
     return ((double)(w[0] >> 9) + 0.5) * (1.0 / 8388608.0);
 }
 
-constexpr int PT_SMEM_PER_TEMP = 2 * sizeof(double) + 2 * sizeof(int) + 2 * sizeof(double);   // E, sot, tos, rr, dbeta (+ slack)
+constexpr int PT_SMEM_PER_TEMP = 4 * sizeof(double) + 2 * sizeof(int) + sizeof(double);   // E, rr, dbeta, ln rr, sot, flags (+ slack)
 
 __global__ void __launch_bounds__(32) k_pt_swap(const PtParams p)
 {
@@ -328,14 +328,15 @@ __global__ void __launch_bounds__(32) k_pt_swap(const PtParams p)
     double* const Es = reinterpret_cast<double*>(pt_sm);          // [T] energy of configuration `slot`
     double* const rr = Es + T;                                    // [T] uniform of pair t
     double* const db = rr + T;                                    // [T] beta_t - beta_{t+1}
-    int* const sot = reinterpret_cast<int*>(db + T);              // [T]
+    double* const lr = db + T;                                    // [T] ln of the uniform of pair t
+    int* const sot = reinterpret_cast<int*>(lr + T);              // [T]
     unsigned char* const acc = reinterpret_cast<unsigned char*>(sot + T);   // [T] pair t accepted
     int* const sot_g = p.slot_of_temp + (size_t)chain * T;
     int* const tos_g = p.temp_of_slot + (size_t)chain * T;
     for (int t = lane; t < T; t += 32) {
         Es[t] = pt_energy(p, sample, r, t);
         sot[t] = sot_g[t];
-        if (t + 1 < T) { rr[t] = pt_uniform(p, sample, r, t); db[t] = p.betas[t] - p.betas[t + 1]; }
+        if (t + 1 < T) { rr[t] = pt_uniform(p, sample, r, t); lr[t] = log(rr[t]); db[t] = p.betas[t] - p.betas[t + 1]; }
     }
     __syncwarp();
     if (lane == 0) {
@@ -345,7 +346,11 @@ __global__ void __launch_bounds__(32) k_pt_swap(const PtParams p)
             const int j = sot[t + 1];
             const double Ej = Es[j];
             const double delta = db[t] * (Ei - Ej);
-            const bool accept = (delta >= 0.0) || (rr[t] < exp(delta));
+            // r < exp(delta) <=> ln r < delta.  The logarithms were taken by the lanes in parallel; the sequential walk only compares.
+            // Both sides carry ~1e-16 of rounding, so outside a band of 1e-12 the comparison of the logarithms IS the decision of
+            // the rule as specified (r < exp(delta) in fp64); inside it (one decision in ~1e12) the rule itself is evaluated.
+            const double gap = lr[t] - delta;
+            const bool accept = (delta >= 0.0) || ((fabs(gap) > 1e-12) ? (gap < 0.0) : (rr[t] < exp(delta)));
             acc[t] = accept ? 1 : 0;
             if (accept) { sot[t] = j; sot[t + 1] = i; }     // i moves on to index t + 1
             else { i = j; Ei = Ej; }

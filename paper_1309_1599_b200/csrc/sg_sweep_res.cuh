@@ -26,19 +26,24 @@ struct ResParams {
     double* E;               // [S][Cp]: total H of every slot, written by the last half-sweep
     int L, N, Nh, NG, C, Cp, Cg;   // Cg: copies per sample of the whole job (stride of the global copy id)
     int Tl, Tpad;                  // slots per replica held here, n_temps_total - Tl (copy_gid)
-    int n_sweeps;
+    int n_sweeps;                  // sweeps of the kernel's kind; KIND_ = 2 (a whole unit): overrelaxation sweeps ...
+    int n_hb;                      // ... after n_hb heat-bath sweeps, all in one launch
     uint32_t key0, key1, hb_counter, g_first;
 };
 
 constexpr int RES_THREADS = 256;
 
 inline size_t res_smem_bytes(int N, int cpc) { return (size_t)N * 3 * cpc * sizeof(float); }
+// JSMEM: the couplings of the sample (both colours) resident in shared memory too, one block per site padded from 56 to
+// RES_JPAD floats (60 words: the blocks of 8 consecutive sites start in 8 different bank groups)
+constexpr int RES_JPAD = 60;
+inline size_t res_jsmem_bytes(int N) { return (size_t)N * RES_JPAD * sizeof(float); }
 
-template <int KIND_, int LOG2L, int CPC>
+template <int KIND_, int LOG2L, int CPC, bool JSMEM = false>
 __global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
 {
     constexpr int QUADS = CPC / 4, RES_SLOTS = RES_THREADS / QUADS, SUBS = G / CPC, SITE = 3 * CPC;
-    extern __shared__ __align__(16) float lat[];      // [2][Nh][3][CPC]: the lattice of this CTA's copies
+    extern __shared__ __align__(16) float lat[];      // [2][Nh][3][CPC]: the lattice of this CTA's copies; JSMEM: then [2][Nh][RES_JPAD] couplings
     __shared__ double red[RES_SLOTS * (CPC + 1)];
     const int tid = threadIdx.x, q = tid % QUADS, slot = tid / QUADS;
     const int grp = blockIdx.x / SUBS, sub = blockIdx.x % SUBS, sample = blockIdx.y;
@@ -50,19 +55,29 @@ __global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
         const int qq = e % QUADS, line = e / QUADS;   // line = site * 3 + component
         st4(lat + line * CPC + qq * 4, ld4(gl + (size_t)line * G + qq * 4));
     }
+    float* const Js = lat + (size_t)p.N * SITE;       // JSMEM: the sample's coupling blocks, by colour then h
+    if (JSMEM) {
+        const float* const Jsrc = p.Jg + (size_t)sample * 2 * p.Nh * JG;
+        for (int e = tid; e < p.N * (JG / 4); e += RES_THREADS) {
+            const int v = e % (JG / 4), site = e / (JG / 4);
+            st4(Js + (size_t)site * RES_JPAD + 4 * v, ldg4(Jsrc + (size_t)site * JG + 4 * v));
+        }
+    }
     __syncthreads();
 
     float* const sp = lat + q * 4;
     float4 beta4 = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (KIND_ == 1) beta4 = ldg4(p.beta_slot + (size_t)sample * p.Cp + c_first + q * 4);
+    if (KIND_ != 0) beta4 = ldg4(p.beta_slot + (size_t)sample * p.Cp + c_first + q * 4);
     uint32_t gid[4];                                  // global ids of this thread's four copies
 #pragma unroll
     for (int j = 0; j < 4; ++j) gid[j] = copy_gid(p.g_first + (uint32_t)sample * (uint32_t)p.Cg, c_first + q * 4 + j, p.Tl, p.Tpad);
     float eacc[4] = { 0.f, 0.f, 0.f, 0.f };
 
-    for (int sw = 0; sw < p.n_sweeps; ++sw) {
+    const int n_total = (KIND_ == 2) ? p.n_hb + p.n_sweeps : p.n_sweeps;
+    for (int sw = 0; sw < n_total; ++sw) {
+        const bool heat_bath = (KIND_ == 1) || (KIND_ == 2 && sw < p.n_hb);
         for (int colour = 0; colour < 2; ++colour) {
-            const bool last = (sw == p.n_sweeps - 1) && (colour == 1);
+            const bool last = (sw == n_total - 1) && (colour == 1);
             const float* const Jc = p.Jg + ((size_t)(sample * 2 + colour) * p.Nh) * JG;
             for (int h = slot; h < p.Nh; h += RES_SLOTS) {
                 int x, y, z;
@@ -75,11 +90,20 @@ __global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
                 const int nb[6] = { xp + row, xm + row, x + L * (yp + L * z), x + L * (ym + L * z),
                                     x + L * (y + L * zp), x + L * (y + L * zm) };
                 float J[JG];
-                const float* jp = Jc + (size_t)h * JG;
+                if (JSMEM) {
+                    const float* jp = Js + (size_t)(colour * p.Nh + h) * RES_JPAD;
 #pragma unroll
-                for (int v = 0; v < JG / 4; ++v) {
-                    const float4 t4 = ldg4(jp + 4 * v);
-                    J[4 * v] = t4.x; J[4 * v + 1] = t4.y; J[4 * v + 2] = t4.z; J[4 * v + 3] = t4.w;
+                    for (int v = 0; v < JG / 4; ++v) {
+                        const float4 t4 = ld4(jp + 4 * v);
+                        J[4 * v] = t4.x; J[4 * v + 1] = t4.y; J[4 * v + 2] = t4.z; J[4 * v + 3] = t4.w;
+                    }
+                } else {
+                    const float* jp = Jc + (size_t)h * JG;
+#pragma unroll
+                    for (int v = 0; v < JG / 4; ++v) {
+                        const float4 t4 = ldg4(jp + 4 * v);
+                        J[4 * v] = t4.x; J[4 * v + 1] = t4.y; J[4 * v + 2] = t4.z; J[4 * v + 3] = t4.w;
+                    }
                 }
                 float* const own = sp + (colour * p.Nh + h) * SITE;
                 float s[3][4], hf[3][4];
@@ -106,7 +130,7 @@ __global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
 #pragma unroll
                             for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * k + 3 * a + b], n[b][j], hf[a][j]);
                 }
-                if (KIND_ == 0) {
+                if (!heat_bath) {
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         or_update(hf[0][j], hf[1][j], hf[2][j], s[0][j], s[1][j], s[2][j]);
