@@ -292,10 +292,12 @@ double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c);
  *                      all pairs) when 2 <= R <= 4, else the staged kernel (default)
  *   SG_MEASURE_STAGED  the staged kernel (sites of all copies through shared memory; any R)
  *   Same products, fp32 row sums in the streaming kernel: results agree to ~1e-8.
+ * SG_TUNE_CLUSTER_CTAS: shape of the cluster-resident kernel (L = 16): 4 (default) = clusters of 4 CTAs, each holding 4 planes of
+ *   16 copies (two clusters per copy group); 8 = clusters of 8 CTAs, each holding 2 planes of all 32 copies.  Same spins.
  * SG_TUNE_GRAPH: 1 (default) = sg_run_units captures one unit in a CUDA graph and replays it (the sweep counters patched in
  *   the captured parameter blocks) when the resident kernel serves the sweeps and n_units >= 8; 0 = always issue the launches
  *   one by one.  Same launches, same results. */
-enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2, SG_TUNE_PACKED = 3, SG_TUNE_MEASURE_IMPL = 4, SG_TUNE_GRAPH = 5 };
+enum { SG_TUNE_SWEEP_IMPL = 0, SG_TUNE_ZCHUNK = 1, SG_TUNE_RES_COPIES = 2, SG_TUNE_PACKED = 3, SG_TUNE_MEASURE_IMPL = 4, SG_TUNE_GRAPH = 5, SG_TUNE_CLUSTER_CTAS = 6 };
 enum { SG_MEASURE_AUTO = 0, SG_MEASURE_STAGED = 1 };
 enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2, SG_SWEEP_RESIDENT = 3, SG_SWEEP_FUSED = 4, SG_SWEEP_CLUSTER = 5 };
 int sg_tune(sg_ctx* ctx, int knob, int value);

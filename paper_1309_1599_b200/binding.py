@@ -13,7 +13,7 @@ GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2,
 KIND_OR, KIND_HB = 0, 1
 SHAPE_FUSED_BUFFER = 1
 SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
-TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES, TUNE_PACKED, TUNE_MEASURE_IMPL, TUNE_GRAPH = 0, 1, 2, 3, 4, 5
+TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES, TUNE_PACKED, TUNE_MEASURE_IMPL, TUNE_GRAPH, TUNE_CLUSTER_CTAS = 0, 1, 2, 3, 4, 5, 6
 MEASURE_AUTO, MEASURE_STAGED = 0, 1
 LOGBINS, LOGBIN_OBS = 32, 6
 SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT, SWEEP_FUSED, SWEEP_CLUSTER = 0, 1, 2, 3, 4, 5

@@ -47,6 +47,7 @@ struct sg_ctx {
     uint32_t zm_attr_set = 0;
     uint32_t fz_attr_set = 0;   // the same for k_sweep_fz
     uint32_t cres_attr_set = 0; // and for k_sweep_cres
+    int cres_cs = 4;                 // SG_TUNE_CLUSTER_CTAS: CTAs per cluster of k_sweep_cres (4: half groups, 4 planes each; 8: whole groups, 2 planes)
     bool cres_unavailable = false;   // a cluster launch failed on this device: the automatic choice stops using it
     int fz_ZC, fz_nzc;          // chunking of the colour-fused sweep   // template instances of k_sweep_zm whose shared-memory attribute this context has set on its device
     // measure geometry
@@ -628,23 +629,24 @@ bool use_cluster(const sg_ctx* ctx, int kind)
     return ctx->sweep_impl == SG_SWEEP_AUTO && !ctx->cres_unavailable && kind == KIND_OR && (long)ctx->S * ctx->NG >= 15;
 }
 
-template <int KIND>
+template <int KIND, int CS>
 int launch_cres(sg_ctx* ctx, const CresParams& p)
 {
-    auto kern = k_sweep_cres<KIND>;
-    const uint32_t bit = 1u << KIND;
+    using Gm = CresGeomT<CS>;
+    auto kern = k_sweep_cres<KIND, CS>;
+    const uint32_t bit = 1u << (KIND * 2 + (CS == 8 ? 1 : 0));
     if (!(ctx->cres_attr_set & bit)) {
-        SG_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CresGeom::SMEM));
+        SG_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Gm::SMEM));
         ctx->cres_attr_set |= bit;
     }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(CresGeom::CS * ctx->NG, ctx->S);
-    cfg.blockDim = dim3(CresGeom::THREADS);
-    cfg.dynamicSmemBytes = CresGeom::SMEM;
+    cfg.gridDim = dim3(CS * (G / Gm::NC) * ctx->NG, ctx->S);
+    cfg.blockDim = dim3(Gm::THREADS);
+    cfg.dynamicSmemBytes = Gm::SMEM;
     cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = CresGeom::CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    attr[0].val.clusterDim.x = CS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     SG_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, p));
     return SG_OK;
@@ -658,10 +660,13 @@ int sweeps_cluster(sg_ctx* ctx, int kind, int n_sweeps)
     p.n_sweeps = n_sweeps;
     p.key0 = (uint32_t)(ctx->shape.seed & 0xffffffffu); p.key1 = (uint32_t)(ctx->shape.seed >> 32);
     p.hb_counter = (uint32_t)ctx->hb_counter; p.g_first = ctx->g_first;
-    if (int rc = (kind == KIND_HB) ? launch_cres<KIND_HB>(ctx, p) : launch_cres<KIND_OR>(ctx, p)) return rc;
+    int rc;
+    if (ctx->cres_cs == 8) rc = (kind == KIND_HB) ? launch_cres<KIND_HB, 8>(ctx, p) : launch_cres<KIND_OR, 8>(ctx, p);
+    else rc = (kind == KIND_HB) ? launch_cres<KIND_HB, 4>(ctx, p) : launch_cres<KIND_OR, 4>(ctx, p);
+    if (rc != SG_OK) return rc;
     SG_LAUNCHED(ctx);
     if (kind == KIND_HB) note_counter_node(ctx, ctx->stream, 0, offsetof(CresParams, hb_counter), sizeof(CresParams));
-    k_reduce_energy<<<ctx->S * ctx->NG, 256, 0, ctx->stream>>>(ctx->Epart, ctx->E, CresGeom::CS);
+    k_reduce_energy<<<ctx->S * ctx->NG, 256, 0, ctx->stream>>>(ctx->Epart, ctx->E, ctx->cres_cs);
     SG_LAUNCHED(ctx);
     if (kind == KIND_HB) ctx->hb_counter += (uint64_t)n_sweeps;
     ctx->energies_fresh = true;
@@ -1574,6 +1579,10 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
     case SG_TUNE_MEASURE_IMPL:
         if (value != SG_MEASURE_AUTO && value != SG_MEASURE_STAGED) return SG_EINVAL;
         ctx->measure_impl = value;
+        return SG_OK;
+    case SG_TUNE_CLUSTER_CTAS:
+        if (value != 4 && value != 8) return SG_EINVAL;
+        ctx->cres_cs = value;
         return SG_OK;
     case SG_TUNE_GRAPH:
         if (value != 0 && value != 1) return SG_EINVAL;

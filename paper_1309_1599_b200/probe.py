@@ -27,6 +27,8 @@ def _context(sg, W, args, stream=None):
     g.tune(sg.TUNE_SWEEP_IMPL, IMPLS[args.impl])
     if args.zchunk:
         g.tune(sg.TUNE_ZCHUNK, args.zchunk)
+    if args.cluster_ctas:
+        g.tune(sg.TUNE_CLUSTER_CTAS, args.cluster_ctas)
     for s in range(S):
         g.init_sample(s, sg.GEN_OFFDIAG_SYM, cfg.sigma_D)
     return cfg, S, g
@@ -49,7 +51,7 @@ def sweep(args):
         torch.cuda.synchronize()
         times.append(e0.elapsed_time(e1) * 1e3 / args.sweeps)
     updates = S * cfg.n_copies * cfg.n_sites
-    out = dict(probe="sweep", cfg=cfg.name, kind=args.kind, impl=args.impl, zchunk=args.zchunk, samples=S, sweeps=args.sweeps,
+    out = dict(probe="sweep", cfg=cfg.name, kind=args.kind, impl=args.impl, zchunk=args.zchunk, cluster_ctas=args.cluster_ctas, samples=S, sweeps=args.sweeps,
                us_per_sweep_best=min(times), us_per_sweep_median=float(np.median(times)),
                ps_per_update_best=min(times) * 1e6 / updates, updates_per_sweep=updates,
                energy_sum=float(g.get_energies().sum()))
@@ -115,6 +117,7 @@ def main():
     ap.add_argument("--impl", choices=sorted(IMPLS), default="auto", help="SG_TUNE_SWEEP_IMPL")
     ap.add_argument("--kind", choices=["or", "hb"], default="or")
     ap.add_argument("--zchunk", type=int, default=0, help="SG_TUNE_ZCHUNK (0 = automatic)")
+    ap.add_argument("--cluster-ctas", type=int, default=0, help="SG_TUNE_CLUSTER_CTAS (0 = the library's default)")
     ap.add_argument("--samples", type=int, default=0, help="samples in the context (0 = the config's)")
     ap.add_argument("--sweeps", type=int, default=32)
     ap.add_argument("--units", type=int, default=0)

@@ -699,8 +699,9 @@ def test_fused_sweep_is_bit_identical_to_two_half_sweeps(sg, L, S, R, T, zc):
     a.close(); b.close()
 
 
+@pytest.mark.parametrize("ctas", [4, 8])
 @pytest.mark.parametrize("S,R,T", [(1, 1, 5), (2, 2, 16), (3, 4, 24), (1, 2, 40)])
-def test_cluster_resident_kernel_is_bit_identical_at_L16(sg, S, R, T):
+def test_cluster_resident_kernel_is_bit_identical_at_L16(sg, S, R, T, ctas):
     """SG_SWEEP_CLUSTER: the L = 16 lattice of a copy group in the shared memory of a cluster of
     8 CTAs, all sweeps of a call in one launch, x3 neighbours across the cuts through distributed shared memory -- spins and
     temperature assignment bit-identical to the z-marching kernel for OR and heat bath, one or several sweeps per call,
@@ -708,7 +709,7 @@ def test_cluster_resident_kernel_is_bit_identical_at_L16(sg, S, R, T):
     L = 16
     betas = np.linspace(0.5, 2.2, T)
     a = sg.SpinGlass(L, S, R, T, betas, seed=31, first_sample=1); b = sg.SpinGlass(L, S, R, T, betas, seed=31, first_sample=1)
-    a.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_ZMARCH); b.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_CLUSTER)
+    a.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_ZMARCH); b.tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_CLUSTER); b.tune(sg.TUNE_CLUSTER_CTAS, ctas)
     for g in (a, b):
         for s in range(S):
             g.init_sample(s, sg.GEN_GENERAL9 if s % 2 else sg.GEN_OFFDIAG_SYM, 1.0)
