@@ -278,8 +278,9 @@ double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c);
  *                     with sg_shape.flags = SG_SHAPE_FUSED_BUFFER.  Measured SLOWER than SG_SWEEP_ZMARCH (DESIGN.md section 10:
  *                     28.7 instead of 38.5 bytes per update from HBM, but 4.9 instead of 3.1 instructions): opt-in.
  *   SG_SWEEP_CLUSTER  L = 16 only (else SG_EINVAL): all n sweeps of an sg_sweep_or / sg_sweep_hb call in ONE launch, the lattice of a
- *                     (sample, group of 32 copies) held in the shared memory of a cluster of 8 CTAs, two planes each; the x3
- *                     neighbours across a cut are read from the neighbouring CTA's shared memory.
+ *                     (sample, group of 32 copies) held in the shared memory of thread-block clusters (SG_TUNE_CLUSTER_CTAS: 4 CTAs
+ *                     holding 4 planes of 16 copies each, or 8 CTAs holding 2 planes of 32 copies); the x3 neighbours across a
+ *                     cut are read from the neighbouring CTA's shared memory.
  * All kernels perform the same arithmetic in the same order: the spins do not depend on the choice.
  * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else even, >= 4 and a divisor of L.
  * SG_TUNE_RES_COPIES: copies per CTA of the resident kernel: 0 = automatic, else 4, 8, 16 or 32 (SG_EINVAL if the lattice
