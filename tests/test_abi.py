@@ -119,3 +119,35 @@ def test_product_does_not_import_the_oracle():
     otext = open(os.path.join(ROOT, "oracle", "sg_oracle.py")).read() + open(os.path.join(ROOT, "oracle", "sg_oracle.c")).read()
     assert "paper_1309_1599_b200" not in otext and "sg_device" not in otext and "sg_kernels" not in otext
     assert not re.search(r"#include\s+\"[^\"]*sg_b200", otext) and "libsg_b200" not in otext
+
+
+def test_binding_constants_and_struct_layout_match_the_header():
+    """The ctypes side restates the header's enums and sg_shape: every enumerator named in include/sg_b200.h has the
+    same value in binding.py, and SgShape has the header's fields in the header's order."""
+    from paper_1309_1599_b200 import binding
+    text = open(os.path.join(ROOT, "include", "sg_b200.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    enums = {}
+    for body in re.findall(r"enum\s*\{(.*?)\}", text, flags=re.S):
+        nxt = 0
+        for item in [t.strip() for t in body.split(",") if t.strip()]:
+            name, _, val = [t.strip() for t in item.partition("=")]
+            nxt = int(val, 0) if val else nxt
+            enums[name] = nxt
+            nxt += 1
+    for m in re.findall(r"#define\s+(SG_[A-Z_]+)\s+(\d+)", text):
+        enums[m[0]] = int(m[1])
+    assert enums["SG_EINVAL"] == binding.SG_EINVAL == -1 and enums["SG_ECUDA"] == binding.SG_ECUDA
+    checked = 0
+    for name, val in enums.items():
+        for prefix in ("SG_", "SG_SHAPE_"):
+            short = name[len(prefix):] if name.startswith(prefix) else None
+            if short and hasattr(binding, short) and isinstance(getattr(binding, short), int):
+                assert getattr(binding, short) == val, name
+                checked += 1
+                break
+    assert checked >= 25, checked
+    struct = re.search(r"typedef struct \{(.*?)\} sg_shape;", text, flags=re.S).group(1)
+    fields = re.findall(r"\b(?:int32_t|uint64_t)\s+([A-Za-z_]+)\s*;", struct)
+    assert fields == [f[0] for f in binding.SgShape._fields_]
+    assert ctypes.sizeof(binding.SgShape) == 48
