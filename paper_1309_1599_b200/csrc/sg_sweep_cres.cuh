@@ -1,14 +1,14 @@
 // sg_sweep_cres.cuh -- the CLUSTER-resident multi-sweep kernel of libsg_b200 for L = 16.
 //
 // Why.  A group of 32 copies of an L = 16 lattice is 4096 sites x 384 bytes = 1.5 MB: too large for one CTA's shared
-// memory (k_sweep_res stops at L = 12), exactly the shared memory of a cluster of 8 CTAs.  The z-marching kernel streams
-// it from HBM / L2 twice per sweep and, at 16 planes, spends a quarter of its time filling and draining its pipeline
-// (cfg 2: 0.71 of the streaming roofline).  Copies are independent between parallel-tempering swaps, so
-// here a cluster keeps the lattice on chip for ALL n sweeps of an sg_sweep_or / sg_sweep_hb call: CTA r of the cluster
-// holds the planes x3 = 2r, 2r+1 (both colours, 192 KB), one spin in six -- the x3 neighbour across the cut -- is read
-// from the neighbouring CTA's shared memory (ld.shared::cluster), a cluster barrier separates the two colours, and the
-// couplings of the 64 sites of a pass (14 KB, shared by the 32 copies) are streamed through a two-stage ring with bulk
-// copies.  Spins cross HBM once per call; per update the SM reads 7 bytes of couplings from L2 and nothing else.
+// memory (k_sweep_res stops at L = 12), exactly the shared memory of 8 SMs.  The z-marching kernel streams it from
+// HBM / L2 twice per sweep and, at 16 planes, spends a quarter of its time filling and draining its pipeline (cfg 2:
+// 0.71 of the streaming roofline).  Copies are independent between parallel-tempering swaps, so here
+// thread-block clusters keep the lattice on chip for ALL n sweeps of an sg_sweep_or / sg_sweep_hb call: every CTA of a
+// cluster holds a slab of consecutive planes (both colours, 192 KB), the x3 neighbours that lie across a cut are read from
+// the neighbouring CTA's shared memory (mapa + ld.shared::cluster), a cluster barrier separates the two colours, and the
+// couplings (shared by the copies of a site) are streamed 64 sites at a time through a two-stage ring of bulk copies.
+// Spins cross HBM once per call; per update the SM reads 7-14 bytes of couplings from L2 and nothing else.
 //
 // Same arithmetic, in the same order, as k_sweep / k_sweep_zm / k_sweep_res (field: neighbours +x1,-x1,+x2,-x2,+x3,-x3),
 // so the spins after a call are bit-identical to the other kernels'.  Thread = (site of the pass, quad of copies).
