@@ -49,10 +49,11 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(_LIB_PATH):
+    path = os.environ.get("SG_B200_LIB", _LIB_PATH)      # another build of the same library (e.g. a measurement variant)
+    if not os.path.exists(path):
         raise ImportError("libsg_b200.so is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
                           "(there is no CPU fallback)")
-    L = ctypes.CDLL(_LIB_PATH)
+    L = ctypes.CDLL(path)
     vp, i, d = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
     u64 = ctypes.c_uint64
     shp = ctypes.POINTER(SgShape)

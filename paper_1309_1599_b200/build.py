@@ -28,6 +28,15 @@ def build(force=False, verbose=False):
     return LIB
 
 
+def build_whatif(n, out):
+    """A measurement-only variant of the library (csrc/sg_sweep_zm.cuh, SG_WHATIF): wrong spins by design, never the product."""
+    subprocess.check_call([nvcc()] + NVCC_FLAGS + ["-DSG_WHATIF=%d" % int(n), "-o", out] + SOURCES)
+    return out
+
+
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    if "--whatif" in sys.argv:
+        print(build_whatif(int(sys.argv[sys.argv.index("--whatif") + 1]), sys.argv[sys.argv.index("--out") + 1]))
+    else:
+        print(build(force=True, verbose="-v" in sys.argv))

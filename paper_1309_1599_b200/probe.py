@@ -5,6 +5,7 @@ measurements and as the short command line `ncu` wraps (profiles/*.md name these
     python -m paper_1309_1599_b200.probe sweep --cfg 4 --impl zmarch --samples 2 --reps 1 --sweeps 6   # a short run for ncu
     python -m paper_1309_1599_b200.probe units --cfg 1 --graph 1                       # us per MCS through sg_run_units
     python -m paper_1309_1599_b200.probe exercise --shape 8,2,2,6 --impl zmarch        # every entry point once (compute-sanitizer)
+    python -m paper_1309_1599_b200.probe sustained --cfg 4 --impl zmarch               # us per OR half-sweep over 6 x 1024 sweeps (power-capped)
 
 Prints one JSON line per measurement.  Timing is on the device (CUDA events on the context's stream), best and median
 of `--reps` repetitions after a warm-up; nothing here is a bench value (bench.py is)."""
@@ -82,6 +83,27 @@ def units(args):
     print(json.dumps(out), flush=True)
 
 
+def sustained(args):
+    """us per OR half-sweep in back-to-back segments of 1024 sweeps: what the kernel holds under the power cap."""
+    import torch
+    import paper_1309_1599_b200 as sg
+    import sg_workloads as W
+    cfg, S, g = _context(sg, W, args)
+    g.sweep_or(8)
+    g.sync()
+    res = []
+    for _ in range(6):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g.sweep_or(1024)
+        e1.record()
+        torch.cuda.synchronize()
+        res.append(round(e0.elapsed_time(e1) * 1e3 / 2048, 1))
+    g.close()
+    print(json.dumps(dict(probe="sustained", cfg=cfg.name, impl=args.impl, lib=os.environ.get("SG_B200_LIB", "libsg_b200.so"),
+                          us_per_halfsweep=res)), flush=True)
+
+
 def exercise(args):
     """Every kernel family once on a small shape: what compute-sanitizer (memcheck / racecheck) is pointed at."""
     import paper_1309_1599_b200 as sg
@@ -111,7 +133,7 @@ def exercise(args):
 
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
-    ap.add_argument("what", choices=["sweep", "units", "exercise"])
+    ap.add_argument("what", choices=["sweep", "units", "exercise", "sustained"])
     ap.add_argument("--shape", default="8,2,2,6", help="exercise: L,S,R,T")
     ap.add_argument("--cfg", type=int, default=4, help="index into BASELINE.json configs (sg_workloads.CONFIGS)")
     ap.add_argument("--impl", choices=sorted(IMPLS), default="auto", help="SG_TUNE_SWEEP_IMPL")
@@ -124,7 +146,7 @@ def main():
     ap.add_argument("--graph", type=int, default=1, help="SG_TUNE_GRAPH")
     ap.add_argument("--reps", type=int, default=5)
     args = ap.parse_args()
-    {"sweep": sweep, "units": units, "exercise": exercise}[args.what](args)
+    {"sweep": sweep, "units": units, "exercise": exercise, "sustained": sustained}[args.what](args)
 
 
 if __name__ == "__main__":
