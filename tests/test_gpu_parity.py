@@ -736,3 +736,39 @@ def test_cluster_resident_kernel_is_bit_identical_at_L16(sg, S, R, T, ctas):
         sg.SpinGlass(8, 1, 1, 2, [0.5, 1.0]).tune(sg.TUNE_SWEEP_IMPL, sg.SWEEP_CLUSTER)
     a.close(); b.close()
 
+
+
+def test_replica_and_slot_sharding_combine(sg):
+    """Four contexts -- replicas (0, 1) / (2, 3) times slots [0, 3) / [3, 6) of every chain -- against one context holding
+    the four replicas and six temperatures of every sample: the global copy id and the global chain id are what key the
+    heat bath and the PT stream, so spins, assignments and PT statistics agree bit for bit after 20 units."""
+    import torch
+    L, S, R, T = 6, 2, 4, 6
+    betas = np.linspace(0.5, 1.5, T)
+    whole = sg.SpinGlass(L, S, R, T, betas, seed=13, first_sample=1)
+    shards = {(rw, sw): sg.SpinGlass(L, S, 2, 3, betas, seed=13, first_sample=1, first_replica=2 * rw, n_replicas_total=4,
+                                     first_slot=3 * sw, n_temps_total=T) for rw in range(2) for sw in range(2)}
+    for g in [whole] + list(shards.values()):
+        for s in range(S):
+            g.init_sample(s, sg.GEN_OFFDIAG_SYM, 1.0)
+    gathered = {rw: torch.empty((2, S, 2, 3), dtype=torch.float64, device="cuda") for rw in range(2)}
+    for _ in range(20):
+        whole.unit(2)
+        for (rw, sw), g in shards.items():
+            g.sweep_hb(1); g.sweep_or(2)
+            g.pt_publish(out=gathered[rw][sw])
+        torch.cuda.synchronize()
+        for (rw, sw), g in shards.items():
+            g.pt_swap_gathered(gathered[rw])
+    for s in range(S):
+        ref = whole.get_spins(s).reshape(R, T, 3, -1)
+        tos = whole.get_perm(s)[0]
+        for (rw, sw), g in shards.items():
+            assert np.array_equal(ref[2 * rw:2 * rw + 2, 3 * sw:3 * sw + 3], g.get_spins(s).reshape(2, 3, 3, -1)), (s, rw, sw)
+            assert np.array_equal(tos[2 * rw:2 * rw + 2], g.get_perm(s)[0])
+    acc = whole.pt_stats()[1]
+    for (rw, sw), g in shards.items():
+        assert np.array_equal(acc[:, 2 * rw:2 * rw + 2], g.pt_stats()[1])
+    assert acc.sum() > 0
+    for g in [whole] + list(shards.values()):
+        g.close()
