@@ -772,3 +772,26 @@ def test_replica_and_slot_sharding_combine(sg):
     assert acc.sum() > 0
     for g in [whole] + list(shards.values()):
         g.close()
+
+
+@pytest.mark.parametrize("T", [853, 1000])
+def test_pt_long_chains_warp_and_serial_kernels_match_oracle(sg, oracle, T):
+    """A chain of 853 temperatures is the longest the warp-per-chain kernel stages in shared memory, 1000 falls back to
+    k_pt_swap_serial: decisions, statistics, walk labels and round trips identical to the oracle (fed identical energies)."""
+    L, S, R = 2, 1, 2
+    betas = np.linspace(0.2, 3.0, T)
+    sim, gpu = make_pair(oracle, sg, L, S, R, T, betas, seed=17)
+    rng = np.random.default_rng(9)
+    for k in range(6):
+        E = rng.normal(0.0, 0.7 / (betas[1] - betas[0]), size=(S, R * T))
+        gpu.set_energies(E)
+        gpu.pt_swap()
+        sim.pt_swap(energies=E)
+    tos, sot = gpu.get_perm(0)
+    assert np.array_equal(tos, sim.temp_of_slot[0]) and np.array_equal(sot, sim.slot_of_temp[0])
+    att, acc = gpu.pt_stats()
+    assert np.array_equal(att, sim.attempts) and np.array_equal(acc, sim.accepts) and 0 < acc.sum() < att.sum()
+    trips, lab = gpu.pt_walk()
+    assert np.array_equal(lab, sim.walk_label) and np.array_equal(trips, sim.round_trips[..., 0])
+    assert np.array_equal(gpu.pt_visits(), sim.visits)
+    gpu.close()
