@@ -99,8 +99,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS) k_sweep(const SweepParams p)
             for (int a = 0; a < 3; ++a)
 #pragma unroll
                 for (int b = 0; b < 3; ++b)
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * k + 3 * a + b], n[b][j], hf[a][j]);
+                    fma4(J[9 * k + 3 * a + b], n[b], hf[a]);
         }
 
         if (KIND == KIND_OR) {
@@ -927,8 +926,7 @@ __global__ void __launch_bounds__(SWEEP_THREADS) k_sd(const SdParams p)
             for (int a = 0; a < 3; ++a)
 #pragma unroll
                 for (int b = 0; b < 3; ++b)
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * k + 3 * a + b], n[b][j], hf[a][j]);
+                    fma4(J[9 * k + 3 * a + b], n[b], hf[a]);
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {

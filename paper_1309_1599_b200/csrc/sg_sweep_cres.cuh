@@ -243,8 +243,7 @@ __global__ void __launch_bounds__(CresGeomT<CS_>::THREADS, 1) k_sweep_cres(const
                     for (int a = 0; a < 3; ++a)
 #pragma unroll
                         for (int bb = 0; bb < 3; ++bb)
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * k + 3 * a + bb], n[bb][j], hf[a][j]);
+                            fma4(J[9 * k + 3 * a + bb], n[bb], hf[a]);
                 }
                 if (KIND_ == KIND_OR) {
 #pragma unroll

@@ -98,8 +98,7 @@ __device__ __forceinline__ void fz_acc(const float (&J)[JG], int nbk, const floa
     for (int a = 0; a < 3; ++a)
 #pragma unroll
         for (int bb = 0; bb < 3; ++bb)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * nbk + 3 * a + bb], n[bb][j], hf[a][j]);
+            fma4(J[9 * nbk + 3 * a + bb], n[bb], hf[a]);
 }
 __device__ __forceinline__ void fz_lds_spin(const unsigned char* p, float (&n)[3][4])
 {

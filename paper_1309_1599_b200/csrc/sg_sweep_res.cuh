@@ -127,8 +127,7 @@ __global__ void __launch_bounds__(RES_THREADS) k_sweep_res(const ResParams p)
                     for (int a = 0; a < 3; ++a)
 #pragma unroll
                         for (int b = 0; b < 3; ++b)
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * k + 3 * a + b], n[b][j], hf[a][j]);
+                    fma4(J[9 * k + 3 * a + b], n[b], hf[a]);
                 }
                 if (!heat_bath) {
 #pragma unroll

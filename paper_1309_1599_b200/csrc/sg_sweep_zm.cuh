@@ -379,9 +379,7 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
-                    for (int bb = 0; bb < 3; ++bb)
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) hf[a][j] = fmaf(J[9 * nbk + 3 * a + bb], n[bb][j], hf[a][j]);
+                    for (int bb = 0; bb < 3; ++bb) fma4(J[9 * nbk + 3 * a + bb], n[bb], hf[a]);
             }
             // the stage of plane k and the coupling stage are dead for this warp once the loads above retire
             __syncwarp();
