@@ -74,7 +74,8 @@ enum {
     SG_EINVAL = -1, /* bad argument: odd or too small L, counts <= 0, non-finite or non-monotone betas,
                        NULL where not allowed, sample out of range, workspace too small or misaligned */
     SG_ESTATE = -2, /* a sample was used before sg_init_sample */
-    SG_ECUDA = -3   /* a CUDA call failed (no device, launch failure, ...); see sg_last_cuda_error */
+    SG_ECUDA = -3,  /* a CUDA call failed (no device, launch failure, ...); see sg_last_cuda_error */
+    SG_ELIMIT = -4  /* sg_chiral_cross_static only: the shape needs more than the fixed SG_STATIC_SCRATCH_BYTES */
 };
 
 /* coupling generator modes of sg_init_sample */
@@ -210,6 +211,57 @@ int sg_measure_cross(sg_ctx* ctx, int r, const void* dev_remote, double* q0, dou
  * Errors: SG_EINVAL (NULL, r out of range, T > 256), SG_ESTATE, SG_ECUDA. */
 int sg_export_chirality(sg_ctx* ctx, int r, void* dev_out);
 int sg_chiral_cross(sg_ctx* ctx, const void* dev_a, const void* dev_b, double* qc0, double* qck);
+
+/* sg_chiral_cross without a context and without any allocation (the arithmetic of sg_chiral_cross, Eq. (2)).
+ *
+ * Who this is for.  Everything above needs an sg_ctx on top of a caller-allocated workspace, and a context itself pins host
+ * memory when it is created (cudaHostAlloc) and creates streams and events the first time some calls are used.  Some callers
+ * of this library cannot make allocating calls, or cannot afford them, at the point where they want the chiral-glass overlaps
+ * of two zeta buffers they already hold on the device (their own sg_export_chirality output, or a partner rank's that
+ * arrived through an all-gather or a peer copy):
+ *   - a measurement process that runs next to the Monte Carlo ranks on a GPU whose HBM has been handed out in full (the sweep
+ *     workspaces sized to the 180 GB, or a framework's memory pool that owns all of it): a cudaMalloc there fails, or succeeds
+ *     only by making the pool give memory back;
+ *   - a caller in the middle of a run for whom cudaMalloc / cudaFree are too expensive: both synchronise the whole device, so
+ *     every sweep in flight on every other stream of the GPU waits for them;
+ *   - code that is not allowed to touch the allocator at all (a callback, a plug-in of a host application that manages device
+ *     memory itself and audits its use).
+ * For them the partial sums that sg_chiral_cross keeps in the context's workspace live in a fixed array that is part of the
+ * library image: SG_STATIC_SCRATCH_BYTES (16 MiB) of device memory, held by every GPU on which the library is loaded from the
+ * moment its CUDA module loads until the process exits, whether or not this call is ever made.
+ *
+ *   L, n_samples (S), n_temps (T)   shape of the two buffers: L even, 2 <= L <= SG_STATIC_MAX_L, S >= 1, 1 <= T <= 256
+ *   dev_a, dev_b   DEVICE, float [S][3][N][T] as sg_export_chirality writes them (mu, site, temperature; temperature fastest);
+ *                  read only; they may be the same buffer
+ *   dev_out        DEVICE, double [S*T*21], caller-owned, 8-byte aligned: qc0 [S][T][3] followed by qck [S][T][3][3][2] with the
+ *                  meaning and normalisation of sg_chiral_cross.  Written asynchronously on the stream; NOT copied to the host
+ *                  (the caller reads it in stream order).  Must not overlap the inputs.
+ *   cuda_stream    a cudaStream_t (NULL = the legacy default stream); the buffers must belong to the CURRENT device
+ *   cuda_error     may be NULL; on SG_ECUDA receives the cudaError_t (there is no context to keep it)
+ *
+ * Capacity.  4096 + S * 128 * ((256/T)*T) * 21 * 8 bytes (256/T an integer division) must not exceed
+ * SG_STATIC_SCRATCH_BYTES: S <= 3 samples per call is accepted for every T, more only where (256/T)*T is small.  A larger job
+ * is split by sample by the caller (one call per group of samples, ordered on one stream): the slice [s][3][N][T] of each input
+ * is contiguous, and each call writes a complete [qc0 | qck] block for its own samples.  Beyond the capacity the call returns
+ * SG_ELIMIT and does nothing; it never falls back to allocating.
+ *
+ * First call on a device.  The device address of the array is looked up once per device (cudaGetSymbolAddress, with that
+ * device current) by the first call made on it; that look-up loads the library's CUDA module if nothing has yet.  Make this
+ * first call during set-up, before any stream capture is begun.  Later calls only launch kernels (three per call) and call
+ * no cudaMalloc, cudaFree, cudaHostAlloc, stream or event creation, nor any library routine that allocates.
+ *
+ * Sharing.  There is ONE array per device and every call on that device uses it, from any thread and any stream.  Calls
+ * that can overlap on the GPU (different streams without an ordering between them, or different host threads) race on it and
+ * return garbage: order them on one stream or with events.  The array keeps whatever the last call left in it; nothing in it
+ * has to start at zero, because every element a call reads has been written by the same call first (the Fourier phase table
+ * and all partial sums of the shape at hand), so leftovers of a call with another shape are harmless.
+ * Results equal sg_chiral_cross to rounding (same products and summation order; the phase table is computed on the device,
+ * within an ulp of the host's).  Errors: SG_EINVAL (NULL, odd or out-of-range L, S < 1, T outside 1..256, misaligned output),
+ * SG_ELIMIT, SG_ECUDA. */
+#define SG_STATIC_SCRATCH_BYTES (16u << 20)
+#define SG_STATIC_MAX_L 256
+int sg_chiral_cross_static(int L, int n_samples, int n_temps, const void* dev_a, const void* dev_b, void* dev_out,
+                           void* cuda_stream, int* cuda_error);
 
 /* Schwinger-Dyson monitor (App. A.4, Eq. (A6)):
  *   2 T <s_x.h_x> - <(h_x)^2 - (s_x.h_x)^2> = 0 in equilibrium, "averaged over all the sites in the lattice".

@@ -12,7 +12,8 @@ _LIB_PATH = os.path.join(_HERE, "libsg_b200.so")
 GEN_OFFDIAG_SYM, GEN_PAPER_SYM6, GEN_GENERAL9, GEN_BIMODAL, GEN_FERRO = 0, 1, 2, 3, 4
 KIND_OR, KIND_HB = 0, 1
 SHAPE_FUSED_BUFFER = 1
-SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA = 0, -1, -2, -3
+SG_OK, SG_EINVAL, SG_ESTATE, SG_ECUDA, SG_ELIMIT = 0, -1, -2, -3, -4
+STATIC_SCRATCH_BYTES, STATIC_MAX_L = 16 << 20, 256
 TUNE_SWEEP_IMPL, TUNE_ZCHUNK, TUNE_RES_COPIES, TUNE_PACKED, TUNE_MEASURE_IMPL, TUNE_GRAPH, TUNE_CLUSTER_CTAS = 0, 1, 2, 3, 4, 5, 6
 MEASURE_AUTO, MEASURE_STAGED = 0, 1
 LOGBINS, LOGBIN_OBS = 32, 6
@@ -21,7 +22,7 @@ SWEEP_AUTO, SWEEP_TILED, SWEEP_ZMARCH, SWEEP_RESIDENT, SWEEP_FUSED, SWEEP_CLUSTE
 # every symbol include/sg_b200.h declares (checked against the header by tests/test_abi.py)
 DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_init_sample_bimodal", "sg_sweep_or", "sg_sweep_hb",
-    "sg_pt_swap", "sg_pt_publish", "sg_pt_swap_gathered", "sg_energy_by_temp", "sg_run_units", "sg_measure", "sg_accumulate", "sg_get_logbins", "sg_export_replica", "sg_measure_cross", "sg_export_chirality", "sg_chiral_cross", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
+    "sg_pt_swap", "sg_pt_publish", "sg_pt_swap_gathered", "sg_energy_by_temp", "sg_run_units", "sg_measure", "sg_accumulate", "sg_get_logbins", "sg_export_replica", "sg_measure_cross", "sg_export_chirality", "sg_chiral_cross", "sg_chiral_cross_static", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
     "sg_halfsweep", "sg_pt_stats", "sg_pt_walk", "sg_pt_visits", "sg_walk_tau_int", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
@@ -92,6 +93,7 @@ def load_library():
     L.sg_measure_cross.argtypes = [vp, i, vp, vp, vp]; L.sg_measure_cross.restype = i
     L.sg_export_chirality.argtypes = [vp, i, vp]; L.sg_export_chirality.restype = i
     L.sg_chiral_cross.argtypes = [vp, vp, vp, vp, vp]; L.sg_chiral_cross.restype = i
+    L.sg_chiral_cross_static.argtypes = [i, i, i, vp, vp, vp, vp, ctypes.POINTER(i)]; L.sg_chiral_cross_static.restype = i
     L.sg_pt_walk.argtypes = [vp, vp, vp]; L.sg_pt_walk.restype = i
     L.sg_tune.argtypes = [vp, i, i]; L.sg_tune.restype = i
     L.sg_sync.argtypes = [vp]; L.sg_sync.restype = i
@@ -132,6 +134,37 @@ def philox4x32_10(ctr, key):
     o = (ctypes.c_uint32 * 4)()
     load_library().sg_philox4x32_10(c, k, o)
     return [int(v) for v in o]
+
+
+def chiral_cross_static(L, n_samples, n_temps, za, zb, out=None, stream=None):
+    """sg_chiral_cross_static: the chiral-glass overlaps between two export_chirality tensors WITHOUT a context and without
+    the library allocating anything -- for callers that hold two zeta buffers on the device but must not (all of HBM is already
+    handed out), cannot afford to (cudaMalloc / cudaFree stall every stream of the GPU) or are not allowed to allocate.  The
+    partial sums go to a fixed 16 MiB array inside the library (STATIC_SCRATCH_BYTES; every GPU that loads the library holds
+    it until the process exits), so n_samples <= 3 per call is always accepted and larger shapes raise SgError(SG_ELIMIT):
+    split them by sample.  All calls on a device share that array: order them on one stream, or they race.  The first call on
+    a device looks the array's address up; make it during set-up.
+
+    za, zb: float32 device tensors [n_samples][3][L^3][n_temps]; out: float64 device tensor of n_samples * n_temps * 21
+    elements (pass one you already own if even torch must not allocate; None = torch.empty).  Asynchronous on `stream` (torch's
+    current stream if None).  Returns (qc0 [S][T][3], qck [S][T][3][3][2]) as views of `out`, still on the device."""
+    import torch
+    S, T, N = int(n_samples), int(n_temps), int(L) ** 3
+    for z in (za, zb):
+        assert z.is_cuda and z.is_contiguous() and z.dtype == torch.float32 and z.numel() == S * 3 * N * T
+    if out is None:
+        out = torch.empty(S * T * 21, dtype=torch.float64, device=za.device)
+    assert out.is_cuda and out.is_contiguous() and out.dtype == torch.float64 and out.numel() == S * T * 21
+    assert out.device == za.device == zb.device == torch.device("cuda", torch.cuda.current_device()), "buffers must be on the current device"
+    if stream is None:
+        stream = torch.cuda.current_stream(za.device)
+    err = ctypes.c_int(0)
+    rc = load_library().sg_chiral_cross_static(int(L), S, T, ctypes.c_void_p(za.data_ptr()), ctypes.c_void_p(zb.data_ptr()),
+                                               ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(stream.cuda_stream), ctypes.byref(err))
+    if rc != SG_OK:
+        raise SgError(rc, "sg_chiral_cross_static", int(err.value))
+    flat = out.view(-1)
+    return flat[:S * T * 3].view(S, T, 3), flat[S * T * 3:].view(S, T, 3, 3, 2)
 
 
 class SpinGlass:

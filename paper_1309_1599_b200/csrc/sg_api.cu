@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1610,6 +1611,90 @@ int sg_sync(sg_ctx* ctx)
 uint64_t sg_kernel_launches(const sg_ctx* ctx) { return ctx ? ctx->launches : 0; }
 int sg_last_cuda_error(const sg_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
 
+}  // extern "C"
+
+// ---- sg_chiral_cross_static: the allocation-free variant of sg_chiral_cross (include/sg_b200.h) ----
+// The partial sums of k_chiral_cross and the Fourier phase table, which a context keeps in the caller's workspace, live here in
+// an array that is part of the library image.  In HOST code the name g_static_scratch is only a handle for the runtime, not a
+// device address (a kernel handed `g_static_scratch` from the host would fault, or scribble over host memory where the GPU can
+// reach it): the device address comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[SG_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr size_t STATIC_PHASE_BYTES = 4096;      // double [SG_STATIC_MAX_L][2] at the head of the array, partial sums behind it
+static_assert((size_t)SG_STATIC_MAX_L * 2 * sizeof(double) <= STATIC_PHASE_BYTES, "phase table");
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;                                   // guards the table below (set-up only; the calls do not hold it)
+unsigned char* g_static_addr[STATIC_MAX_DEVICES] = {};       // device address of g_static_scratch on device d; nullptr = not set up
+
+// Set-up of the current device on the first call made on it.  No allocation: the array already exists on every device that
+// has the module loaded; cudaGetSymbolAddress only reports where (and loads the module if this is the library's first CUDA call).
+int static_scratch_of_current_device(unsigned char** out, cudaError_t* err)
+{
+    int dev = -1;
+    *err = cudaGetDevice(&dev);
+    if (*err != cudaSuccess) return SG_ECUDA;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) { *err = cudaErrorInvalidDevice; return SG_ECUDA; }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        void* p = nullptr;
+        *err = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (*err != cudaSuccess || !p) { if (*err == cudaSuccess) *err = cudaErrorInvalidSymbol; return SG_ECUDA; }
+        g_static_addr[dev] = (unsigned char*)p;
+    }
+    *out = g_static_addr[dev];
+    return SG_OK;
+}
+}  // namespace
+
+// phase[x] = (cos, sin)(2 pi x / L), the table sg_create uploads for a context, here written by the device for itself
+__global__ void k_static_phase(double* __restrict__ phase, int L)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= L) return;
+    double sn, cs;
+    sincospi(2.0 * (double)x / (double)L, &sn, &cs);
+    phase[2 * x] = cs;
+    phase[2 * x + 1] = sn;
+}
+
+extern "C" {
+
+int sg_chiral_cross_static(int L, int n_samples, int n_temps, const void* dev_a, const void* dev_b, void* dev_out,
+                           void* cuda_stream, int* cuda_error)
+{
+    if (cuda_error) *cuda_error = 0;
+    if (!dev_a || !dev_b || !dev_out || ((uintptr_t)dev_out & 7)) return SG_EINVAL;
+    if (L < 2 || (L & 1) || L > SG_STATIC_MAX_L || n_samples < 1 || n_temps < 1 || n_temps > XTHREADS) return SG_EINVAL;
+    const int S = n_samples, T = n_temps, N = L * L * L;
+    const int rows = XTHREADS / T;
+    // the partial sums k_chiral_cross writes and k_reduce_chiral_cross reads: [S][XCHUNKS * rows][T][21] doubles
+    const unsigned long long need = (unsigned long long)S * XCHUNKS * rows * T * 21ull * sizeof(double);
+    if (need > (unsigned long long)SG_STATIC_SCRATCH_BYTES - STATIC_PHASE_BYTES) return SG_ELIMIT;
+    if ((long long)S * T * 21 > 0x7fffffffLL) return SG_ELIMIT;     // unreachable under the byte limit; keeps the int arithmetic below honest
+    unsigned char* base = nullptr;
+    cudaError_t e = cudaSuccess;
+    if (int rc = static_scratch_of_current_device(&base, &e)) { if (cuda_error) *cuda_error = (int)e; return rc; }
+    double* phase = (double*)base;
+    double* xpart = (double*)(base + STATIC_PHASE_BYTES);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    // Every element read below is written first by this call: the phase table for this L, then all S * XCHUNKS * rows * T * 21
+    // partial sums (chunks past the end of the lattice store zeros), so the leftovers of earlier calls never matter.
+    k_static_phase<<<(L + 127) / 128, 128, 0, stream>>>(phase, L);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        k_chiral_cross<<<dim3(XCHUNKS, S), XTHREADS, 0, stream>>>((const float*)dev_a, (const float*)dev_b, phase, xpart, L, N, T);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) {
+        const int total = S * T * 21;
+        k_reduce_chiral_cross<<<(total + 127) / 128, 128, 0, stream>>>(xpart, (double*)dev_out, S, T, XCHUNKS * rows, N);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) { if (cuda_error) *cuda_error = (int)e; return SG_ECUDA; }
+    return SG_OK;
+}
+
 const char* sg_strerror(int code)
 {
     switch (code) {
@@ -1617,6 +1702,7 @@ const char* sg_strerror(int code)
     case SG_EINVAL: return "invalid argument";
     case SG_ESTATE: return "sample not initialised";
     case SG_ECUDA: return "CUDA call failed (see sg_last_cuda_error)";
+    case SG_ELIMIT: return "shape exceeds the fixed scratch array of the allocation-free entry point (SG_STATIC_SCRATCH_BYTES): split the call by sample";
     default: return "unknown error";
     }
 }

@@ -99,6 +99,31 @@ def test_create_rejects_bad_arguments_without_a_device(lib):
     assert lib.sg_measure_chiral(None, None, None) == binding.SG_EINVAL and lib.sg_schwinger_dyson(None, None) == binding.SG_EINVAL
 
 
+def test_static_entry_point_validates_before_touching_the_device(lib):
+    """sg_chiral_cross_static checks its arguments and its fixed capacity before any CUDA call, so the codes can be
+    checked without a device: NULL / bad shapes -> SG_EINVAL, a shape beyond SG_STATIC_SCRATCH_BYTES -> SG_ELIMIT."""
+    from paper_1309_1599_b200 import binding
+    p = ctypes.c_void_p(4096)      # never dereferenced: every call below is rejected first
+    err = ctypes.c_int(7)
+    call = lambda L, S, T, a=p, b=p, o=p: lib.sg_chiral_cross_static(L, S, T, a, b, o, None, ctypes.byref(err))
+    assert call(8, 1, 4, a=None) == binding.SG_EINVAL and call(8, 1, 4, b=None) == binding.SG_EINVAL
+    assert call(8, 1, 4, o=None) == binding.SG_EINVAL and call(8, 1, 4, o=ctypes.c_void_p(4100)) == binding.SG_EINVAL
+    assert err.value == 0                                                         # cleared on entry
+    for L, S, T in ((7, 1, 4), (0, 1, 4), (binding.STATIC_MAX_L + 2, 1, 4), (8, 0, 4), (8, 1, 0), (8, 1, 257)):
+        assert call(L, S, T) == binding.SG_EINVAL, (L, S, T)
+    # capacity: 4096 + S * 128 * ((256 // T) * T) * 21 * 8 bytes against the fixed 16 MiB
+    need = lambda S, T: 4096 + S * 128 * ((256 // T) * T) * 21 * 8
+    for S, T in ((4, 256), (4, 48), (4, 1), (7, 129), (100, 3)):
+        assert need(S, T) > binding.STATIC_SCRATCH_BYTES
+        assert call(8, S, T) == binding.SG_ELIMIT, (S, T)
+    assert need(3, 256) <= binding.STATIC_SCRATCH_BYTES and need(6, 130) <= binding.STATIC_SCRATCH_BYTES < need(6, 131)
+    assert call(8, 6, 131) == binding.SG_ELIMIT
+    msg = lib.sg_strerror(binding.SG_ELIMIT).decode()
+    assert "SG_STATIC_SCRATCH_BYTES" in msg and "split" in msg
+    text = open(os.path.join(ROOT, "include", "sg_b200.h")).read()
+    assert re.search(r"#define\s+SG_STATIC_SCRATCH_BYTES\s+\(16u << 20\)", text) and binding.STATIC_SCRATCH_BYTES == 16 << 20
+
+
 def test_no_cpu_fallback():
     """Without a CUDA device the product path must fail loudly, not compute on the host."""
     import torch
