@@ -333,7 +333,15 @@ double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c);
  *                     (sample, group of 32 copies) held in the shared memory of thread-block clusters (SG_TUNE_CLUSTER_CTAS: 4 CTAs
  *                     holding 4 planes of 16 copies each, or 8 CTAs holding 2 planes of 32 copies); the x3 neighbours across a
  *                     cut are read from the neighbouring CTA's shared memory.
- * All kernels perform the same arithmetic in the same order: the spins do not depend on the choice.
+ * All kernels perform the same arithmetic in the same order: the spins do not depend on the choice.  The ENERGIES do, in the
+ * last bits: each kernel sums its per-CTA partials of E in its own fixed order (they agree to ~1e-7 * N relative to |E|), and E
+ * feeds the PT acceptance.  SG_SWEEP_AUTO looks at the LOCAL shape (the cluster kernel needs n_samples * copy groups >= 15 in this
+ * context; SG_TUNE_ZCHUNK = 0 picks the chunk from the local grid), so the same job split over ranks by sample, replica or slot
+ * may run another kernel per shard than the single context would, and a PT decision whose random number falls within that
+ * rounding of the threshold can then differ.  A shard reproduces the single-context chain BIT FOR BIT only when both pin
+ * SG_TUNE_SWEEP_IMPL (SG_SWEEP_ZMARCH or SG_SWEEP_TILED) and SG_TUNE_ZCHUNK to the same explicit values; left on AUTO the two
+ * chains are equally valid samples of the same Markov chain but not guaranteed identical.
+ * sg_sweep_impl_used reports which kernel served the last sg_sweep_or / sg_sweep_hb call (below).
  * SG_TUNE_ZCHUNK: planes per CTA of the z-marching kernel; 0 = automatic, else even, >= 4 and a divisor of L.
  * SG_TUNE_RES_COPIES: copies per CTA of the resident kernel: 0 = automatic, else 4, 8, 16 or 32 (SG_EINVAL if the lattice
  *   of that many copies does not fit in shared memory).
@@ -344,7 +352,11 @@ double sg_walk_tau_int(const int32_t* series, int64_t n, double window_c);
  *   SG_MEASURE_AUTO    the streaming row kernel (thread = (lattice row, temperature), every replica's spin loaded once for
  *                      all pairs) when 2 <= R <= 4, else the staged kernel (default)
  *   SG_MEASURE_STAGED  the staged kernel (sites of all copies through shared memory; any R)
- *   Same products, fp32 row sums in the streaming kernel: results agree to ~1e-8.
+ *   Same fp32 products.  The staged kernel adds them in fp64 from the single site on; the streaming kernel adds the L sites of a
+ *   lattice row (and their x1 phases, rounded to fp32) in fp32 and goes on in fp64.  |difference of any q^| <= L * 2^-24 in the worst
+ *   case (every rounding of every row in the same direction: 3.8e-6 at L = 64), ~1e-8 in practice (roundings of different rows are
+ *   independent); the tests hold it to 2e-7 absolute at cfg 4's full size, for random copies and for identical copies (q^(0) = 1, the
+ *   coherent worst case), and both kernels to 1e-6 against the oracle.
  * SG_TUNE_CLUSTER_CTAS: shape of the cluster-resident kernel (L = 16): 4 (default) = clusters of 4 CTAs, each holding 4 planes of
  *   16 copies (two clusters per copy group); 8 = clusters of 8 CTAs, each holding 2 planes of all 32 copies.  Same spins.
  * SG_TUNE_GRAPH: 1 (default) = sg_run_units captures one unit in a CUDA graph and replays it (the sweep counters patched in
@@ -356,8 +368,18 @@ enum { SG_SWEEP_AUTO = 0, SG_SWEEP_TILED = 1, SG_SWEEP_ZMARCH = 2, SG_SWEEP_RESI
 int sg_tune(sg_ctx* ctx, int knob, int value);
 
 /* ---- utilities ---- */
+/* Which kernel served the last sg_sweep_or (kind = SG_KIND_OR) or sg_sweep_hb (SG_KIND_HB) call, sg_run_units included: one of
+ * SG_SWEEP_TILED / ZMARCH / RESIDENT / FUSED / CLUSTER; 0 (SG_SWEEP_AUTO) before the first such call; SG_EINVAL for a NULL context
+ * or another kind.  cluster_fallback_cuda (may be NULL) receives the cudaError_t of the cluster launch that made the automatic
+ * choice give up k_sweep_cres in this context (that sweep call itself went on with the z-marching kernel and returned SG_OK;
+ * sg_last_cuda_error is not set by it), 0 if that never happened.  The automatic choice tries the cluster kernel again after
+ * the next sg_tune(SG_TUNE_SWEEP_IMPL / SG_TUNE_CLUSTER_CTAS, ...).  Host book-keeping only: no device work. */
+int sg_sweep_impl_used(const sg_ctx* ctx, int kind, int* cluster_fallback_cuda);
 int sg_sync(sg_ctx* ctx);                       /* cudaStreamSynchronize on the context's stream        */
 uint64_t sg_kernel_launches(const sg_ctx* ctx); /* kernels launched by this context so far              */
+uint64_t sg_graph_replays(const sg_ctx* ctx);   /* units sg_run_units issued as replays of a captured CUDA graph so far (0 when
+                                                   every unit was issued launch by launch: SG_TUNE_GRAPH off, fewer than 8 units,
+                                                   a lattice the resident kernel does not serve, or a capture that failed)   */
 int sg_last_cuda_error(const sg_ctx* ctx);      /* cudaError_t of the last failed CUDA call, 0 if none  */
 const char* sg_strerror(int code);              /* static string for an SG_* code                       */
 /* Philox4x32-10 block on the host (the library's own implementation; known-answer tests). */

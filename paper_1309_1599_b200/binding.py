@@ -24,7 +24,7 @@ DECLARED_SYMBOLS = [
     "sg_workspace_bytes", "sg_create", "sg_destroy", "sg_init_sample", "sg_init_sample_bimodal", "sg_sweep_or", "sg_sweep_hb",
     "sg_pt_swap", "sg_pt_publish", "sg_pt_swap_gathered", "sg_energy_by_temp", "sg_run_units", "sg_measure", "sg_accumulate", "sg_get_logbins", "sg_export_replica", "sg_measure_cross", "sg_export_chirality", "sg_chiral_cross", "sg_chiral_cross_static", "sg_measure_chiral", "sg_schwinger_dyson", "sg_correlation_length", "sg_get_spins", "sg_set_spins", "sg_get_couplings", "sg_get_perm",
     "sg_set_perm", "sg_get_energies", "sg_set_energies", "sg_get_counters", "sg_set_counters",
-    "sg_halfsweep", "sg_pt_stats", "sg_pt_walk", "sg_pt_visits", "sg_walk_tau_int", "sg_tune", "sg_sync", "sg_kernel_launches", "sg_last_cuda_error", "sg_strerror",
+    "sg_halfsweep", "sg_pt_stats", "sg_pt_walk", "sg_pt_visits", "sg_walk_tau_int", "sg_tune", "sg_sweep_impl_used", "sg_sync", "sg_kernel_launches", "sg_graph_replays", "sg_last_cuda_error", "sg_strerror",
     "sg_philox4x32_10",
 ]
 
@@ -50,7 +50,7 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
-    path = os.environ.get("SG_B200_LIB", _LIB_PATH)      # another build of the same library (e.g. a measurement variant)
+    path = _LIB_PATH
     if not os.path.exists(path):
         raise ImportError("libsg_b200.so is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
                           "(there is no CPU fallback)")
@@ -96,8 +96,10 @@ def load_library():
     L.sg_chiral_cross_static.argtypes = [i, i, i, vp, vp, vp, vp, ctypes.POINTER(i)]; L.sg_chiral_cross_static.restype = i
     L.sg_pt_walk.argtypes = [vp, vp, vp]; L.sg_pt_walk.restype = i
     L.sg_tune.argtypes = [vp, i, i]; L.sg_tune.restype = i
+    L.sg_sweep_impl_used.argtypes = [vp, i, ctypes.POINTER(i)]; L.sg_sweep_impl_used.restype = i
     L.sg_sync.argtypes = [vp]; L.sg_sync.restype = i
     L.sg_kernel_launches.argtypes = [vp]; L.sg_kernel_launches.restype = u64
+    L.sg_graph_replays.argtypes = [vp]; L.sg_graph_replays.restype = u64
     L.sg_last_cuda_error.argtypes = [vp]; L.sg_last_cuda_error.restype = i
     L.sg_strerror.argtypes = [i]; L.sg_strerror.restype = ctypes.c_char_p
     L.sg_philox4x32_10.argtypes = [ctypes.POINTER(ctypes.c_uint32)] * 3; L.sg_philox4x32_10.restype = None
@@ -415,8 +417,21 @@ class SpinGlass:
     def tune(self, knob, value):
         self._check(self._lib.sg_tune(self._ctx, int(knob), int(value)), "sg_tune")
 
+    def sweep_impl_used(self, kind=KIND_OR):
+        """(SWEEP_* constant of the kernel that served the last sweep_or / sweep_hb call, cudaError of the cluster launch that
+        made the automatic choice fall back, 0 if none)."""
+        err = ctypes.c_int(0)
+        rc = self._lib.sg_sweep_impl_used(self._ctx, int(kind), ctypes.byref(err))
+        if rc < 0:
+            raise SgError(rc, "sg_sweep_impl_used")
+        return int(rc), int(err.value)
+
     def sync(self):
         self._check(self._lib.sg_sync(self._ctx), "sg_sync")
 
     def kernel_launches(self):
         return int(self._lib.sg_kernel_launches(self._ctx))
+
+    def graph_replays(self):
+        """Units run_units has issued as CUDA-graph replays so far."""
+        return int(self._lib.sg_graph_replays(self._ctx))

@@ -49,7 +49,10 @@ struct sg_ctx {
     uint32_t fz_attr_set = 0;   // the same for k_sweep_fz
     uint32_t cres_attr_set = 0; // and for k_sweep_cres
     int cres_cs = 4;                 // SG_TUNE_CLUSTER_CTAS: CTAs per cluster of k_sweep_cres (4: half groups, 4 planes each; 8: whole groups, 2 planes)
-    bool cres_unavailable = false;   // a cluster launch failed on this device: the automatic choice stops using it
+    bool cres_unavailable = false;   // a cluster launch failed on this device: the automatic choice stops using it (until the next sg_tune of the sweep kernel)
+    int cres_fail_cuda = 0;          // the cudaError_t of that launch (sg_sweep_impl_used reports it; last_cuda is cleared: the call succeeded)
+    uint64_t graph_replays = 0;      // units issued by sg_run_units as replays of a captured CUDA graph (sg_graph_replays)
+    int served_impl[2] = { 0, 0 };   // SG_SWEEP_* of the kernel that served the last sg_sweep_or [0] / sg_sweep_hb [1] (0: none yet)
     int fz_ZC, fz_nzc;          // chunking of the colour-fused sweep   // template instances of k_sweep_zm whose shared-memory attribute this context has set on its device
     // measure geometry
     int nchunk, chunk_sites, MS;
@@ -678,20 +681,27 @@ int sweeps(sg_ctx* ctx, int kind, int n_sweeps)
 {
     if (!ctx || n_sweeps < 0) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
-    if (n_sweeps > 0 && use_resident(ctx)) return sweeps_resident(ctx, kind, n_sweeps);
-    if (n_sweeps > 0 && use_cluster(ctx, kind)) {
+    if (n_sweeps == 0) return SG_OK;
+    int& served = ctx->served_impl[kind == KIND_HB ? 1 : 0];
+    if (use_resident(ctx)) { served = SG_SWEEP_RESIDENT; return sweeps_resident(ctx, kind, n_sweeps); }
+    if (use_cluster(ctx, kind)) {
         const int rc = sweeps_cluster(ctx, kind, n_sweeps);
         // the automatic choice falls back to the z-marching kernel where 8-CTA clusters of 192 KB cannot be launched
         // (the launch call itself fails: nothing ran); an explicit request reports the error
+        if (rc == SG_OK) served = SG_SWEEP_CLUSTER;
         if (rc == SG_OK || ctx->sweep_impl == SG_SWEEP_CLUSTER || ctx->capturing) return rc;
         cudaGetLastError();
         ctx->cres_unavailable = true;
+        ctx->cres_fail_cuda = ctx->last_cuda;     // kept for sg_sweep_impl_used; this call goes on and succeeds,
+        ctx->last_cuda = 0;                       // so sg_last_cuda_error must not report a failure for it
     }
     if (kind == KIND_OR && ctx->sweep_impl == SG_SWEEP_FUSED && ctx->fz_ZC > 0 && !use_packed(ctx)) {
+        served = SG_SWEEP_FUSED;
         for (int k = 0; k < n_sweeps; ++k)
             if (int rc = sweep_fused(ctx, k == n_sweeps - 1)) return rc;
         return SG_OK;
     }
+    served = (ctx->zm_ok && ctx->sweep_impl != SG_SWEEP_TILED) ? SG_SWEEP_ZMARCH : SG_SWEEP_TILED;
     for (int k = 0; k < n_sweeps; ++k) {
         if (int rc = half_sweep(ctx, kind, 0, false)) return rc;
         if (int rc = half_sweep(ctx, kind, 1, k == n_sweeps - 1)) return rc;
@@ -1096,6 +1106,7 @@ static int one_unit(sg_ctx* ctx, int n_or)
 {
     if (n_or > 0 && use_resident(ctx)) {              // small lattices: the unit's sweeps in one launch
         if (int rc = all_inited(ctx)) return rc;
+        ctx->served_impl[0] = ctx->served_impl[1] = SG_SWEEP_RESIDENT;
         if (int rc = sweeps_resident_unit(ctx, 1, n_or)) return rc;
         return sg_pt_swap(ctx);
     }
@@ -1160,7 +1171,7 @@ static int replay_units(sg_ctx* ctx, int n_units, int n_or, bool* done)
             if (rc != SG_OK) break;
             const cudaError_t e = cudaGraphLaunch(exec, cap);
             if (e != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
-            ctx->hb_counter += 1; ctx->pt_counter += 1; ctx->launches += per_unit;
+            ctx->hb_counter += 1; ctx->pt_counter += 1; ctx->launches += per_unit; ctx->graph_replays += 1;
         }
         ctx->energies_fresh = true;
         *done = (rc == SG_OK);
@@ -1566,6 +1577,7 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
         if (value == SG_SWEEP_CLUSTER && ctx->L != CresGeom::L) return SG_EINVAL;
         if (value == SG_SWEEP_RESIDENT && !ctx->res_ok) return SG_EINVAL;
         ctx->sweep_impl = value;
+        ctx->cres_unavailable = false;      // a fresh choice re-arms the automatic use of the cluster kernel
         return SG_OK;
     case SG_TUNE_RES_COPIES:
         if (value != 0 && value != 4 && value != 8 && value != 16 && value != 32) return SG_EINVAL;
@@ -1584,6 +1596,7 @@ int sg_tune(sg_ctx* ctx, int knob, int value)
     case SG_TUNE_CLUSTER_CTAS:
         if (value != 4 && value != 8) return SG_EINVAL;
         ctx->cres_cs = value;
+        ctx->cres_unavailable = false;      // the other cluster shape may launch where this one did not
         return SG_OK;
     case SG_TUNE_GRAPH:
         if (value != 0 && value != 1) return SG_EINVAL;
@@ -1608,7 +1621,15 @@ int sg_sync(sg_ctx* ctx)
     return SG_OK;
 }
 
+int sg_sweep_impl_used(const sg_ctx* ctx, int kind, int* cluster_fallback_cuda)
+{
+    if (!ctx || (kind != SG_KIND_OR && kind != SG_KIND_HB)) return SG_EINVAL;
+    if (cluster_fallback_cuda) *cluster_fallback_cuda = ctx->cres_unavailable ? ctx->cres_fail_cuda : 0;
+    return ctx->served_impl[kind == SG_KIND_HB ? 1 : 0];
+}
+
 uint64_t sg_kernel_launches(const sg_ctx* ctx) { return ctx ? ctx->launches : 0; }
+uint64_t sg_graph_replays(const sg_ctx* ctx) { return ctx ? ctx->graph_replays : 0; }
 int sg_last_cuda_error(const sg_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
 
 }  // extern "C"

@@ -4,7 +4,9 @@ and the north star's covariance checks (3) and (4) on the CUDA path itself:
 
     cfg 1  L =  8, 8 samples, 4 x 16 copies (C =  64, 2 copy groups)                  resident multi-sweep kernel
            + its isotropic rerun (sigma_D = 0): global O(3) covariance of the OR sweep, invariance of e and q
-    cfg 2  L = 16, 32 samples, 4 x 24 copies (C =  96, 3 copy groups)                 z-marching kernel, 2 chunks
+    cfg 2  L = 16, 32 samples, 4 x 24 copies (C =  96, 3 copy groups)                 OR sweeps: cluster-resident kernel (the full-
+           sweep pass holds 5 samples = 15 copy groups, the least the automatic choice takes it for); heat bath and
+           sg_halfsweep: z-marching kernel, 2 chunks
     cfg 3  L = 32, 16 samples, 4 x 32 copies (C = 128, 4 copy groups), sigma_D = sqrt 2  z-marching kernel
 
 Element by element against the oracle on the same seeded inputs (oracle -> CUDA only), tolerances of the north star
@@ -34,7 +36,11 @@ def sg():
 
 
 # (config index, samples used for the element-by-element pass, samples for the full-sweep pass)
-CASES = [(1, 8, 8), (2, 32, 4), (3, 2, 1)]
+CASES = [(1, 8, 8), (2, 32, 5), (3, 2, 1)]
+# the kernel the library's automatic choice must have taken for the sweep call, per (config, kind): asserted, so that a change
+# of the dispatch cannot silently move a configuration's oracle comparison onto another kernel
+SERVED_BY = {(1, 0): "SWEEP_RESIDENT", (1, 1): "SWEEP_RESIDENT", (2, 0): "SWEEP_CLUSTER", (2, 1): "SWEEP_ZMARCH",
+             (3, 0): "SWEEP_ZMARCH", (3, 1): "SWEEP_ZMARCH"}
 
 
 @pytest.mark.parametrize("k,S,S_sweep", CASES)
@@ -60,12 +66,14 @@ def test_half_sweeps_at_config_shape(sg, oracle, k, S, S_sweep, kind):
 @pytest.mark.parametrize("k,S,S_sweep", CASES)
 @pytest.mark.parametrize("kind", [0, 1])
 def test_full_sweep_energy_and_measure_at_config_shape(sg, oracle, k, S, S_sweep, kind):
-    """The product's sweep call (for cfg 1 the resident kernel, else two z-marching launches + fused energy), then the
-    measurement through a random temperature assignment."""
+    """The product's sweep call through the automatic kernel choice (cfg 1: the resident kernel; cfg 2: the cluster-resident
+    kernel for OR, two z-marching launches for the heat bath; cfg 3: z-marching; energies fused), then the measurement through
+    a random temperature assignment."""
     cfg = W.CONFIGS[k]
     L, R, T, N = cfg.L, cfg.n_replicas, cfg.n_temps, cfg.n_sites
     sim, gpu = make_pair(oracle, sg, L, S_sweep, R, T, cfg.betas, seed=cfg.seed, sigma_D=cfg.sigma_D, first_sample=1)
     sweep_both(sim, gpu, kind, L)
+    assert gpu.sweep_impl_used(kind) == (getattr(sg, SERVED_BY[(k, kind)]), 0)
     e_gpu, e_ref = gpu.get_energies() / N, sim.energies() / N
     assert np.all(np.abs(e_gpu - e_ref) <= 1e-6 * np.maximum(1.0, np.abs(e_ref)))
     rng = np.random.default_rng(40 + k)
