@@ -185,3 +185,31 @@ def test_two_rank_gloo_temperature_slot_sharding():
     assert multi.slot_window_of_rank(1, 3, 12) == (4, 4)
     with pytest.raises(ValueError):
         multi.slot_window_of_rank(0, 4, 6)
+
+
+def test_bench_gpus_n_starts_n_ranks_and_prints_one_line():
+    """`python bench.py --gpus 2` outside torchrun must start two ranks itself (the command the round driver
+    runs for the scaling record): --check-launch drives exactly that path -- re-exec under torch.distributed.run, rendezvous on
+    127.0.0.1, an all-reduce over the ranks (gloo here, nccl on a GPU box), ONE JSON line from rank 0 -- without the workload.
+    Without the devices the workload itself must refuse to start rather than run fewer ranks than asked for."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    env["CUDA_VISIBLE_DEVICES"] = ""                       # gloo ranks also on a box that has GPUs
+    run = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--check-launch"], env=env,
+                         capture_output=True, text=True, timeout=300)
+    assert run.returncode == 0, run.stderr[-2000:]
+    lines = [l for l in run.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, run.stdout
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["asked"] == 2 and out["backend"] == "gloo" and out["rank_sum"] == out["rank_sum_expected"] == 1.0
+    run = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "1"], env=env,
+                         capture_output=True, text=True, timeout=300)
+    assert run.returncode != 0 and "refusing to run fewer ranks" in run.stderr and not run.stdout.strip()
+    sys.path.insert(0, root)
+    import bench
+    cmd = bench.spawn_command(4, ["--gpus", "4", "--steps", "3"], 29512)
+    assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node" in cmd and cmd[cmd.index("--nproc-per-node") + 1] == "4"
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[-4:] == ["--gpus", "4", "--steps", "3"]
