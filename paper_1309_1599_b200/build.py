@@ -28,16 +28,6 @@ def build(force=False, verbose=False):
     return LIB
 
 
-def build_whatif(n, out, defines=()):
-    """A measurement-only variant of the library (csrc/sg_sweep_zm.cuh, SG_WHATIF): wrong spins by design, never the product."""
-    subprocess.check_call([nvcc()] + NVCC_FLAGS + ["-DSG_WHATIF=%d" % int(n)] + ["-D" + d for d in defines] + ["-o", out] + SOURCES)
-    return out
-
-
 if __name__ == "__main__":
     import sys
-    if "--whatif" in sys.argv:
-        defs = [sys.argv[k + 1] for k, a in enumerate(sys.argv) if a == "--define"]
-        print(build_whatif(int(sys.argv[sys.argv.index("--whatif") + 1]), sys.argv[sys.argv.index("--out") + 1], defs))
-    else:
-        print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv))

@@ -57,24 +57,16 @@ __device__ __forceinline__ uint32_t copy_gid(uint32_t gbase, int c, int Tl, int 
     return gbase + (uint32_t)c + (Tpad ? (uint32_t)((c / Tl) * Tpad) : 0u);
 }
 
-// h[j] += c * n[j] for the four copies a thread holds: the inner step of every field computation.  SG_FFMA2 = 1 (default): two
-// FFMA2 (fma.rn.f32x2 with the coupling as its scalar operand) instead of four FFMA -- the same four fp32 FMAs with round to
-// nearest, bit for bit, in half the issue slots (measured on the power-capped cfg-4 loop: OR half-sweep 659.5 -> 649.6 us, heat
-// bath -4.4 %).  SG_FFMA2 = 0 keeps the scalar form for A/B builds.
-#ifndef SG_FFMA2
-#define SG_FFMA2 1
-#endif
+// h[j] += c * n[j] for the four copies a thread holds: the inner step of every field computation.  Two FFMA2 (fma.rn.f32x2 with
+// the coupling as its scalar operand) instead of four FFMA -- the same four fp32 FMAs with round to nearest, bit for bit, in half
+// the issue slots (measured on the power-capped cfg-4 loop against the scalar form: OR half-sweep 659.5 -> 649.6 us, heat bath
+// -4.4 %; profiles/r2e_whatif.md, profiles/r2_sass_histogram.md).
 __device__ __forceinline__ void fma4(float c, const float (&n)[4], float (&h)[4])
 {
-#if SG_FFMA2
     const float2 cc = make_float2(c, c);
     const float2 lo = __ffma2_rn(cc, make_float2(n[0], n[1]), make_float2(h[0], h[1]));
     const float2 hi = __ffma2_rn(cc, make_float2(n[2], n[3]), make_float2(h[2], h[3]));
     h[0] = lo.x; h[1] = lo.y; h[2] = hi.x; h[3] = hi.y;
-#else
-#pragma unroll
-    for (int j = 0; j < 4; ++j) h[j] = fmaf(c, n[j], h[j]);
-#endif
 }
 
 // r = ((w >> 9) + 1/2) 2^-23: exact in fp32

@@ -15,13 +15,6 @@
 #pragma once
 #include "sg_device.cuh"
 
-// SG_WHATIF (default 0 = the product): compile-time variants of k_sweep_zm that drop one resource each and compute WRONG spins.
-// They exist to measure what the power-capped half-sweep is sensitive to (profiles/r2e_whatif.md): built into a separate library
-// by `python paper_1309_1599_b200/build.py --whatif N --out PATH` and loaded through SG_B200_LIB; never part of libsg_b200.so.
-#ifndef SG_WHATIF
-#define SG_WHATIF 0
-#endif
-
 namespace sg {
 
 enum : int { KIND_OR = 0, KIND_HB = 1, KIND_ENERGY = 2 };
@@ -352,30 +345,19 @@ __global__ void __launch_bounds__(ZmGeom<TX, TY>::THREADS, 2) k_sweep_zm(const Z
 #pragma unroll
                 for (int j = 0; j < 4; ++j) hf[a][j] = 0.f;
             float J[JG];
-#if SG_WHATIF == 1          // measurement only: no coupling loads
-#pragma unroll
-            for (int v = 0; v < JG; ++v) J[v] = __int_as_float(0x3f800000 + v * 4096 + (k & 1));
-            (void)Jp;
-#else
 #pragma unroll
             for (int v = 0; v < JG / 4; ++v) {
                 const float4 t4 = lds4(Jp + 16 * v);
                 J[4 * v] = t4.x; J[4 * v + 1] = t4.y; J[4 * v + 2] = t4.z; J[4 * v + 3] = t4.w;
             }
-#endif
 #pragma unroll
-            for (int nbk = 0; nbk < (SG_WHATIF == 2 ? 3 : 6); ++nbk) {      // SG_WHATIF 2, measurement only: half the neighbours (loads and FFMAs)
+            for (int nbk = 0; nbk < 6; ++nbk) {
                 float n[3][4];
-#if SG_WHATIF == 3          // measurement only: no neighbour loads, all FFMAs (operands from the prefetched own spin)
-#pragma unroll
-                for (int bb = 0; bb < 3; ++bb) { n[bb][0] = pre[d][bb].x + (float)nbk; n[bb][1] = pre[d][bb].y; n[bb][2] = pre[d][bb].z; n[bb][3] = pre[d][bb].w; }
-#else
 #pragma unroll
                 for (int bb = 0; bb < 3; ++bb) {
                     const float4 t4 = lds4(nbp[nbk] + bb * (G * 4));
                     n[bb][0] = t4.x; n[bb][1] = t4.y; n[bb][2] = t4.z; n[bb][3] = t4.w;
                 }
-#endif
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
