@@ -148,6 +148,27 @@ def test_pt_and_measure_at_full_size(full, oracle):
         assert np.abs(qk[s, p, t].reshape(-1) - o[1:]).max() <= 1e-6
     for s, r, t in [(0, 0, 0), (3, 3, 47), (1, 2, 20)]:
         assert abs(e[s, r, t] - E[s, r * T + sot[s, r, t]] / N) <= 1e-12 * abs(E).max()
+    # The default overlap kernel at R = 4 (k_measure_rows: fp32 sums over the 64 sites of a lattice row, fp64 from there on)
+    # against the staged kernel (fp64 from the single site on) at full size; bound stated in include/sg_b200.h (SG_TUNE_MEASURE_IMPL)
+    # and DESIGN.md section 6: 2e-7 absolute.  Random copies first (q ~ 0), then the coherent worst case: every copy of sample 0 set to
+    # the same configuration, so that all 64 terms of every row sum are +1 and q^(0) = 1, q^(k_min) = 0 for every pair and temperature.
+    sg = full["sg"]
+    def both_kernels():
+        gpu.tune(sg.TUNE_MEASURE_IMPL, sg.MEASURE_STAGED)
+        staged = gpu.measure()
+        gpu.tune(sg.TUNE_MEASURE_IMPL, sg.MEASURE_AUTO)
+        return gpu.measure(), staged
+    (_, q0_r, qk_r), (_, q0_s, qk_s) = both_kernels()
+    assert np.array_equal(q0_r, q0) and np.array_equal(qk_r, qk)                    # what was compared with the oracle above was the row kernel
+    d_random = max(np.abs(q0_r - q0_s).max(), np.abs(qk_r - qk_s).max())
+    gpu.set_spins(0, np.broadcast_to(full["X"][0][5], full["X"][0].shape).copy())
+    (_, q0_r, qk_r), (_, q0_s, qk_s) = both_kernels()
+    d_ordered = max(np.abs(q0_r - q0_s).max(), np.abs(qk_r - qk_s).max())
+    print("MEASURE-ROWS-MARGIN cfg 4: rows vs staged max |dq| = %.2e (random copies), %.2e (identical copies); bar 2e-7" % (d_random, d_ordered))
+    assert d_random <= 2e-7 and d_ordered <= 2e-7
+    for q0_x, qk_x in ((q0_r, qk_r), (q0_s, qk_s)):
+        assert np.abs(q0_x[0] - 1.0).max() <= 1e-6 and np.abs(qk_x[0]).max() <= 1e-6       # |s|^2 = 1 to fp32 rounding; sum of the phases = 0
+    reset(full)
 
 
 def test_fused_and_cluster_kernels_stay_bit_identical_over_many_sweeps():

@@ -10,12 +10,16 @@ comparison within max |z| < 4 and chi^2/n consistent with 1 (n = 12 comparisons 
 north star's 3 sigma is a per-comparison statement, P(|z| > 3) = 2.7e-3, so over n comparisons the family-wise
 bar at the same confidence is |z| < 4).  The observed max |z| and chi^2/n are printed (pytest -s / -rP shows them)
 and recorded in DESIGN.md section 6.  Seeds are fixed, both chains are deterministic."""
+import warnings
+
 import numpy as np
 import pytest
 
 import sg_workloads as W
 
 pytestmark = pytest.mark.gpu
+
+FAMILY = {}        # test name -> z values of its comparisons (the family-wise bar is taken over all of them, last test of the file)
 
 
 @pytest.fixture(scope="module")
@@ -52,7 +56,7 @@ def run_chain(chain, n_units, n_or, measure_every=1):
     return [np.array(a) for a in out]
 
 
-def compare(obs_gpu, obs_ref, names, n_bins):
+def compare(obs_gpu, obs_ref, names, n_bins, family_key):
     zs = []
     for g, r, name in zip(obs_gpu, obs_ref, names):
         mg, sg_ = bin_mean_err(g, n_bins)
@@ -62,8 +66,11 @@ def compare(obs_gpu, obs_ref, names, n_bins):
         zs.append(z.reshape(-1))
     z = np.concatenate(zs)
     chi2 = float((z ** 2).mean())
-    print("STATS-MARGIN %s: n = %d comparisons, max |z| = %.3f (bar 4), chi^2/n = %.3f (bar %.3f), fraction |z| > 3: %.3f"
-          % ("+".join(names), z.size, np.abs(z).max(), chi2, 1.1 + 4.0 * np.sqrt(2.0 / z.size), np.mean(np.abs(z) > 3)))
+    msg = ("STATS-MARGIN %s %s: n = %d comparisons, max |z| = %.3f (bar 4), chi^2/n = %.3f (bar %.3f), fraction |z| > 3: %.3f"
+           % (family_key, "+".join(names), z.size, np.abs(z).max(), chi2, 1.1 + 4.0 * np.sqrt(2.0 / z.size), np.mean(np.abs(z) > 3)))
+    print(msg)
+    warnings.warn(msg)          # pytest's warnings summary keeps the line in a plain `pytest -q` log (DESIGN.md section 6 quotes it)
+    FAMILY[family_key] = z
     assert np.abs(z).max() < 4.0, ("max |z|", np.abs(z).max(), "chi2/n", chi2, z)
     assert chi2 < 1.1 + 4.0 * np.sqrt(2.0 / z.size), ("chi2/n", chi2, z.size, "max |z|", np.abs(z).max())
     return z
@@ -89,7 +96,7 @@ def test_cfg0_thermal_averages_within_errors(sg, oracle):
     sim, gpu = make_chains(oracle, sg, cfg, K)
     ref = run_chain(sim, n_units, cfg.n_or)
     got = run_chain(gpu, n_units, cfg.n_or)
-    compare(got, ref, ("e", "q0^2", "|qk|^2"), n_bins=5)
+    compare(got, ref, ("e", "q0^2", "|qk|^2"), n_bins=5, family_key="cfg0")
     # PT: the same number of attempts; acceptance rates of the two sides agree
     att_g, acc_g = gpu.pt_stats()
     assert np.array_equal(att_g, sim.attempts)
@@ -107,4 +114,20 @@ def test_cfg1_thermal_averages_within_errors(sg, oracle):
     sim, gpu = make_chains(oracle, sg, cfg, K)
     ref = run_chain(sim, n_units, cfg.n_or, measure_every=4)
     got = run_chain(gpu, n_units, cfg.n_or, measure_every=4)
-    compare(got[:2], ref[:2], ("e", "q0^2"), n_bins=5)
+    compare(got, ref, ("e", "q0^2", "|qk|^2"), n_bins=5, family_key="cfg1")
+
+
+def test_family_of_all_comparisons():
+    """SURVEY.md section 8(c) as written: `max |z| < 4` is the bar for a family of MORE THAN 50 comparisons (the north star's 3 sigma
+    is a per-comparison statement).  The two tests above make 12 + 48 = 60; this one takes the bar over all of them together
+    and checks the per-comparison statement in the form it can be checked: no more than 2 of the 60 beyond 3 sigma
+    (expected 0.16; P(>= 3) = 6e-4 for a correct code)."""
+    if set(FAMILY) != {"cfg0", "cfg1"}:
+        pytest.skip("needs both chains of this file (run the whole file)")
+    z = np.concatenate([FAMILY["cfg0"], FAMILY["cfg1"]])
+    msg = "STATS-MARGIN family: n = %d comparisons, max |z| = %.3f (bar 4), |z| > 3: %d (bar 2), chi^2/n = %.3f" % (
+        z.size, np.abs(z).max(), int(np.sum(np.abs(z) > 3)), float((z ** 2).mean()))
+    print(msg)
+    warnings.warn(msg)
+    assert z.size > 50
+    assert np.abs(z).max() < 4.0 and np.sum(np.abs(z) > 3) <= 2, msg
