@@ -65,8 +65,9 @@ typedef struct {
                                   keyed by the global copy id); it keeps the WHOLE temperature assignment of its chains, and
                                   the PT step is sg_pt_publish -> all-gather of the energies -> sg_pt_swap_gathered, the same
                                   decisions on every shard (identical Philox counters).  sg_pt_swap, sg_run_units, sg_measure,
-                                  sg_accumulate, sg_measure_chiral, sg_schwinger_dyson, sg_export_chirality return SG_EINVAL in
-                                  such a context; overlaps go through sg_export_replica / sg_measure_cross */
+                                  sg_accumulate, sg_measure_chiral, sg_schwinger_dyson return SG_EINVAL in such a context;
+                                  overlaps go through sg_export_replica / sg_measure_cross, chiral-glass overlaps through
+                                  sg_export_chirality / sg_chiral_cross */
 } sg_shape;
 
 enum {
@@ -208,6 +209,12 @@ int sg_measure_cross(sg_ctx* ctx, int r, const void* dev_remote, double* q0, dou
  * ordered by temperature, float [S][3][N][T] (mu, site, temperature; temperature fastest) to the device buffer dev_out
  * (asynchronous); sg_chiral_cross forms kappa = zeta^a zeta^b between two such device buffers (one local, one the partner's):
  * qc0 double [S][T][3], qck double [S][T][3][3][2] as in sg_measure_chiral, host outputs, either may be NULL; synchronises.
+ * In a context sharded by temperature slot T is n_temps_total throughout: sg_export_chirality writes zeta for the temperatures
+ * whose configuration the shard holds and ZEROS for the others, so the element-wise sum of the shards' buffers (an all-reduce)
+ * is the replica ordered by temperature; sg_chiral_cross of a shard's own (zero-padded) export of replica a with the summed
+ * buffer of replica b gives the overlaps at the shard's temperatures and exact zeros elsewhere, and the sum of these over
+ * the shards completes every temperature (multi.overlaps_sharded(chirality=True); Eq. (2) was measured on exactly the runs the
+ * paper sharded this way).
  * Errors: SG_EINVAL (NULL, r out of range, T > 256), SG_ESTATE, SG_ECUDA. */
 int sg_export_chirality(sg_ctx* ctx, int r, void* dev_out);
 int sg_chiral_cross(sg_ctx* ctx, const void* dev_a, const void* dev_b, double* qc0, double* qck);

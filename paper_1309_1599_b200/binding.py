@@ -394,10 +394,11 @@ class SpinGlass:
         return out
 
     def chiral_cross(self, za, zb):
-        """(qc0 [S][T][3], qck [S][T][3][3][2]) between two export_chirality tensors (both on this device)."""
+        """(qc0 [S][T][3], qck [S][T][3][3][2]) between two export_chirality tensors (both on this device); T = the temperatures of
+        the whole chain (n_temps_total in a slot-sharded context)."""
         for z in (za, zb):
-            assert z.is_cuda and z.is_contiguous() and z.numel() == self.S * 3 * self.N * self.T
-        qc0 = np.empty((self.S, self.T, 3)); qck = np.empty((self.S, self.T, 3, 3, 2))
+            assert z.is_cuda and z.is_contiguous() and z.numel() == self.S * 3 * self.N * self.Tt
+        qc0 = np.empty((self.S, self.Tt, 3)); qck = np.empty((self.S, self.Tt, 3, 3, 2))
         self._check(self._lib.sg_chiral_cross(self._ctx, ctypes.c_void_p(za.data_ptr()), ctypes.c_void_p(zb.data_ptr()), _ptr(qc0), _ptr(qck)),
                     "sg_chiral_cross")
         return qc0, qck

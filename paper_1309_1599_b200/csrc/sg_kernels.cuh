@@ -622,14 +622,23 @@ __global__ void k_reduce_cross(const double* __restrict__ Xpart, double* __restr
 // The chiral-glass counterpart (Eq. (2)): k_export_zeta_by_temp writes zeta_{x,mu} of local replica r ordered by
 // temperature, out[sample][mu][i][t]; k_chiral_cross forms, per temperature, the 21 sums of kappa_{x,mu} = zeta^a zeta^b and
 // kappa e^{i 2 pi x_nu / L} between two such buffers (either may be the partner's).  Same thread mapping as k_overlap_cross.
+// T: temperatures of the chain; Tl, slot0: slots per replica held by this context and the first of them (T, 0 unless the chain is
+// sharded by slot): a temperature whose configuration lives in another shard gets zeros, as in k_export_by_temp, so that the sum
+// of the shards' exports is the replica ordered by temperature.
 __global__ void k_export_zeta_by_temp(const float* __restrict__ spins, const int* __restrict__ slot_of_temp, float* __restrict__ out,
-                                      int L, int N, int NG, int R, int T, int r)
+                                      int L, int N, int NG, int R, int T, int Tl, int slot0, int r)
 {
     const int sample = blockIdx.y;
     const size_t f = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // (site, temperature), temperature fastest
     if (f >= (size_t)N * T) return;
     const int i = (int)(f / T), t = (int)(f - (size_t)i * T);
-    const int c = r * T + slot_of_temp[((size_t)sample * R + r) * T + t];
+    const int slot = slot_of_temp[((size_t)sample * R + r) * T + t] - slot0;
+    if (slot < 0 || slot >= Tl) {
+#pragma unroll
+        for (int mu = 0; mu < 3; ++mu) out[(size_t)sample * 3 * N * T + (size_t)mu * N * T + f] = 0.f;
+        return;
+    }
+    const int c = r * Tl + slot;
     const float* gb = spins + ((size_t)sample * NG + c / G) * N * SITE_FLOATS + (c % G);
     const int Nh = N >> 1;
     const float* c0 = gb + site_slot(i, L, Nh) * SITE_FLOATS;

@@ -160,13 +160,17 @@ def unit_sharded(gpu, n_or, world_size, gathered=None):
     return pt_step_sharded(gpu, world_size, gathered)
 
 
-def overlaps_sharded(gpu, world_size, pairs=None):
+def overlaps_sharded(gpu, world_size, pairs=None, chirality=False):
     """Overlaps of slot-sharded chains.  The two configurations at temperature t of a replica pair (a, b) may live on
     different ranks.  Per replica b: every rank exports the temperatures whose configuration it holds (zeros elsewhere,
     sg_export_replica), an all-reduce (sum) assembles the replica ordered by temperature on every rank, every rank forms the
     overlap with its part of replica a (sg_measure_cross: zero where it does not hold the configuration), and a last
     all-reduce (sum) of the few numbers completes every temperature.  Returns (q0 [S][P][T], qk [S][P][T][3][2]) on every
-    rank, pairs a < b in the order of sg_measure (or the given list).  At measurement time only."""
+    rank, pairs a < b in the order of sg_measure (or the given list).  At measurement time only.
+    chirality=True: the chiral-glass overlaps instead, (qc0 [S][P][T][3], qck [S][P][T][3][3][2]) (Eq. (2); the
+    paper measured them on the runs it sharded by temperature): sg_export_chirality in place of sg_export_replica
+    (zeta of the temperatures a rank holds, zeros elsewhere), sg_chiral_cross between the rank's own zero-padded export of
+    replica a and the all-reduced buffer of replica b, and the same final all-reduce."""
     import numpy as np
     import torch
     import torch.distributed as dist
@@ -175,12 +179,18 @@ def overlaps_sharded(gpu, world_size, pairs=None):
         pairs = [(a, b) for a in range(R) for b in range(a + 1, R)]
     q0s, qks = {}, {}
     with _on_stream(gpu):
+        own = {}
         for b in sorted({b for _, b in pairs}):
-            full = gpu.export_replica(b)
+            full = gpu.export_chirality(b) if chirality else gpu.export_replica(b)
             if world_size > 1:
                 dist.all_reduce(full, op=dist.ReduceOp.SUM)
             for a in [a for a, bb in pairs if bb == b]:
-                q0s[(a, b)], qks[(a, b)] = gpu.measure_cross(a, full)
+                if chirality:
+                    if a not in own:
+                        own[a] = gpu.export_chirality(a)
+                    q0s[(a, b)], qks[(a, b)] = gpu.chiral_cross(own[a], full)
+                else:
+                    q0s[(a, b)], qks[(a, b)] = gpu.measure_cross(a, full)
     q0 = np.stack([q0s[pr] for pr in pairs], axis=1)
     qk = np.stack([qks[pr] for pr in pairs], axis=1)
     if world_size > 1:

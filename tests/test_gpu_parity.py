@@ -627,6 +627,18 @@ def test_temperature_slot_shards_reproduce_the_single_context(sg, L, S, R, T, W,
         assert np.abs(q0_x - q0[:, p]).max() <= 1e-12 and np.abs(qk_x - qk[:, p]).max() <= 1e-12
         # every temperature is held by exactly one shard: the other shards contribute exact zeros
         assert all(((pp[0] == 0) | (pp[0] == q0_x)).all() for pp in parts)
+    # the chiral-glass overlaps across the shards the same way (Eq. (2); measured by the paper on the runs it sharded by
+    # temperature): zero-padded zeta exports, their sum, each shard's own export against it, sum of the shards' results
+    qc0, qck = whole.measure_chiral()
+    for p, (a, b) in enumerate(pairs):
+        full = sum(g.export_chirality(b) for g in shards)
+        parts = [g.chiral_cross(g.export_chirality(a), full) for g in shards]
+        qc0_x = sum(pp[0] for pp in parts); qck_x = sum(pp[1] for pp in parts)
+        assert qc0_x.shape == qc0[:, p].shape
+        assert np.abs(qc0_x - qc0[:, p]).max() <= 1e-12 and np.abs(qck_x - qck[:, p]).max() <= 1e-12
+        assert all(((pp[0] == 0) | (pp[0] == qc0_x)).all() for pp in parts)
+    if L > 2:
+        assert np.abs(qc0).max() > 1e-5
     # one shard alone through the orchestration (world size 1 path of multi.pt_step_sharded on a whole-chain context)
     solo = sg.SpinGlass(L, S, R, T, betas, seed=91, first_sample=2)
     solo.tune(sg.TUNE_SWEEP_IMPL, impl)

@@ -150,6 +150,15 @@ class _FakeSlotShard:
         qk[:, own] = q0[:, own, None, None]
         return q0, qk
 
+    def export_chirality(self, r):
+        return 100.0 * self.export_replica(r)                                 # 100 (1 + r) at the temperatures held, zeros elsewhere
+
+    def chiral_cross(self, za, zb):
+        # product of the two buffers at one site: non-zero only where this shard's own export is (its temperatures)
+        prod = (za[:, :, 0, :] * zb[:, :, 0, :]).numpy()                       # [S][3][Tt]
+        qc0 = np.moveaxis(prod, 1, 2).copy()                                  # [S][Tt][3]
+        return qc0, np.zeros((self.S, self.Tt, 3, 3, 2))
+
 
 def _slot_worker(rank, world, port, out):
     os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
@@ -157,7 +166,8 @@ def _slot_worker(rank, world, port, out):
     shard = _FakeSlotShard(rank, world, 6)
     gathered = multi.unit_sharded(shard, 3, world)
     q0, qk = multi.overlaps_sharded(shard, world)
-    out.put((rank, shard.calls, gathered.tolist(), shard.swapped_with.tolist(), q0.tolist(), qk.shape))
+    qc0, qck = multi.overlaps_sharded(shard, world, chirality=True)
+    out.put((rank, shard.calls, gathered.tolist(), shard.swapped_with.tolist(), q0.tolist(), qk.shape, qc0.tolist(), qck.shape))
     multi.barrier()
     import torch.distributed as dist
     dist.destroy_process_group()
@@ -182,6 +192,8 @@ def test_two_rank_gloo_temperature_slot_sharding():
         assert g[1] == ["hb", "or3", "publish", "swap"]
         assert g[2] == expect and g[3] == expect                 # identical gathered energies on both ranks
         assert g[4] == [[[0.0 + 2.0] * 6]] * 2 and g[5] == (2, 1, 6, 3, 2)   # pair (0, 1): 10*0 + (1 + 1) at all six temperatures
+        # chirality: own zero-padded export of replica 0 (100) x the summed export of replica 1 (200), complete at every temperature
+        assert g[6] == [[[[20000.0] * 3] * 6]] * 2 and g[7] == (2, 1, 6, 3, 3, 2)
     assert multi.slot_window_of_rank(1, 3, 12) == (4, 4)
     with pytest.raises(ValueError):
         multi.slot_window_of_rank(0, 4, 6)
