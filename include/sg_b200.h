@@ -65,7 +65,7 @@ typedef struct {
                                   keyed by the global copy id); it keeps the WHOLE temperature assignment of its chains, and
                                   the PT step is sg_pt_publish -> all-gather of the energies -> sg_pt_swap_gathered, the same
                                   decisions on every shard (identical Philox counters).  sg_pt_swap, sg_run_units, sg_measure,
-                                  sg_accumulate, sg_measure_chiral, sg_schwinger_dyson return SG_EINVAL in such a context;
+                                  sg_accumulate, sg_measure_chiral return SG_EINVAL in such a context; sg_schwinger_dyson reports the held slots;
                                   overlaps go through sg_export_replica / sg_measure_cross, chiral-glass overlaps through
                                   sg_export_chirality / sg_chiral_cross */
 } sg_shape;
@@ -274,7 +274,10 @@ int sg_chiral_cross_static(int L, int n_samples, int n_temps, const void* dev_a,
  *   2 T <s_x.h_x> - <(h_x)^2 - (s_x.h_x)^2> = 0 in equilibrium, "averaged over all the sites in the lattice".
  *   sd double [S][R][T][2]   sd[..][0] = sum_x s_x.h_x / N,  sd[..][1] = sum_x [h_x.h_x - (s_x.h_x)^2] / N
  * of the copy of replica r at temperature t (current configuration; the caller averages over time and forms
- * 2 sd[0]/beta_t - sd[1]).  Host output, required.  fp32 fields, fp64 sums in a fixed order.  Synchronises. */
+ * 2 sd[0]/beta_t - sd[1]).  Host output, required.  fp32 fields, fp64 sums in a fixed order.  Synchronises.
+ * In a context sharded by temperature slot T is n_temps_total and the entries of the temperatures whose configuration another
+ * shard holds are exact zeros: the sum over the shards (an all-reduce of S*R*T*2 doubles, multi.schwinger_dyson_sharded) is the
+ * whole chain's monitor -- the paper's check ran on its temperature-sharded L = 64 runs. */
 int sg_schwinger_dyson(sg_ctx* ctx, double* sd);
 
 /* Second-moment correlation length, Eq. (4) PAPER.md:93-97 (host arithmetic, no device work):

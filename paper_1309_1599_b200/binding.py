@@ -288,7 +288,7 @@ class SpinGlass:
 
     def schwinger_dyson(self):
         """sd [S][R][T][2]: site averages of s.h and of h.h - (s.h)^2 per (replica, temperature), Eq. (A6)."""
-        sd = np.empty((self.S, self.R, self.T, 2))
+        sd = np.empty((self.S, self.R, self.Tt, 2))      # by the chain's temperatures; zeros for those another slot shard holds
         self._check(self._lib.sg_schwinger_dyson(self._ctx, _ptr(sd)), "sg_schwinger_dyson")
         return sd
 

@@ -1421,16 +1421,16 @@ int sg_chiral_cross(sg_ctx* ctx, const void* dev_a, const void* dev_b, double* q
 
 int sg_schwinger_dyson(sg_ctx* ctx, double* sd)
 {
-    if (!ctx || !sd || ctx->Tt != ctx->T) return SG_EINVAL;
+    if (!ctx || !sd) return SG_EINVAL;
     if (int rc = all_inited(ctx)) return rc;
     SdParams p;
     p.spins = ctx->spins; p.Jg = ctx->Jg; p.SDpart = ctx->SDpart;
     p.L = ctx->L; p.N = ctx->N; p.Nh = ctx->Nh; p.NG = ctx->NG; p.ntiles = ctx->ntiles; p.tile_sites = ctx->tile_sites;
     k_sd<<<dim3(ctx->NG * ctx->ntiles, ctx->S, 2), SWEEP_THREADS, 0, ctx->stream>>>(p);
     SG_LAUNCHED(ctx);
-    const int total = ctx->S * ctx->R * ctx->T * 2;
-    k_reduce_sd<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->SDpart, ctx->slot_of_temp, ctx->result, ctx->S, ctx->R, ctx->T,
-                                                              ctx->NG, ctx->ntiles, ctx->N);
+    const int total = ctx->S * ctx->R * ctx->Tt * 2;      // by the temperatures of the whole chain (zeros for those held by other shards)
+    k_reduce_sd<<<(total + 127) / 128, 128, 0, ctx->stream>>>(ctx->SDpart, ctx->slot_of_temp, ctx->result, ctx->S, ctx->R, ctx->Tt, ctx->T,
+                                                              ctx->slot0, ctx->NG, ctx->ntiles, ctx->N);
     SG_LAUNCHED(ctx);
     {
         int rc;

@@ -960,13 +960,17 @@ __global__ void __launch_bounds__(SWEEP_THREADS) k_sd(const SdParams p)
 }
 
 // sd[S][R][T][2] = (sum_x s.h / N, sum_x [h.h - (s.h)^2] / N) of the copy of replica r at temperature t
+// T: temperatures of the chain; Tl, slot0: slots per replica held here and the first of them (T, 0 unless sharded by slot): exact zeros
+// for the temperatures whose configuration lives in another shard, so that the sum over the shards completes every temperature
 __global__ void k_reduce_sd(const double* __restrict__ SDpart, const int* __restrict__ slot_of_temp, double* __restrict__ result,
-                            int S, int R, int T, int NG, int ntiles, int N)
+                            int S, int R, int T, int Tl, int slot0, int NG, int ntiles, int N)
 {
     const int u = blockIdx.x * blockDim.x + threadIdx.x;
     if (u >= S * R * T * 2) return;
     const int k = u & 1, t = (u >> 1) % T, r = (u / (2 * T)) % R, sample = u / (2 * T * R);
-    const int c = r * T + slot_of_temp[((size_t)sample * R + r) * T + t];
+    const int slot = slot_of_temp[((size_t)sample * R + r) * T + t] - slot0;
+    if (slot < 0 || slot >= Tl) { result[u] = 0.0; return; }
+    const int c = r * Tl + slot;
     const int grp = c / G, lane = c % G;
     double acc = 0.0;
     for (int b = 0; b < 2 * ntiles; ++b) acc += SDpart[((((size_t)(sample * NG + grp)) * 2 * ntiles + b) * G + lane) * 2 + k];

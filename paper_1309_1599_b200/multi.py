@@ -203,6 +203,21 @@ def overlaps_sharded(gpu, world_size, pairs=None, chirality=False):
     return q0, qk
 
 
+def schwinger_dyson_sharded(gpu, world_size):
+    """Schwinger-Dyson monitor (Eq. (A6)) of slot-sharded chains: every rank reduces the two site averages of
+    the configurations it holds (sg_schwinger_dyson: indexed by temperature, exact zeros elsewhere) and one all-reduce (sum) of
+    S*R*T*2 doubles completes every temperature on every rank.  Returns sd [S][R][T][2]."""
+    import torch
+    import torch.distributed as dist
+    sd = gpu.schwinger_dyson()
+    if world_size > 1:
+        dev = getattr(gpu, "device", "cpu") if dist.get_backend() == "nccl" else "cpu"
+        t = torch.from_numpy(sd).to(dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        sd = t.cpu().numpy()
+    return sd
+
+
 def init_process_group(backend, world_size):
     """Joins the torchrun rendezvous (MASTER_ADDR / MASTER_PORT from the environment) when world_size > 1."""
     import torch.distributed as dist

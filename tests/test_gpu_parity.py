@@ -639,6 +639,11 @@ def test_temperature_slot_shards_reproduce_the_single_context(sg, L, S, R, T, W,
         assert all(((pp[0] == 0) | (pp[0] == qc0_x)).all() for pp in parts)
     if L > 2:
         assert np.abs(qc0).max() > 1e-5
+    # Schwinger-Dyson monitor (Eq. (A6)): each shard reports the temperatures it holds, zeros elsewhere; their sum is the whole chain's
+    sd_w = whole.schwinger_dyson()
+    sd_parts = [g.schwinger_dyson() for g in shards]
+    assert sd_parts[0].shape == sd_w.shape and np.abs(sum(sd_parts) - sd_w).max() <= 1e-12
+    assert all(((pp == 0) | (pp == sd_w)).all() for pp in sd_parts) and np.abs(sd_w).min() > 0
     # one shard alone through the orchestration (world size 1 path of multi.pt_step_sharded on a whole-chain context)
     solo = sg.SpinGlass(L, S, R, T, betas, seed=91, first_sample=2)
     solo.tune(sg.TUNE_SWEEP_IMPL, impl)

@@ -150,6 +150,11 @@ class _FakeSlotShard:
         qk[:, own] = q0[:, own, None, None]
         return q0, qk
 
+    def schwinger_dyson(self):
+        sd = np.zeros((self.S, self.R, self.Tt, 2))
+        sd[:, :, self.first_slot:self.first_slot + self.T] = 1.0 + self.rank      # the temperatures held, zeros elsewhere
+        return sd
+
     def export_chirality(self, r):
         return 100.0 * self.export_replica(r)                                 # 100 (1 + r) at the temperatures held, zeros elsewhere
 
@@ -167,7 +172,8 @@ def _slot_worker(rank, world, port, out):
     gathered = multi.unit_sharded(shard, 3, world)
     q0, qk = multi.overlaps_sharded(shard, world)
     qc0, qck = multi.overlaps_sharded(shard, world, chirality=True)
-    out.put((rank, shard.calls, gathered.tolist(), shard.swapped_with.tolist(), q0.tolist(), qk.shape, qc0.tolist(), qck.shape))
+    sd = multi.schwinger_dyson_sharded(shard, world)
+    out.put((rank, shard.calls, gathered.tolist(), shard.swapped_with.tolist(), q0.tolist(), qk.shape, qc0.tolist(), qck.shape, sd[0, 0, :, 0].tolist()))
     multi.barrier()
     import torch.distributed as dist
     dist.destroy_process_group()
@@ -194,6 +200,7 @@ def test_two_rank_gloo_temperature_slot_sharding():
         assert g[4] == [[[0.0 + 2.0] * 6]] * 2 and g[5] == (2, 1, 6, 3, 2)   # pair (0, 1): 10*0 + (1 + 1) at all six temperatures
         # chirality: own zero-padded export of replica 0 (100) x the summed export of replica 1 (200), complete at every temperature
         assert g[6] == [[[[20000.0] * 3] * 6]] * 2 and g[7] == (2, 1, 6, 3, 3, 2)
+        assert g[8] == [1.0, 1.0, 1.0, 2.0, 2.0, 2.0]              # Schwinger-Dyson: every temperature from the rank that holds it
     assert multi.slot_window_of_rank(1, 3, 12) == (4, 4)
     with pytest.raises(ValueError):
         multi.slot_window_of_rank(0, 4, 6)
